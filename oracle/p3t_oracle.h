@@ -1,0 +1,84 @@
+/* oracle/p3t_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of what the P3T regular-force path computes,
+ * written from /root/reference/PAPER.md (Arnold, Baumgardt & Wang, arXiv:2110.11658).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may load it.  It shares no code with the CUDA library under
+ * paper_2110_11658_b200/csrc and neither includes the other.
+ *
+ * Part I   (p3t_oracle_direct.c)  plain definitions: cutoff K/W (eq. 6), pair potential psi,
+ *          direct O(N^2) split sums (eq. 1, 3, 4), brute-force neighbour lists.
+ * Part II  (p3t_oracle_tree.c)    a reference octree, step by step: cube, Morton keys, order,
+ *          canonical topology, moments, sibling-run groups, opening rule, evaluation.
+ *          The paper names only the library (Bonsai) and theta; every
+ *          rule of Part II is a DESIGN.md reading (R-numbers cited at each function).
+ *
+ * Pins: tests/test_oracle_*.py (-m "not gpu").  Unpinned: the opening rule itself (a design
+ * choice; pinned only through theta->0 == direct sum and the direct-sum error bound).
+ */
+#ifndef P3T_ORACLE_H
+#define P3T_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- Part I ---- */
+double p3t_o_W(double x);                                   /* 1 - K(x), eq. 6      */
+double p3t_o_dW(double x);                                  /* polynomial of eq. 7  */
+double p3t_o_psi(double r, double r_out, double r_in);      /* -dpsi/dr = W/r^2, psi(inf) = 0   */
+
+/* Direct sums for nt targets (indices into the n particles; NULL = all, nt = n).
+ * pos_mass: n x {x,y,z,m} fp32.  Outputs (any may be NULL): acc_reg[3nt], phi_reg[nt],
+ * acc_irr[3nt], phi_newt[nt]; returns the number of coincident (r = 0, j != i) pairs seen. */
+int64_t p3t_o_direct(int64_t n, const float* pos_mass, double r_out, double r_in,
+                     int64_t nt, const int64_t* targets,
+                     double* acc_reg, double* phi_reg, double* acc_irr, double* phi_newt);
+
+/* Brute-force neighbour rows for nt targets.  fp32_predicate = 1: the bit-spec predicate
+ * (R10); 0: the fp64 "physics" predicate r_ij < r_out.  counts[nt] is always written;
+ * if indices != NULL rows are written back to back (ascending j) and must hold sum(counts). */
+int64_t p3t_o_neighbours(int64_t n, const float* pos_mass, float r_out, int fp32_predicate,
+                         int64_t nt, const int64_t* targets, int64_t* counts, int32_t* indices);
+
+/* ---- Part II ---- */
+typedef struct p3t_o_tree p3t_o_tree;
+
+p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pos_mass, int key_bits, int nleaf, int ncrit);
+void        p3t_o_tree_free(p3t_o_tree* t);
+
+/* sizes: out[0]=n, [1]=n_nodes, [2]=n_leaves, [3]=max_level, [4]=n_groups, [5]=bits per axis */
+void p3t_o_tree_sizes(const p3t_o_tree* t, int64_t out[6]);
+void p3t_o_tree_cube(const p3t_o_tree* t, float lo[3], float* side);
+void p3t_o_tree_keys(const p3t_o_tree* t, uint64_t* sorted_keys, uint32_t* order);
+/* nodes in breadth-first order, levels ascending, begin ascending inside a level */
+void p3t_o_tree_nodes(const p3t_o_tree* t, int32_t* level, int32_t* begin, int32_t* end,
+                      int32_t* first_child, int32_t* n_child);
+/* fp32-rounded node data: com_m[4], quad[6] (xx,yy,zz,xy,xz,yz; traceless), clo[3], chi[3], delta */
+void p3t_o_tree_moments(const p3t_o_tree* t, float* com_m, float* quad, float* clo, float* chi, float* delta);
+/* unrounded fp64 moments: mass, com[3], quad[6] */
+void p3t_o_tree_moments64(const p3t_o_tree* t, double* mass, double* com, double* quad);
+void p3t_o_tree_groups(const p3t_o_tree* t, int32_t* begin, int32_t* end, float* glo, float* ghi);
+
+/* Tree force for ng groups (ids into the group list; NULL = all).  acc_pot: n x 4 fp64 in
+ * ORIGINAL particle order, only the rows of the targets in those groups are written.
+ * npp/npc (may be NULL): per requested group, particles on the p-p list / cells on the p-c list.
+ * pot_mode 0: regular potential, 1: unsplit Newtonian.  abs_sum (may be NULL): n fp64, per target
+ * the sum over its interactions of |a_ij| (conditioning of the sum; R15). */
+void p3t_o_tree_force(const p3t_o_tree* t, float r_out, float r_in, float theta, int pot_mode,
+                      int64_t ng, const int64_t* group_ids, double* acc_pot,
+                      int64_t* npp, int64_t* npc, double* abs_sum);
+
+/* single particle-cell term (fp64) from fp32 node data: out = {ax, ay, az, phi} */
+void p3t_o_pc_term(const double xi[3], const float com_m[4], const float quad[6], double out[4]);
+/* the fp32 opening test alone (R7): returns 1 = open */
+int  p3t_o_open_test(const float glo[3], const float ghi[3], const float com[3], const float clo[3],
+                     const float chi[3], float l, float delta, float theta, float r_out);
+/* Morton key of integer grid coordinates (x highest) */
+uint64_t p3t_o_interleave(uint32_t gx, uint32_t gy, uint32_t gz, int bits);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

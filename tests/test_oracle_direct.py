@@ -1,0 +1,208 @@
+"""Pins of oracle Part I (plain definitions) against what the paper and the mathematics fix.
+CPU only.  Citations are /root/reference/PAPER.md lines."""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate, special
+
+import oracle
+import workloads
+from conftest import read_golden
+
+R_OUT, R_IN = 0.05, 0.005      # config 1 radii, gamma = 0.1
+
+
+# ---- P1: cutoff polynomial, eq. 6 ----
+def test_W_values_from_eq6():
+    for x, w in read_golden("cutoff_eq6.txt"):
+        assert abs(oracle.W(x) - w) < 5e-7
+        assert abs(oracle.K(x) - (1.0 - w)) < 5e-7
+
+
+def test_W_limits_symmetry_and_regions():
+    assert oracle.W(0.0) == 0.0 and oracle.W(1.0) == 1.0 and oracle.W(0.5) == 0.5
+    assert oracle.W(-3.0) == 0.0 and oracle.W(7.0) == 1.0          # eq. 6 outer branches
+    xs = np.linspace(0.0, 1.0, 257)
+    w = np.array([oracle.W(x) for x in xs])
+    assert np.all(np.diff(w) >= 0.0)
+    assert np.allclose(w + w[::-1], 1.0, atol=1e-14)                # W(x) + W(1-x) = 1
+
+
+def test_W_is_regularised_incomplete_beta():
+    # 140 x^3 (1-x)^3 is the Beta(4,4) density => W = I_x(4,4)  (library special case)
+    for x in np.linspace(0.01, 0.99, 41):
+        assert abs(oracle.W(x) - special.betainc(4, 4, x)) < 1e-13
+
+
+def test_dW_matches_eq7_polynomial_and_smooth_joins():
+    h = 1e-5
+    for x in np.linspace(0.05, 0.95, 19):
+        assert abs(oracle.dW(x) - 140 * x ** 3 * (1 - x) ** 3) < 1e-12          # eq. 7
+        assert abs((oracle.W(x + h) - oracle.W(x - h)) / (2 * h) - oracle.dW(x)) < 1e-8
+    # C^3 joins: W ~ 35 x^4 at 0 and 1 - 35 (1-x)^4 at 1
+    e = 1e-3
+    assert abs(oracle.W(e) / e ** 4 - 35.0) < 0.1
+    assert abs((1.0 - oracle.W(1 - e)) / e ** 4 - 35.0) < 0.1
+
+
+# ---- P6: pair potential ----
+def test_psi_equals_quadrature_of_W_over_s2():
+    D = R_OUT - R_IN
+    for r in [0.0051, 0.01, 0.02, 0.03, 0.045, 0.0499]:
+        val, _ = integrate.quad(lambda s: oracle.W((s - R_IN) / D) / s ** 2, r, R_OUT, epsabs=1e-13, epsrel=1e-13)
+        assert abs(oracle.psi(r, R_OUT, R_IN) - (-1.0 / R_OUT - val)) < 1e-10 / R_OUT
+
+
+def test_psi_derivative_limits_and_constant():
+    D = R_OUT - R_IN
+    for r in [0.006, 0.0123, 0.027, 0.04, 0.049]:
+        h = 1e-7
+        dpsi = (oracle.psi(r + h, R_OUT, R_IN) - oracle.psi(r - h, R_OUT, R_IN)) / (2 * h)
+        assert abs(dpsi - oracle.W((r - R_IN) / D) / r ** 2) < 1e-5 / r ** 2 * 1e-2
+    assert oracle.psi(R_OUT, R_OUT, R_IN) == pytest.approx(-1.0 / R_OUT, rel=1e-14)
+    assert oracle.psi(2.0, R_OUT, R_IN) == -0.5
+    # inside r_in the regular force is zero, psi is the constant psi(r_in); it depends only on gamma
+    a = oracle.psi(0.5 * R_IN, R_OUT, R_IN) * R_OUT
+    b = oracle.psi(0.001, 0.7, 0.07) * 0.7
+    assert a == pytest.approx(b, rel=1e-13)
+    val, _ = integrate.quad(lambda y: special.betainc(4, 4, (y - 0.1) / 0.9) / y ** 2, 0.1, 1.0, epsabs=1e-12, epsrel=1e-12)
+    assert a == pytest.approx(-1.0 - val, rel=1e-12)
+
+
+# ---- P2: two bodies in each radial zone, sign reading R1 ----
+@pytest.mark.parametrize("r", [0.5 * R_IN, R_IN, 0.3 * R_OUT, 0.0275, 0.9 * R_OUT, R_OUT, 3 * R_OUT])
+def test_two_body_zones(r):
+    m2 = 0.37
+    pm = np.array([[0.1, -0.2, 0.3, 0.63], [0.1 + r * 0.6, -0.2, 0.3 + r * 0.8, m2]], dtype=np.float32)
+    rr = float(np.linalg.norm(pm[1, :3].astype(np.float64) - pm[0, :3].astype(np.float64)))
+    m2 = float(pm[1, 3])
+    d = oracle.direct(pm, R_OUT, R_IN)
+    x = (rr - R_IN) / (R_OUT - R_IN)
+    w = 0.0 if x <= 0 else 1.0 if x >= 1 else float(special.betainc(4, 4, x))
+    unit = (pm[1, :3].astype(np.float64) - pm[0, :3].astype(np.float64)) / rr       # toward the partner
+    tol = 1e-13 * m2 / rr ** 2                            # 1 - W cancels near x = 1: absolute bound
+    assert np.allclose(d["acc_reg"][0], m2 * w / rr ** 2 * unit, rtol=0, atol=tol)
+    assert np.allclose(d["acc_irr"][0], m2 * (1 - w) / rr ** 2 * unit, rtol=0, atol=tol)
+    assert d["phi_newt"][0] == pytest.approx(-m2 / rr, rel=1e-14)
+    if x >= 1:
+        assert d["phi_reg"][0] == pytest.approx(-m2 / rr, rel=1e-14)
+    if x <= 0:
+        assert np.all(d["acc_reg"][0] == 0.0)
+
+
+def _newton_numpy(pm):
+    p = pm[:, :3].astype(np.float64); m = pm[:, 3].astype(np.float64)
+    d = p[None, :, :] - p[:, None, :]                     # x_j - x_i
+    r2 = (d ** 2).sum(-1)
+    np.fill_diagonal(r2, np.inf)
+    acc = (m[None, :, None] * d / r2[..., None] ** 1.5).sum(1)
+    phi = -(m[None, :] / np.sqrt(r2)).sum(1)
+    return acc, phi
+
+
+# ---- P3 / P4: F_I + F_R = Newton (eq. 3); momentum ----
+def test_split_sums_to_newton_and_momentum():
+    pm = workloads.make_config(1, n_override=1500).pos_mass
+    pm[:, :3] *= 0.08                                      # shrink so that many pairs fall inside r_out
+    d = oracle.direct(pm, R_OUT, R_IN)
+    acc, phi = _newton_numpy(pm)
+    assert np.abs(d["acc_reg"] + d["acc_irr"] - acc).max() < 1e-12 * np.abs(acc).max()
+    assert np.abs(d["phi_newt"] - phi).max() < 1e-12 * np.abs(phi).max()
+    assert np.linalg.norm(d["acc_irr"], axis=1).max() > 0          # the test does exercise the cutoff zone
+    m = pm[:, 3].astype(np.float64)
+    scale = (m[:, None] * np.abs(d["acc_reg"])).sum()
+    assert np.abs((m[:, None] * d["acc_reg"]).sum(0)).max() < 1e-13 * scale      # pair antisymmetry
+    assert np.abs((m[:, None] * d["acc_irr"]).sum(0)).max() < 1e-13 * (m[:, None] * np.abs(d["acc_irr"])).sum()
+    # targets subset == rows of the full result
+    tg = np.array([3, 77, 1499], dtype=np.int64)
+    s = oracle.direct(pm, R_OUT, R_IN, targets=tg)
+    assert np.array_equal(s["acc_reg"], d["acc_reg"][tg]) and np.array_equal(s["phi_reg"], d["phi_reg"][tg])
+
+
+# ---- P5: uniform shell (Newton's shell theorem) ----
+def test_uniform_shell():
+    n = 20000
+    k = np.arange(n) + 0.5
+    cz = 1 - 2 * k / n
+    az = math.pi * (1 + 5 ** 0.5) * k
+    s = np.sqrt(1 - cz * cz)
+    R = 2.0
+    pm = np.zeros((n + 2, 4), dtype=np.float32)
+    pm[:n, 0] = R * s * np.cos(az); pm[:n, 1] = R * s * np.sin(az); pm[:n, 2] = R * cz; pm[:n, 3] = 1.0 / n
+    pm[n] = [0.3, -0.2, 0.4, 1e-30]           # interior test point (negligible mass)
+    pm[n + 1] = [3.0, 4.0, 0.0, 1e-30]        # exterior, r = 5
+    d = oracle.direct(pm, R_OUT, R_IN, targets=np.array([n, n + 1], dtype=np.int64))
+    assert np.linalg.norm(d["acc_reg"][0]) < 2e-3 * (1.0 / R ** 2)
+    expect = -np.array([3.0, 4.0, 0.0]) / 5.0 * (1.0 / 25.0)
+    assert np.allclose(d["acc_reg"][1], expect, atol=2e-4 / 25.0)
+    assert d["phi_reg"][0] == pytest.approx(-1.0 / R, rel=1e-3)
+
+
+# ---- P7: Plummer analytic potential ----
+def test_plummer_potential():
+    w = workloads.make_config(1)
+    tg = workloads.sample_targets(w.n, 512)
+    d = oracle.direct(w.pos_mass, w.r_out, w.r_in, targets=tg)
+    a = workloads.PLUMMER_A
+    rt = workloads.PLUMMER_TRUNC * a
+    r = np.linalg.norm(w.pos_mass[tg, :3].astype(np.float64), axis=1)
+    mt = (rt / a) ** 3 / (1 + (rt / a) ** 2) ** 1.5
+    phi_p = lambda x: -1.0 / np.sqrt(x * x + a * a)
+    expect = (phi_p(r) - phi_p(rt) - mt / rt) / mt
+    rel = (d["phi_newt"] - expect) / expect
+    assert abs(np.mean(rel)) < 5e-3 and np.abs(rel).max() < 5e-2
+
+
+# ---- P9 / P10: neighbour lists ----
+def test_neighbour_sets_small():
+    pm = workloads.make_config(1, n_override=3000).pos_mass
+    pm[:, :3] *= 0.25
+    off, idx = oracle.neighbours(pm, R_OUT)
+    off64, idx64 = oracle.neighbours(pm, R_OUT, fp32_predicate=False)
+    p = pm[:, :3].astype(np.float64)
+    d = np.sqrt(((p[:, None, :] - p[None, :, :]) ** 2).sum(-1))
+    member = d < float(np.float32(R_OUT))
+    np.fill_diagonal(member, False)
+    rows = [np.nonzero(member[i])[0] for i in range(len(p))]
+    assert off64[-1] == sum(len(r) for r in rows) and off64[-1] > 2000
+    for i in range(len(p)):
+        assert np.array_equal(idx64[off64[i]:off64[i + 1]], rows[i])
+    # the fp32 bit-spec predicate may differ from the fp64 one only for pairs within rounding of r_out
+    s32 = {(i, int(j)) for i in range(len(p)) for j in idx[off[i]:off[i + 1]]}
+    s64 = {(i, int(j)) for i in range(len(p)) for j in idx64[off64[i]:off64[i + 1]]}
+    for (i, j) in s32 ^ s64:
+        assert abs(d[i, j] / R_OUT - 1.0) < 1e-6
+    assert len(s32 ^ s64) <= 4
+    for (i, j) in s32:                                           # symmetric, no self, ascending rows
+        assert (j, i) in s32 and i != j
+    for i in range(len(p)):
+        assert np.all(np.diff(idx[off[i]:off[i + 1]]) > 0)
+
+
+def test_neighbour_statistics_plummer(cfg1):
+    off, idx = oracle.neighbours(cfg1.pos_mass, cfg1.r_out)
+    mean = off[-1] / cfg1.n
+    # uniform-density estimate: N (r_out/a)^3 15 pi/256 * (1/mt correction) -- "usually < 1" for the paper's
+    # r_cut = 4 tau; BASELINE.json's 0.05 prefactor gives 1.84
+    est = cfg1.n * (cfg1.r_out / workloads.PLUMMER_A) ** 3 * 15 * math.pi / 256
+    assert est == pytest.approx(1.84, abs=0.01)
+    assert mean == pytest.approx(est, rel=0.08)
+    assert off[-1] % 2 == 0
+    tg = np.array([0, 5, 16383], dtype=np.int64)
+    o2, i2 = oracle.neighbours(cfg1.pos_mass, cfg1.r_out, targets=tg)
+    for k, t in enumerate(tg):
+        assert np.array_equal(i2[o2[k]:o2[k + 1]], idx[off[t]:off[t + 1]])
+    # the paper's own radius r_cut = 4 tau = 1/32 at N = 2^14 (eq. 21-22): mean count < 1
+    off_p, _ = oracle.neighbours(cfg1.pos_mass, 1.0 / 32.0)
+    assert off_p[-1] / cfg1.n < 1.0
+
+
+def test_coincident_pair_reading_R8():
+    pm = np.array([[0, 0, 0, 0.5], [0, 0, 0, 0.25], [1, 0, 0, 0.25]], dtype=np.float32)
+    d = oracle.direct(pm, R_OUT, R_IN)
+    assert d["coincident"] == 2
+    assert np.allclose(d["acc_reg"][0], [0.25, 0, 0]) and np.all(d["acc_irr"][0] == 0)
+    assert d["phi_reg"][0] == pytest.approx(0.25 * oracle.psi(0.0, R_OUT, R_IN) - 0.25)
+    off, idx = oracle.neighbours(pm, R_OUT)
+    assert list(idx[off[0]:off[1]]) == [1] and list(idx[off[1]:off[2]]) == [0] and off[3] == off[2]

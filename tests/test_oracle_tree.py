@@ -1,0 +1,275 @@
+"""Pins of oracle Part II (reference octree).  CPU only.  The paper fixes only theta and the library
+name; the rules are DESIGN.md readings R-S1..R-S8, pinned here by hand cases, brute
+force on small inputs, invariants and the two limits the paper does state: theta -> 0 is the direct sum
+ and the force equals eq. 3's direct sum within the north-star error bound."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+NLEAF, NCRIT = 16, 64
+
+
+def _small(n=3000, seed_cfg=1, scale=1.0):
+    pm = workloads.make_config(seed_cfg, n_override=n).pos_mass
+    pm[:, :3] *= scale
+    return pm
+
+
+# ---- P11: keys ----
+def test_interleave_hand_cases():
+    assert oracle.interleave(1, 0, 0, 21) == 4 and oracle.interleave(0, 1, 0, 21) == 2 and oracle.interleave(0, 0, 1, 21) == 1
+    assert oracle.interleave(2, 0, 0, 21) == 32 and oracle.interleave(3, 5, 6, 10) == 0b011_101_110 and True
+    assert oracle.interleave(2 ** 21 - 1, 2 ** 21 - 1, 2 ** 21 - 1, 21) == 2 ** 63 - 1
+    assert oracle.interleave(2 ** 10 - 1, 2 ** 10 - 1, 2 ** 10 - 1, 10) == 2 ** 30 - 1
+
+
+def test_interleave_bit_pattern():
+    # x = 0b011, y = 0b101, z = 0b110: digit k = (x_k, y_k, z_k); k=0: (1,1,0)=6, k=1: (1,0,1)=5, k=2: (0,1,1)=3
+    assert oracle.interleave(0b011, 0b101, 0b110, 3) == (3 << 6) | (5 << 3) | 6
+
+
+@pytest.mark.parametrize("bits", [63, 30])
+def test_cube_keys_order_bruteforce(bits):
+    pm = _small(2500)
+    t = oracle.Tree(pm, bits, NLEAF, NCRIT)
+    lo, side = t.cube()
+    keys, order = t.keys()
+    p = pm[:, :3]
+    assert np.array_equal(lo, p.min(0))
+    ext = float((p.max(0) - p.min(0)).max())
+    assert side > ext and side / 2 <= ext and np.log2(side) == round(np.log2(side))
+    B = bits // 3
+    # grid coordinates straight from the definition, in exact arithmetic on the fp32 subtraction result
+    d = (p - lo).astype(np.float32).astype(np.float64)
+    g = np.minimum(np.floor(d * (2.0 ** B / side)).astype(np.int64), 2 ** B - 1)
+    k_ref = np.array([oracle.interleave(int(a), int(b), int(c), B) for a, b, c in g], dtype=np.uint64)
+    assert np.array_equal(keys, k_ref[order])
+    assert np.all(np.diff(keys.astype(np.float64)) >= 0) and np.all(keys[1:] >= keys[:-1])
+    assert sorted(order.tolist()) == list(range(len(p)))
+    tie = keys[1:] == keys[:-1]
+    assert np.all(order[1:][tie] > order[:-1][tie])             # ties by original index
+    assert keys[np.nonzero(order == int(np.argmin(p[:, 0])))[0][0]] >> np.uint64(3 * B - 1) == 0
+    # particle sitting at the cube corner has key 0
+    pm2 = pm.copy(); pm2[7, :3] = lo
+    t2 = oracle.Tree(pm2, bits, NLEAF, NCRIT); k2, o2 = t2.keys()
+    assert k2[0] == 0 and o2[0] == 7
+
+
+# ---- topology (R-S4) by brute force ----
+@pytest.mark.parametrize("bits,nleaf", [(63, 16), (30, 4), (63, 1)])
+def test_topology_bruteforce(bits, nleaf):
+    pm = _small(1200 if nleaf > 1 else 300)
+    t = oracle.Tree(pm, bits, nleaf, max(NCRIT, nleaf))
+    nd = t.nodes(); keys, order = t.keys(); lo, side = t.cube()
+    B = bits // 3
+    assert nd["level"][0] == 0 and nd["begin"][0] == 0 and nd["end"][0] == len(pm)
+    p_sorted = pm[order, :3]
+    seen = set()
+    for k in range(t.n_nodes):
+        lev, b, e = int(nd["level"][k]), int(nd["begin"][k]), int(nd["end"][k])
+        assert e > b
+        seen.add((lev, b, e))
+        # all particles of the node share the 3*lev-bit prefix, and nobody outside the range does
+        sh = np.uint64(3 * (B - lev))
+        pre = keys[b] >> sh
+        assert np.all(keys[b:e] >> sh == pre)
+        if b > 0:
+            assert keys[b - 1] >> sh != pre
+        if e < len(pm):
+            assert keys[e] >> sh != pre
+        # geometric meaning: same cell of edge side/2^lev
+        l = side / 2 ** lev
+        cell = np.floor((p_sorted[b:e] - lo).astype(np.float32).astype(np.float64) / l)
+        assert np.all(cell == cell[0]) or lev == 0
+        internal = (e - b > nleaf) and lev < B
+        if internal:
+            fc, nc = int(nd["first_child"][k]), int(nd["n_child"][k])
+            assert 1 <= nc <= 8
+            assert nd["begin"][fc] == b and nd["end"][fc + nc - 1] == e
+            assert np.all(nd["level"][fc:fc + nc] == lev + 1)
+            assert np.all(nd["begin"][fc + 1:fc + nc] == nd["end"][fc:fc + nc - 1])
+            digits = [int((keys[nd["begin"][c]] >> np.uint64(3 * (B - lev - 1))) & np.uint64(7)) for c in range(fc, fc + nc)]
+            assert digits == sorted(set(digits))
+        else:
+            assert nd["n_child"][k] == 0
+    assert len(seen) == t.n_nodes
+    assert np.all(np.diff(nd["level"]) >= 0)                    # breadth-first
+    assert t.n_leaves == int((nd["n_child"] == 0).sum()) and t.max_level == nd["level"].max()
+    leaves = nd["n_child"] == 0
+    assert (nd["end"][leaves] - nd["begin"][leaves]).sum() == len(pm)      # leaves partition the particles
+
+
+def test_degenerate_inputs():
+    one = np.array([[1.0, 2.0, 3.0, 1.0]], dtype=np.float32)
+    t = oracle.Tree(one, 63, NLEAF, NCRIT)
+    assert t.n_nodes == 1 and t.n_groups == 1 and t.cube()[1] == 1.0
+    f = t.force(0.05, 0.005, 0.4)
+    assert np.all(f["acc_pot"][0] == 0.0)
+    same = np.tile(np.array([[0.5, 0.5, 0.5, 0.01]], dtype=np.float32), (100, 1))
+    t = oracle.Tree(same, 63, NLEAF, NCRIT)
+    nd = t.nodes()
+    assert t.max_level == 21 and t.n_nodes == 22                 # a chain down to the deepest level
+    g = t.groups()
+    assert list(g["end"] - g["begin"]) == [64, 36]              # over-full deepest leaf cut into runs of NCRIT
+    f = t.force(0.05, 0.005, 0.4)
+    assert np.all(f["acc_pot"][:, :3] == 0.0)
+    assert np.allclose(f["acc_pot"][:, 3], 99 * 0.01 * oracle.psi(0.0, float(np.float32(0.05)), float(np.float32(0.005))), rtol=1e-6)
+
+
+# ---- P12: moments ----
+def test_moments_root_and_parallel_axis():
+    pm = _small(4000, seed_cfg=2)
+    t = oracle.Tree(pm, 63, NLEAF, NCRIT)
+    nd = t.nodes(); m64 = t.moments64(); mo = t.moments(); keys, order = t.keys()
+    ps = pm[order].astype(np.float64)
+    M = ps[:, 3].sum()
+    com = (ps[:, 3:4] * ps[:, :3]).sum(0) / M
+    assert m64["mass"][0] == pytest.approx(M, rel=1e-14) and np.allclose(m64["com"][0], com, rtol=0, atol=1e-14)
+    d = ps[:, :3] - com
+    q_ref = np.einsum("i,ia,ib->ab", ps[:, 3], d, d) * 3 - np.eye(3) * (ps[:, 3] * (d ** 2).sum(1)).sum()
+    q = m64["quad"][0]
+    assert np.allclose([q[0], q[1], q[2], q[3], q[4], q[5]],
+                       [q_ref[0, 0], q_ref[1, 1], q_ref[2, 2], q_ref[0, 1], q_ref[0, 2], q_ref[1, 2]], rtol=1e-12, atol=1e-16)
+    assert abs(q[0] + q[1] + q[2]) < 1e-14 * np.abs(q).max()    # traceless
+    for k in np.nonzero(nd["n_child"] > 0)[0][:200]:
+        ch = np.arange(nd["first_child"][k], nd["first_child"][k] + nd["n_child"][k])
+        Mk = m64["mass"][ch].sum()
+        ck = (m64["mass"][ch, None] * m64["com"][ch]).sum(0) / Mk
+        assert m64["mass"][k] == pytest.approx(Mk, rel=1e-13) and np.allclose(m64["com"][k], ck, rtol=0, atol=1e-13)
+        qq = np.zeros(6)
+        for c in ch:
+            s = m64["com"][c] - ck
+            s2 = (s ** 2).sum()
+            shift = np.array([3 * s[0] ** 2 - s2, 3 * s[1] ** 2 - s2, 3 * s[2] ** 2 - s2, 3 * s[0] * s[1], 3 * s[0] * s[2], 3 * s[1] * s[2]])
+            qq += m64["quad"][c] + m64["mass"][c] * shift
+        assert np.allclose(m64["quad"][k], qq, rtol=1e-10, atol=1e-12 * np.abs(qq).max() + 1e-30)
+    # fp32 node data are the fp64 values rounded once; boxes are exact min/max
+    assert np.array_equal(mo["com_m"][:, :3], m64["com"].astype(np.float32)) and np.array_equal(mo["com_m"][:, 3], m64["mass"].astype(np.float32))
+    for k in [0, 1, t.n_nodes // 2, t.n_nodes - 1]:
+        b, e = nd["begin"][k], nd["end"][k]
+        assert np.array_equal(mo["clo"][k], pm[order[b:e], :3].min(0)) and np.array_equal(mo["chi"][k], pm[order[b:e], :3].max(0))
+    # delta = |COM - geometric centre| <= half diagonal of the cell
+    lo, side = t.cube()
+    l = side / 2.0 ** nd["level"]
+    assert np.all(mo["delta"] <= 0.8661 * l)
+    assert mo["delta"][0] == pytest.approx(np.linalg.norm(com - (lo + 0.5 * side)), rel=1e-6)
+
+
+# ---- groups (R-S5) ----
+@pytest.mark.parametrize("ncrit", [16, 32, 64])
+def test_groups_partition_and_rule(ncrit):
+    pm = _small(5000, seed_cfg=2)
+    t = oracle.Tree(pm, 63, NLEAF, ncrit)
+    g = t.groups(); nd = t.nodes(); keys, order = t.keys()
+    assert g["begin"][0] == 0 and g["end"][-1] == len(pm) and np.array_equal(g["begin"][1:], g["end"][:-1])
+    cnt = g["end"] - g["begin"]
+    assert cnt.min() >= 1 and cnt.max() <= ncrit
+    # every group is a run of consecutive children of ONE node with count > ncrit, each child <= ncrit,
+    # and two neighbouring runs under the same parent cannot be merged (greedy)
+    node_of = {(int(b), int(e)): k for k, (b, e) in enumerate(zip(nd["begin"], nd["end"]))}
+    starts = {}
+    for k in range(t.n_nodes):
+        for c in range(nd["first_child"][k], nd["first_child"][k] + nd["n_child"][k]):
+            starts.setdefault(int(nd["begin"][c]), []).append((k, c))
+    for b, e in zip(g["begin"], g["end"]):
+        ok = False
+        for parent, c in starts[int(b)]:
+            if nd["end"][parent] - nd["begin"][parent] <= ncrit:
+                continue
+            cc = c
+            while cc < nd["first_child"][parent] + nd["n_child"][parent] and nd["end"][cc] < e:
+                cc += 1
+            if cc < nd["first_child"][parent] + nd["n_child"][parent] and nd["end"][cc] == e and \
+                    all(nd["end"][x] - nd["begin"][x] <= ncrit for x in range(c, cc + 1)):
+                ok = True
+        assert ok
+    for q in range(0, t.n_groups, 37):
+        b, e = g["begin"][q], g["end"][q]
+        assert np.array_equal(g["glo"][q], pm[order[b:e], :3].min(0)) and np.array_equal(g["ghi"][q], pm[order[b:e], :3].max(0))
+    # n <= ncrit: one group
+    t1 = oracle.Tree(pm[:ncrit], 63, NLEAF, ncrit)
+    assert t1.n_groups == 1
+
+
+# ---- opening rule (R-S7) hand cases; "parity unpinned" beyond these and the two limits below ----
+def test_open_test_hand_cases():
+    glo, ghi = [0, 0, 0], [1, 1, 1]
+    far = dict(com=[11, 0.5, 0.5], clo=[10.5, 0, 0], chi=[11.5, 1, 1])
+    # distance box->COM = 10; l = 1, theta = 0.4, delta = 0: r_crit = 2.5 -> accepted
+    assert not oracle.open_test(glo, ghi, far["com"], far["clo"], far["chi"], 1.0, 0.0, 0.4, 0.05)
+    # l = 4: r_crit = 10 -> d2 = 100 is not < 100 -> accepted; delta pushes it over
+    assert not oracle.open_test(glo, ghi, far["com"], far["clo"], far["chi"], 4.0, 0.0, 0.4, 0.05)
+    assert oracle.open_test(glo, ghi, far["com"], far["clo"], far["chi"], 4.0, 0.01, 0.4, 0.05)
+    # tiny theta opens everything (theta = 0 is the direct sum)
+    assert oracle.open_test(glo, ghi, far["com"], far["clo"], far["chi"], 1.0, 0.0, 1e-3, 0.05)
+    # second clause: a tiny far cell whose box comes within r_out of the group box must open
+    near = dict(com=[1.2, 0.5, 0.5], clo=[1.04, 0.5, 0.5], chi=[1.3, 0.5, 0.5])
+    assert oracle.open_test(glo, ghi, near["com"], near["clo"], near["chi"], 1e-3, 0.0, 0.4, 0.05)
+    near["clo"] = [1.06, 0.5, 0.5]
+    assert not oracle.open_test(glo, ghi, near["com"], near["clo"], near["chi"], 1e-3, 0.0, 0.4, 0.05)
+    # COM inside the group box: distance 0 -> always open
+    assert oracle.open_test(glo, ghi, [0.5, 0.5, 0.5], [0.4, 0.4, 0.4], [0.6, 0.6, 0.6], 1e-6, 0.0, 0.4, 0.0)
+
+
+# ---- R-S8: particle-cell term ----
+def test_pc_term_axis_closed_form_and_convergence():
+    m, s, R = 0.25, 0.0078125, 1.5          # exactly representable in fp32
+    # two equal masses at +-s on z: Qzz = 4 m s^2, Qxx = Qyy = -2 m s^2; on axis phi_Q = -2 m s^2 / R^3
+    com_m = [0, 0, 0, 2 * m]; quad = [-2 * m * s * s, -2 * m * s * s, 4 * m * s * s, 0, 0, 0]
+    o = oracle.pc_term([0, 0, R], com_m, quad)
+    exact_phi = -m / (R - s) - m / (R + s)
+    exact_az = -m / (R - s) ** 2 - m / (R + s) ** 2
+    assert o[3] + 2 * m / R == pytest.approx(-2 * m * s * s / R ** 3, rel=1e-5)
+    assert o[3] == pytest.approx(exact_phi, rel=1e-7) and o[2] == pytest.approx(exact_az, rel=1e-6)
+    # random cluster: the error of monopole+quadrupole falls like (size/R)^3 relative to the monopole
+    rng = np.random.default_rng(5)
+    pts = rng.normal(size=(40, 3)); mass = rng.uniform(0.5, 1.5, 40)
+    errs = []
+    for size in (0.08, 0.04, 0.02):
+        p = (pts * size).astype(np.float32).astype(np.float64)
+        M = mass.sum(); c = (mass[:, None] * p).sum(0) / M; d = p - c
+        q = 3 * np.einsum("i,ia,ib->ab", mass, d, d) - np.eye(3) * (mass * (d ** 2).sum(1)).sum()
+        x = np.array([1.0, -0.7, 0.4])
+        o = oracle.pc_term(x, [*c, M], [q[0, 0], q[1, 1], q[2, 2], q[0, 1], q[0, 2], q[1, 2]])
+        dd = p - x; r = np.linalg.norm(dd, axis=1)
+        a_exact = (mass[:, None] * dd / r[:, None] ** 3).sum(0); phi_exact = -(mass / r).sum()
+        errs.append((np.linalg.norm(o[:3] - a_exact) / np.linalg.norm(a_exact), abs(o[3] - phi_exact) / abs(phi_exact)))
+    for k in range(2):
+        assert 6.0 < errs[k][0] / errs[k + 1][0] < 10.5 and 6.0 < errs[k][1] / errs[k + 1][1] < 10.5
+    assert errs[0][0] < 2e-3
+
+
+# ---- P8: theta -> 0 is the direct sum ----
+@pytest.mark.parametrize("bits", [63, 30])
+def test_tree_theta_to_zero_is_direct_sum(bits):
+    pm = _small(2048, scale=0.3)
+    t = oracle.Tree(pm, bits, NLEAF, NCRIT)
+    for mode, key in ((0, "phi_reg"), (1, "phi_newt")):
+        f = t.force(0.05, 0.005, 1e-3, pot_mode=mode)
+        d = oracle.direct(pm, float(np.float32(0.05)), float(np.float32(0.005)))
+        assert np.all(f["npc"] == 0) and np.all(f["npp"] == len(pm))
+        err = np.linalg.norm(f["acc_pot"][:, :3] - d["acc_reg"], axis=1) / np.linalg.norm(d["acc_reg"], axis=1)
+        assert err.max() < 1e-11
+        assert np.abs(f["acc_pot"][:, 3] / d[key] - 1).max() < 1e-12
+
+
+# ---- north-star bound: tree vs eq. 3 direct sum at theta = 0.4 ----
+def test_tree_vs_direct_error_bound(cfg1):
+    t = oracle.Tree(cfg1.pos_mass, 63, NLEAF, NCRIT)
+    f = t.force(cfg1.r_out, cfg1.r_in, 0.4, want_abs=True)
+    d = oracle.direct(cfg1.pos_mass, cfg1.r_out, cfg1.r_in)
+    err = np.linalg.norm(f["acc_pot"][:, :3] - d["acc_reg"], axis=1) / np.linalg.norm(d["acc_reg"], axis=1)
+    assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2
+    assert np.median(err) < 2e-4                                # what monopole+quadrupole at 0.4 actually gives
+    assert np.abs(f["acc_pot"][:, 3] / d["phi_reg"] - 1).max() < 1e-3
+    assert np.all(f["abs_sum"] >= np.linalg.norm(f["acc_pot"][:, :3], axis=1) * (1 - 1e-12))
+    # a monopole-only evaluation (quadrupole zeroed) must be clearly worse: the quadrupole term is live
+    g = t.groups(); cnt = g["end"] - g["begin"]
+    assert (f["npc"] * cnt).sum() / cfg1.n > 500 and (f["npp"] * cnt).sum() / cfg1.n > 500
+    # subset of groups fills only their rows
+    sub = t.force(cfg1.r_out, cfg1.r_in, 0.4, group_ids=np.array([0, 5], dtype=np.int64))
+    filled = ~np.isnan(sub["acc_pot"][:, 0])
+    assert filled.sum() == cnt[0] + cnt[5]
+    assert np.array_equal(sub["acc_pot"][filled], f["acc_pot"][filled])
