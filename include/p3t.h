@@ -1,0 +1,146 @@
+/* include/p3t.h -- C-ABI of the B200-native P3T regular-force library (libp3t.so).
+ *
+ * The library computes the data-parallel hot path of NBODY6+P3T (Arnold, Baumgardt & Wang,
+ * arXiv:2110.11658; citations are /root/reference/PAPER.md:<line>): for every particle i
+ *
+ *     F_R,i = sum_{j != i} m_j (x_j - x_i) / |r_ij|^3 * (1 - K_ij)          (eq. 1, 3, 4)
+ *
+ * with the 7th-order cutoff K(x), x = (r - r_in)/(r_out - r_in) (eq. 6, 8-10; PAPER.md:52-66;
+ * the paper's r_cut is called r_out here), evaluated with a Barnes-Hut octree with opening angle
+ * theta, together with each particle's neighbour list { j != i : r_ij < r_out }
+ * that the CPU Hermite/KS side consumes.  G = 1.
+ * The readings taken where the paper is silent (sign of eq. 4, potential, opening rule, ...) are
+ * listed in DESIGN.md (R-numbers).
+ *
+ * Conventions
+ *  - Every call returns P3T_OK (0) or a negative error code; no exceptions, no exit, no stdout.
+ *  - "DEVICE pointer": memory of the context's CUDA device.  "HOST pointer": ordinary host memory
+ *    (pinned or pageable).  "ANY pointer": either one (copied with cudaMemcpyDefault).
+ *  - Calls enqueue work on the context's stream and do NOT synchronise unless stated.
+ *  - The library never frees caller memory and writes only to the output arguments named below.
+ *  - One context per host thread; a context is bound to one device and one stream.
+ *  - Every step runs in the library's CUDA kernels; there is no CPU fallback.
+ */
+#ifndef P3T_H
+#define P3T_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define P3T_OK       0
+#define P3T_EINVAL  -1   /* bad argument: n < 1, n > P3T_MAX_N, r_in < 0, r_in >= r_out, theta <= 0,
+                            key_bits not 30/63, null pointer, NaN/Inf position or mass (found by
+                            the bounding-cube reduction; reported by the next synchronising call) */
+#define P3T_ESTATE  -2   /* force before build, neighbours before force, ... */
+#define P3T_ENOMEM  -3   /* device allocation failed */
+#define P3T_ECUDA   -4   /* a CUDA call failed; sticky; text via p3t_last_error */
+#define P3T_ERANGE  -5   /* p3t_neighbours_nbody6: a row is longer than lmax */
+
+#define P3T_MAX_N   (1ll << 30)
+#define P3T_MAX_NCRIT 64
+
+typedef struct p3t_ctx p3t_ctx;      /* opaque; owns all device scratch */
+
+/* Sizes and timings of the last build / force call (p3t_get_stats synchronises the stream). */
+typedef struct p3t_stats {
+    int64_t n;               /* particles                                               */
+    int64_t n_nodes;         /* octree cells                                            */
+    int64_t n_leaves;
+    int64_t n_groups;        /* target groups of the walk                               */
+    int32_t max_level;
+    int32_t key_bits;
+    int64_t n_pp;            /* sum over targets of particle-particle terms evaluated   */
+    int64_t n_pc;            /* sum over targets of particle-cell terms evaluated       */
+    int64_t n_pp_list;       /* sum over groups of p-p list lengths                     */
+    int64_t n_pc_list;       /* sum over groups of p-c list lengths                     */
+    int64_t nb_total;        /* neighbour-list entries                                  */
+    int32_t nb_max;          /* longest row                                             */
+    int32_t input_bad;       /* 1 if the last build saw a NaN/Inf position or mass      */
+    float   cube_lo[3];      /* bounding cube (DESIGN.md R-S1)                          */
+    float   cube_side;
+    float   ms_build;        /* CUDA-event time of the last p3t_build_tree (a1-a6)      */
+    float   ms_force;        /* CUDA-event time of the last p3t_regular_force (a7-a11)  */
+    float   ms_walk;         /* ... of its walk+force kernel alone                      */
+    float   ms_sort;         /* ... of the radix sort inside the last build             */
+} p3t_stats;
+
+/* Create a context on CUDA device `device`, enqueuing on `cuda_stream` (a cudaStream_t passed as
+ * void*; NULL = the legacy default stream).  *out is set on success. */
+int p3t_create(p3t_ctx** out, int device, void* cuda_stream);
+int p3t_destroy(p3t_ctx* ctx);
+
+/* Tree parameters (DESIGN.md R-S4/R-S5): a cell with more than nleaf particles is split;
+ * target groups hold at most ncrit particles.  1 <= nleaf <= ncrit <= P3T_MAX_NCRIT.
+ * Defaults 16 / 64.  Takes effect at the next build. */
+int p3t_set_tree_params(p3t_ctx* ctx, int nleaf, int ncrit);
+
+/* Steps a1-a6: bounding cube, Morton keys (key_bits = 30 or 63), stable radix sort,
+ * body permutation, canonical octree, monopole + traceless quadrupole moments, target groups.
+ * pos_mass: DEVICE pointer, n x {x, y, z, m} fp32 (16-byte aligned), caller-owned, read-only;
+ * it is copied (permuted) during the call and need not stay valid afterwards.
+ * The paper names only "the BONSAI library" for this step. */
+int p3t_build_tree(p3t_ctx* ctx, int64_t n, const float* pos_mass, int key_bits);
+
+/* Steps a7-a11: group tree walk, particle-cell and particle-particle regular force with the cutoff
+ * of eq. 6 and neighbour-list emission fused in.
+ * acc_pot: DEVICE pointer, n x {ax, ay, az, phi} fp32, caller-owned, ORIGINAL particle order.
+ * pot_mode 0: phi = regular potential (its gradient is -a; R6); 1: unsplit Newtonian
+ * potential -sum m_j / r_ij.  Requires a prior build; theta, r_out, r_in may change between
+ * calls without a rebuild.  Also produces the neighbour lists returned by p3t_neighbours. */
+int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float* acc_pot);
+
+/* Neighbour lists L(i) = { j != i : r_ij < r_out } of the last
+ * p3t_regular_force, as CSR in ORIGINAL particle ids: offsets[n+1] (int64), indices[total]
+ * (int32, 0-based, every row strictly ascending, self excluded; empty rows are legal,
+ * PAPER.md:113).  The pointers are library-owned DEVICE pointers, valid until the next
+ * force/build/destroy.  Synchronises the stream (total is returned on the host). */
+int p3t_neighbours(p3t_ctx* ctx, const int64_t** offsets, const int32_t** indices, int64_t* total);
+
+/* Same lists copied out: offsets_out[n+1], indices_out[total]: ANY pointers (either may be NULL). */
+int p3t_neighbours_copy(p3t_ctx* ctx, int64_t* offsets_out, int32_t* indices_out);
+
+/* NBODY6-style view "in a format compatible with NBODY6": HOST array
+ * n x (lmax + 1) int32; row i = { count, 1-based ids ascending, zero padding }.
+ * P3T_ERANGE if a row is longer than lmax (nothing is written then). */
+int p3t_neighbours_nbody6(p3t_ctx* ctx, int32_t lmax, int32_t* host_list);
+
+/* One whole regular-force step with HOST buffers (what the host integrator calls once per
+ * dt_reg, steps (i)/(iv) of PAPER.md:89-94): copies pos_mass host->device, builds, evaluates,
+ * and copies acc_pot[n x 4] and the neighbour CSR back.  nb_offsets[n+1] and nb_indices[nb_cap]
+ * may be NULL (lists are then left on the device).  *nb_total receives the entry count; if it
+ * exceeds nb_cap the indices are not copied and P3T_ERANGE is returned.  Synchronises. */
+int p3t_step_host(p3t_ctx* ctx, int64_t n, const float* pos_mass_host, int key_bits,
+                  float r_out, float r_in, float theta, int pot_mode,
+                  float* acc_pot_host, int64_t* nb_offsets_host, int32_t* nb_indices_host,
+                  int64_t nb_cap, int64_t* nb_total);
+
+/* ---- parity / debug accessors: synchronise; outputs are ANY pointers sized from p3t_get_stats ---- */
+int p3t_get_stats(p3t_ctx* ctx, p3t_stats* out);
+/* sorted Morton keys [n] (30-bit keys are widened to uint64) and order[n] (sorted position -> original id) */
+int p3t_get_keys(p3t_ctx* ctx, uint64_t* sorted_keys, uint32_t* order);
+/* nodes in breadth-first order (levels ascending, begin ascending inside a level), each [n_nodes];
+ * first_child = -1 and n_child = 0 for a leaf */
+int p3t_get_nodes(p3t_ctx* ctx, int32_t* level, int32_t* begin, int32_t* end,
+                  int32_t* first_child, int32_t* n_child);
+/* fp32 node data: com_m [n_nodes x 4], quad [n_nodes x 6] (xx yy zz xy xz yz, traceless),
+ * clo / chi [n_nodes x 3] tight box, delta [n_nodes] = |COM - geometric centre| */
+int p3t_get_moments(p3t_ctx* ctx, float* com_m, float* quad, float* clo, float* chi, float* delta);
+/* target groups as ranges of sorted positions, each [n_groups], ascending */
+int p3t_get_groups(p3t_ctx* ctx, int32_t* begin, int32_t* end);
+/* per-group list lengths of the last force call: npp[n_groups], npc[n_groups] (int32) */
+int p3t_get_list_lengths(p3t_ctx* ctx, int32_t* npp, int32_t* npc);
+
+const char* p3t_strerror(int code);
+const char* p3t_last_error(p3t_ctx* ctx);     /* text of the last CUDA failure ("" if none) */
+
+/* Host helper, eq. 20-25: tau = (1/128)(N/2^14)^(-1/3), r_cut = 4 tau,
+ * r_buff = 3 tau sigma, dt_reg = largest 2^-k <= tau, dt_max = dt_reg / 4.  Any output may be NULL. */
+int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, double* r_buff,
+                      double* dt_reg, double* dt_max);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,385 @@
+// p3t_api.cu -- the C-ABI of include/p3t.h: context, argument checks, buffer management,
+// call sequencing, accessors.  All arithmetic of the method lives in p3t_sort/tree/walk.cu.
+#include "p3t_internal.cuh"
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+int p3t_fail_cuda(p3t_ctx* ctx, cudaError_t e, const char* what, int line)
+{
+    if (ctx) {
+        snprintf(ctx->err, sizeof(ctx->err), "%s (%s) at line %d: %s", cudaGetErrorName(e), cudaGetErrorString(e), line, what);
+        ctx->sticky = 1;
+    }
+    return e == cudaErrorMemoryAllocation ? P3T_ENOMEM : P3T_ECUDA;
+}
+
+int p3t_reserve(p3t_ctx* ctx, p3t_buf* b, size_t bytes)
+{
+    if (bytes <= b->bytes) return P3T_OK;
+    if (b->p) { P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); P3T_CUDA(ctx, cudaFree(b->p)); b->p = nullptr; b->bytes = 0; }
+    size_t want = bytes + bytes / 8 + 256;                 // a little head-room: lists grow slowly between steps
+    cudaError_t e = cudaMalloc(&b->p, want);
+    if (e != cudaSuccess) { b->p = nullptr; (void)cudaGetLastError(); return p3t_fail_cuda(ctx, e, "cudaMalloc", __LINE__); }
+    b->bytes = want;
+    return P3T_OK;
+}
+
+extern "C" {
+
+const char* p3t_strerror(int code)
+{
+    switch (code) {
+    case P3T_OK: return "ok";
+    case P3T_EINVAL: return "invalid argument";
+    case P3T_ESTATE: return "call out of order (build before force, force before neighbours)";
+    case P3T_ENOMEM: return "out of device memory";
+    case P3T_ECUDA: return "CUDA failure (see p3t_last_error)";
+    case P3T_ERANGE: return "a neighbour row or list exceeds the capacity given";
+    default: return "unknown error code";
+    }
+}
+
+const char* p3t_last_error(p3t_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return P3T_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { (void)cudaGetLastError(); return P3T_EINVAL; }
+    p3t_ctx* c = new (std::nothrow) p3t_ctx();
+    if (!c) return P3T_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->device = device; c->stream = (cudaStream_t)cuda_stream;
+    c->nleaf = 16; c->ncrit = 64;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evw[k]);
+    if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
+    int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
+    if (rc == P3T_OK) rc = p3t_tree_init(c);
+    if (rc != P3T_OK) { p3t_destroy(c); return rc; }
+    *out = c;
+    return P3T_OK;
+}
+
+int p3t_destroy(p3t_ctx* c)
+{
+    if (!c) return P3T_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
+                        &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp,
+                        &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill,
+                        &c->info, &c->stage_in, &c->stage_out };
+    for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
+    for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
+    (void)cudaGetLastError();
+    delete c;
+    return P3T_OK;
+}
+
+int p3t_set_tree_params(p3t_ctx* c, int nleaf, int ncrit)
+{
+    if (!c || nleaf < 1 || ncrit < nleaf || ncrit > P3T_MAX_NCRIT) return P3T_EINVAL;
+    c->nleaf = nleaf; c->ncrit = ncrit;
+    return P3T_OK;
+}
+
+int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
+{
+    if (!c || !pos_mass || n < 1 || n > P3T_MAX_N || (key_bits != 30 && key_bits != 63)) return P3T_EINVAL;
+    if (((uintptr_t)pos_mass & 15u) != 0) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    c->state = 0; c->nb_valid = 0;
+    c->n = n; c->key_bits = key_bits; c->bits = key_bits / 3;
+    // hard bound on the cell count (data layout): leaves <= n, branching cells < n,
+    // one-child chain cells <= levels * n / (nleaf + 1)
+    int64_t cap = 2 * n + (int64_t)c->bits * (n / (c->nleaf + 1)) + 64;
+    if (cap > 0x7fffff00ll) cap = 0x7fffff00ll;
+    c->node_cap = cap;
+    const size_t N = (size_t)n, C = (size_t)cap;
+    const size_t ntiles = (N + P3T_SORT_TILE - 1) / P3T_SORT_TILE;
+    int rc;
+#define RES(buf, bytes) if ((rc = p3t_reserve(c, &c->buf, (bytes))) != P3T_OK) return rc
+    RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16);
+    RES(hist, (ntiles + 1) * P3T_RADIX * 4);
+    RES(nlevel, C * 4); RES(nbegin, C * 4); RES(nend, C * 4); RES(nfirst, C * 4); RES(nnchild, C * 4);
+    RES(m64, C * 80);
+    RES(ncom, C * 16); RES(nlo, C * 16); RES(nhi, C * 16); RES(nq0, C * 16); RES(nq1, C * 8); RES(nlink, C * 8);
+    RES(scan_tmp, (size_t)c->coop_blocks_tree * 4 + 64);
+    RES(gflag, N + 64); RES(gbegin, (N + 2) * 4); RES(gnpp, (N + 1) * 4); RES(gnpc, (N + 1) * 4);
+#undef RES
+    const float4* pm = (const float4*)pos_mass;
+    P3T_CUDA(c, cudaEventRecord(c->ev[0], c->stream));
+    P3T_CUDA(c, cudaMemsetAsync(c->info.p, 0, sizeof(p3t_devinfo), c->stream));
+    if ((rc = p3t_launch_cube_keys(c, pm)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaEventRecord(c->ev[2], c->stream));
+    if ((rc = p3t_launch_sort(c)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaEventRecord(c->ev[3], c->stream));
+    if ((rc = p3t_launch_permute(c, pm)) != P3T_OK) return rc;
+    if ((rc = p3t_launch_tree(c)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
+    c->state = 1;
+    return P3T_OK;
+}
+
+int p3t_regular_force(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float* acc_pot)
+{
+    if (!c || !acc_pot) return P3T_EINVAL;
+    if (!(r_in >= 0.0f) || !(r_in < r_out) || !(theta > 0.0f) || !isfinite(r_out) || !isfinite(theta)) return P3T_EINVAL;
+    if (pot_mode != 0 && pot_mode != 1) return P3T_EINVAL;
+    if (((uintptr_t)acc_pot & 15u) != 0) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    c->nb_valid = 0;
+    c->r_out = r_out; c->r_in = r_in; c->theta = theta;
+    int rc = p3t_launch_force(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot);
+    if (rc != P3T_OK) return rc;
+    c->state = 2; c->nb_valid = 1;
+    return P3T_OK;
+}
+
+static int sync_and_check(p3t_ctx* c, p3t_devinfo* h)
+{
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    P3T_CUDA(c, cudaMemcpyAsync(h, c->info.p, sizeof(p3t_devinfo), cudaMemcpyDeviceToHost, c->stream));
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (h->node_overflow || h->stack_overflow) {
+        snprintf(c->err, sizeof(c->err), "internal capacity exceeded (node_overflow=%d stack_overflow=%d)", h->node_overflow, h->stack_overflow);
+        return P3T_ECUDA;
+    }
+    if (h->bad_input) return P3T_EINVAL;
+    return P3T_OK;
+}
+
+int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
+{
+    if (!c || !out) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    memset(out, 0, sizeof(*out));
+    out->n = c->n; out->n_nodes = h.n_nodes; out->n_leaves = h.n_leaves; out->n_groups = h.n_groups;
+    out->max_level = h.max_level; out->key_bits = c->key_bits;
+    out->input_bad = h.bad_input;
+    for (int a = 0; a < 3; ++a) out->cube_lo[a] = h.lo[a];
+    out->cube_side = h.side;
+    if (rc == P3T_ECUDA) return rc;
+    (void)cudaEventElapsedTime(&out->ms_build, c->ev[0], c->ev[1]);
+    (void)cudaEventElapsedTime(&out->ms_sort, c->ev[2], c->ev[3]);
+    if (c->state >= 2) {
+        out->n_pp = (int64_t)h.n_pp; out->n_pc = (int64_t)h.n_pc;
+        out->n_pp_list = (int64_t)h.n_pp_list; out->n_pc_list = (int64_t)h.n_pc_list;
+        out->nb_total = (int64_t)h.nb_total; out->nb_max = h.nb_max;
+        (void)cudaEventElapsedTime(&out->ms_force, c->ev[4], c->ev[5]);
+        (void)cudaEventElapsedTime(&out->ms_walk, c->evw[0], c->evw[1]);
+    }
+    (void)cudaGetLastError();
+    return rc;
+}
+
+static int copy_out(p3t_ctx* c, void* dst, const void* src, size_t bytes)
+{
+    if (!dst || bytes == 0) return P3T_OK;
+    P3T_CUDA(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, c->stream));
+    return P3T_OK;
+}
+
+int p3t_neighbours(p3t_ctx* c, const int64_t** offsets, const int32_t** indices, int64_t* total)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 2 || !c->nb_valid) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    if (rc != P3T_OK) return rc;
+    if (offsets) *offsets = (const int64_t*)c->nboff.p;
+    if (indices) *indices = (const int32_t*)c->nbidx.p;
+    if (total) *total = (int64_t)h.nb_total;
+    return P3T_OK;
+}
+
+int p3t_neighbours_copy(p3t_ctx* c, int64_t* offsets_out, int32_t* indices_out)
+{
+    const int64_t* off; const int32_t* idx; int64_t total;
+    int rc = p3t_neighbours(c, &off, &idx, &total);
+    if (rc != P3T_OK) return rc;
+    if ((rc = copy_out(c, offsets_out, off, ((size_t)c->n + 1) * 8)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, indices_out, idx, (size_t)total * 4)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
+int p3t_neighbours_nbody6(p3t_ctx* c, int32_t lmax, int32_t* host_list)
+{
+    if (!c || !host_list || lmax < 0) return P3T_EINVAL;
+    const int64_t* off; const int32_t* idx; int64_t total;
+    int rc = p3t_neighbours(c, &off, &idx, &total);
+    if (rc != P3T_OK) return rc;
+    p3t_devinfo h;
+    if ((rc = sync_and_check(c, &h)) != P3T_OK) return rc;
+    if (h.nb_max > lmax) return P3T_ERANGE;
+    const size_t n = (size_t)c->n;
+    int64_t* ho = (int64_t*)malloc((n + 1) * 8);
+    int32_t* hi = (int32_t*)malloc((size_t)total * 4 + 4);
+    if (!ho || !hi) { free(ho); free(hi); return P3T_ENOMEM; }
+    rc = p3t_neighbours_copy(c, ho, hi);
+    if (rc == P3T_OK) {
+        const size_t stride = (size_t)lmax + 1;
+        for (size_t i = 0; i < n; ++i) {
+            int32_t* row = host_list + i * stride;
+            const int64_t b = ho[i], len = ho[i + 1] - b;
+            row[0] = (int32_t)len;
+            for (int64_t k = 0; k < len; ++k) row[1 + k] = hi[b + k] + 1;        // NBODY6 is 1-based
+            for (size_t k = (size_t)len + 1; k < stride; ++k) row[k] = 0;
+        }
+    }
+    free(ho); free(hi);
+    return rc;
+}
+
+int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bits,
+                  float r_out, float r_in, float theta, int pot_mode,
+                  float* acc_pot_host, int64_t* nb_offsets_host, int32_t* nb_indices_host,
+                  int64_t nb_cap, int64_t* nb_total)
+{
+    if (!c || !pos_mass_host || !acc_pot_host || n < 1 || n > P3T_MAX_N) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    int rc;
+    if ((rc = p3t_reserve(c, &c->stage_in, (size_t)n * 32)) != P3T_OK) return rc;     // pos_mass in, acc_pot out
+    float* d_pm = (float*)c->stage_in.p;
+    float* d_out = d_pm + (size_t)n * 4;
+    P3T_CUDA(c, cudaMemcpyAsync(d_pm, pos_mass_host, (size_t)n * 16, cudaMemcpyHostToDevice, c->stream));
+    if ((rc = p3t_build_tree(c, n, d_pm, key_bits)) != P3T_OK) return rc;
+    if ((rc = p3t_regular_force(c, r_out, r_in, theta, pot_mode, d_out)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
+    const int64_t total = c->nb_total_host;                  // known on the host since the force call sized the lists
+    if (nb_total) *nb_total = total;
+    if (nb_offsets_host) P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
+    int over = 0;
+    if (nb_indices_host) {
+        if (total > nb_cap) over = 1;
+        else if (total > 0) P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
+    }
+    p3t_devinfo h;
+    if ((rc = sync_and_check(c, &h)) != P3T_OK) return rc;
+    return over ? P3T_ERANGE : P3T_OK;
+}
+
+// ---- accessors ----
+int p3t_get_keys(p3t_ctx* c, uint64_t* sorted_keys, uint32_t* order)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    int rc;
+    if ((rc = copy_out(c, sorted_keys, c->keys[0].p, (size_t)c->n * 8)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, order, c->idx[0].p, (size_t)c->n * 4)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
+int p3t_get_nodes(p3t_ctx* c, int32_t* level, int32_t* begin, int32_t* end, int32_t* first_child, int32_t* n_child)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    if (rc != P3T_OK) return rc;
+    const size_t b = (size_t)h.n_nodes * 4;
+    if ((rc = copy_out(c, level, c->nlevel.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, begin, c->nbegin.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, end, c->nend.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, first_child, c->nfirst.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, n_child, c->nnchild.p, b)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
+int p3t_get_moments(p3t_ctx* c, float* com_m, float* quad, float* clo, float* chi, float* delta)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    if (rc != P3T_OK) return rc;
+    const size_t nn = (size_t)h.n_nodes;
+    // the walk's SoA packs delta and the level into the .w lanes: unpack on the host
+    float4* t = (float4*)malloc(nn * 16 * 3 + nn * 8 + 16);
+    if (!t) return P3T_ENOMEM;
+    float4 *lo = t, *hi = t + nn, *q0 = t + 2 * nn; float2* q1 = (float2*)(t + 3 * nn);
+    cudaError_t e = cudaMemcpyAsync(lo, c->nlo.p, nn * 16, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hi, c->nhi.p, nn * 16, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(q0, c->nq0.p, nn * 16, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(q1, c->nq1.p, nn * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && com_m) e = cudaMemcpyAsync(com_m, c->ncom.p, nn * 16, cudaMemcpyDefault, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { free(t); return p3t_fail_cuda(c, e, "p3t_get_moments copies", __LINE__); }
+    for (size_t k = 0; k < nn; ++k) {
+        if (quad) { float* q = quad + 6 * k; q[0] = q0[k].x; q[1] = q0[k].y; q[2] = q0[k].z; q[3] = q0[k].w; q[4] = q1[k].x; q[5] = q1[k].y; }
+        if (clo) { clo[3 * k] = lo[k].x; clo[3 * k + 1] = lo[k].y; clo[3 * k + 2] = lo[k].z; }
+        if (chi) { chi[3 * k] = hi[k].x; chi[3 * k + 1] = hi[k].y; chi[3 * k + 2] = hi[k].z; }
+        if (delta) delta[k] = lo[k].w;
+    }
+    free(t);
+    return P3T_OK;
+}
+
+int p3t_get_groups(p3t_ctx* c, int32_t* begin, int32_t* end)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    if (rc != P3T_OK) return rc;
+    const size_t b = (size_t)h.n_groups * 4;
+    if ((rc = copy_out(c, begin, c->gbegin.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, end, (const int32_t*)c->gbegin.p + 1, b)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
+int p3t_get_list_lengths(p3t_ctx* c, int32_t* npp, int32_t* npc)
+{
+    if (!c) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 2) return P3T_ESTATE;
+    p3t_devinfo h;
+    int rc = sync_and_check(c, &h);
+    if (rc != P3T_OK) return rc;
+    const size_t b = (size_t)h.n_groups * 4;
+    if ((rc = copy_out(c, npp, c->gnpp.p, b)) != P3T_OK) return rc;
+    if ((rc = copy_out(c, npc, c->gnpc.p, b)) != P3T_OK) return rc;
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
+// eq. 20-25
+int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, double* r_buff, double* dt_reg, double* dt_max)
+{
+    if (n < 1 || !(sigma > 0.0)) return P3T_EINVAL;
+    const double t = (1.0 / 128.0) * pow((double)n / 16384.0, -1.0 / 3.0);   // eq. 22
+    double dt = 1.0;
+    while (dt > t * (1.0 + 1e-12)) dt *= 0.5;                                 // eq. 23: largest 2^-k <= tau (reading R12)
+    if (tau) *tau = t;
+    if (r_cut) *r_cut = 4.0 * t;                                              // eq. 21
+    if (r_buff) *r_buff = 3.0 * t * sigma;                                    // eq. 20
+    if (dt_reg) *dt_reg = dt;
+    if (dt_max) *dt_max = dt / 4.0;                                           // eq. 24-25
+    return P3T_OK;
+}
+
+}  // extern "C"

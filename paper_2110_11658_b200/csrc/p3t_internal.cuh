@@ -1,0 +1,93 @@
+// p3t_internal.cuh -- context record and launcher prototypes shared by the .cu files of libp3t.so.
+// Nothing here is shared with oracle/ (the CPU checker); the two only agree on RULES.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "p3t.h"
+
+#define P3T_RADIX_BITS 8
+#define P3T_RADIX      256
+#define P3T_SORT_THREADS 256
+#define P3T_SORT_ITEMS   16                                  // keys per thread in one sort tile
+#define P3T_SORT_TILE    (P3T_SORT_THREADS * P3T_SORT_ITEMS) // 4096 keys per block
+
+// device-side counters written by the build and force kernels (one 256-byte record)
+struct p3t_devinfo {
+    float    lo[3];          // bounding cube, R-S1
+    float    side;
+    float    scale;          // 2^B / side
+    int32_t  bad_input;      // NaN/Inf seen
+    int32_t  n_nodes;
+    int32_t  n_leaves;
+    int32_t  max_level;
+    int32_t  n_groups;
+    int32_t  node_overflow;
+    int32_t  level_begin[24]; // first node of each level; level_begin[max_level+1] = n_nodes
+    uint32_t group_cursor;   // dynamic group scheduler of the walk kernels
+    uint32_t group_cursor2;
+    unsigned long long n_pp, n_pc, n_pp_list, n_pc_list;
+    unsigned long long nb_total;
+    int32_t  nb_max;
+    int32_t  stack_overflow;
+    uint32_t minmax[6];      // order-preserving uint encodings of min xyz / max xyz
+};
+
+struct p3t_buf { void* p; size_t bytes; };
+
+struct p3t_ctx {
+    int device;
+    cudaStream_t stream;
+    int num_sms;
+    int nleaf, ncrit;
+    int state;               // 0 = created, 1 = built, 2 = force done
+    int64_t n;
+    int key_bits, bits;      // bits per axis
+    int64_t node_cap;
+    char err[256];
+    int sticky;
+    // device buffers (grow-only)
+    p3t_buf keys[2], idx[2];         // uint64 / uint32 ping-pong; after the sort [0] holds the result
+    p3t_buf spm;                     // float4 sorted bodies
+    p3t_buf hist;                    // sort: per-block digit counts
+    p3t_buf nlevel, nbegin, nend, nfirst, nnchild;        // int32 per node
+    p3t_buf m64;                     // double[10] per node: M, com[3], Q[6]
+    p3t_buf ncom, nlo, nhi, nq0, nq1, nlink;              // walk SoA (see p3t_tree.cu)
+    p3t_buf scan_tmp;                // block sums of the cooperative kernels
+    p3t_buf gflag, gbegin;           // group start flags [n+1] / compacted starts [n_groups+1]
+    p3t_buf gnpp, gnpc;              // per-group list lengths
+    p3t_buf nbcount, nboff, nbidx;   // neighbour CSR: counts (sorted order) -> offsets (original order), indices
+    p3t_buf nbcur;                   // int64 per sorted particle: write cursor base
+    p3t_buf spill;                   // walk stack spill
+    p3t_buf info;                    // p3t_devinfo
+    p3t_buf stage_in, stage_out;     // p3t_step_host staging
+    int64_t nb_total_host;           // valid after p3t_neighbours
+    int nb_valid;
+    cudaEvent_t ev[6];               // build begin/end, sort begin/end ... force begin/end, walk begin/end
+    cudaEvent_t evw[4];
+    int coop_blocks_tree;            // co-resident grid of the tree kernel
+    p3t_stats last;
+    float r_out, r_in, theta;
+};
+
+#define P3T_CUDA(ctx, call)                                                              \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) return p3t_fail_cuda((ctx), e_, #call, __LINE__);         \
+    } while (0)
+
+int  p3t_fail_cuda(p3t_ctx* ctx, cudaError_t e, const char* what, int line);
+int  p3t_reserve(p3t_ctx* ctx, p3t_buf* b, size_t bytes);
+
+template <typename T> static inline T* P(p3t_buf& b) { return (T*)b.p; }
+static inline p3t_devinfo* INFO(p3t_ctx* c) { return (p3t_devinfo*)c->info.p; }
+
+// p3t_sort.cu : a1-a3
+int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pos_mass);
+int p3t_launch_sort(p3t_ctx* ctx);
+int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
+// p3t_tree.cu : a4-a6
+int p3t_tree_init(p3t_ctx* ctx);
+int p3t_launch_tree(p3t_ctx* ctx);
+// p3t_walk.cu : a7-a11
+int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot);
