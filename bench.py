@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py -- the regular-force step of NBODY6+P3T on B200 (BASELINE.json metric:
+regular-force particles/s and interactions/s at N = 1M; ms per force step).
+
+A "step" is one pass of the whole hot path over one synthetic cluster:
+p3t_build_tree + p3t_regular_force (cube, keys, sort, octree, moments, groups, walk, p-c / p-p force
+with cutoff, neighbour lists, scatter), i.e. what the host integrator asks for once per dt_reg
+(PAPER.md:89-94).  Default workload = BASELINE config 3 (Plummer 2^20, Kroupa masses, theta 0.4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  `value` times the path with inputs resident in HBM; `e2e` times
+p3t_step_host with pinned HOST buffers (H2D of positions, D2H of forces and neighbour lists inside
+the timed region).  `roofline` is for the dominant kernel (walk + force), an FP32-ALU-bound kernel;
+`cpu_baseline` is the fp64 oracle on the host cores, on a bounded sample.  Multi-GPU: the path does
+not shard in this build ("replicas only"): every rank runs an independent replica.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+# FP32-pipe instructions the method needs per interaction
+INSTR_PP, INSTR_PC = 15, 37
+FLOP_PP, FLOP_PC = 20, 60
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm_gbs=float(d.get("hbm_gbs", 6650.0)), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of /opt/skills/guides/B200_PROFILING.md, sampled during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_run(w, n_groups_target: int):
+    """The oracle as it stands, on a bounded sample: full tree build + force of every k-th group."""
+    import oracle
+    t0 = time.perf_counter()
+    T = oracle.Tree(w.pos_mass, 63, 16, 64)
+    t_build = time.perf_counter() - t0
+    stride = max(1, T.n_groups // n_groups_target)
+    gi = np.arange(0, T.n_groups, stride, dtype=np.int64)
+    g = T.groups()
+    cnt = (g["end"] - g["begin"]).astype(np.int64)
+    t0 = time.perf_counter()
+    f = T.force(w.r_out, w.r_in, w.theta, 0, group_ids=gi)
+    t_force = time.perf_counter() - t0
+    n_s = int(cnt[gi].sum())
+    inter = int(((f["npp"] + f["npc"]) * cnt[gi]).sum())
+    # whole-path time of the full N, extrapolated from the sample: build + force * N / n_s
+    t_full = t_build + t_force * w.n / n_s
+    return dict(t_build=t_build, t_force=t_force, n_sample=n_s, groups=len(gi), stride=stride, interactions=inter,
+                particles_per_s=w.n / t_full, interactions_per_s=inter / t_force, t_full=t_full, cores=oracle.omp_threads())
+
+
+def run_reference(args, w, rank):
+    """--impl reference: the fp64 CPU oracle (there is no other reference implementation: the paper's
+    code is not available).  Rank 0 only; every step is a bounded sample of the workload."""
+    if rank != 0:
+        return
+    n_groups = 1200 if w.n >= 500000 else 100000
+    for _ in range(args.warmup):
+        oracle_sample_run(w, max(50, n_groups // 20))
+    t0 = time.perf_counter()
+    runs = [oracle_sample_run(w, n_groups) for _ in range(args.steps)]
+    wall = time.perf_counter() - t0
+    pps = float(np.mean([r["particles_per_s"] for r in runs]))
+    r0 = runs[-1]
+    sample = (f"per step: full oracle tree build ({r0['t_build']:.2f} s) + fp64 tree force of every {r0['stride']}th group "
+              f"({r0['groups']} groups, {r0['n_sample']} particles, {r0['t_force']:.2f} s); particles/s extrapolated to the "
+              f"full N as N / (t_build + t_force * N / n_sample)")
+    line = {
+        "impl": "reference", "metric": "regular_force_particles_per_s", "value": pps, "unit": "particles/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "n": w.n, "r_out": w.r_out, "r_in": w.r_in, "theta": w.theta},
+        "interactions_per_s": float(np.mean([r["interactions_per_s"] for r in runs])),
+        "cpu_baseline": {"value": pps, "unit": "particles/s", "cores": r0["cores"], "kind": "oracle", "sample": sample},
+        "e2e": {"value": pps, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def reduce_over_ranks(total_ms: float, units: float, dist) -> tuple:
+    """Max of the timed region over ranks and sum of the units processed (host-side logic of the N > 1
+    path; covered by a world_size-2 gloo test on CPU)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return total_ms, units
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def run_ours(args, w, rank, world, local_rank, dist):
+    import torch
+    import paper_2110_11658_b200 as p3t
+
+    p3t.lib()                                             # fail loudly when the CUDA library is missing
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    pk = peaks()
+    n = w.n
+    pm_dev = torch.from_numpy(w.pos_mass).to(dev)
+    out_dev = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)       # > 126 MB of L2
+    ctx = p3t.Context(local_rank)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device():
+        ctx.build_tree(pm_dev, 63)
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0, out=out_dev)
+
+    for _ in range(max(3, args.warmup)):
+        step_device()
+    torch.cuda.synchronize()
+    st0 = ctx.stats()
+
+    # ---- device-resident arm ----
+    sampler = ClockSampler(local_rank)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    walk_ms, build_ms, force_ms, sort_ms = [], [], [], []
+    for k in range(args.steps):
+        flush.zero_()                                     # L2 flush between timed iterations (outside the event pair)
+        ev[k][0].record()
+        step_device()
+        ev[k][1].record()
+        st = ctx.stats()                                  # synchronises; after the closing event
+        walk_ms.append(st["ms_walk"]); build_ms.append(st["ms_build"]); force_ms.append(st["ms_force"]); sort_ms.append(st["ms_sort"])
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    launches = int(st["launches"] - st0["launches"])
+
+    # ---- end-to-end arm: HOST buffers through p3t_step_host ----
+    pm_host = torch.from_numpy(w.pos_mass).pin_memory()
+    acc_host = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+    nb_cap = int(st["nb_total"] * 1.25) + 1024
+    off_host = torch.empty(n + 1, dtype=torch.int64).pin_memory()
+    idx_host = torch.empty(nb_cap, dtype=torch.int32).pin_memory()
+
+    def step_host():
+        return ctx.step_host(pm_host, w.r_out, w.r_in, w.theta, 0, 63, acc_pot=acc_host, nb_offsets=off_host, nb_indices=idx_host)
+
+    for _ in range(3):
+        step_host()
+    barrier()
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.zero_()
+        ev2[k][0].record()
+        _, _, _, nb_total = step_host()
+        ev2[k][1].record()
+    barrier()
+    e2e_ms = float(sum(a.elapsed_time(b) for a, b in ev2))
+    assert torch.isfinite(acc_host).all()
+
+    total_ms_max, units = reduce_over_ranks(total_ms, float(n) * args.steps, dist)
+    e2e_ms_max, _ = reduce_over_ranks(e2e_ms, float(n) * args.steps, dist)
+    if rank != 0:
+        return
+    value = units / (total_ms_max * 1e-3)
+    e2e_value = units / (e2e_ms_max * 1e-3)
+    n_int = st["n_pp"] + st["n_pc"]
+    wms = float(np.mean(walk_ms))
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    alg_instr = INSTR_PP * st["n_pp"] + INSTR_PC * st["n_pc"]
+    peak_instr = sms * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # Tinstr/s, FP32 lanes x clock
+    achieved = alg_instr / (wms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "k_walk<1> (walk + p-c/p-p force + cutoff + neighbour emission)",
+        "achieved": achieved, "peak": peak_instr, "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / peak_instr,
+        "traffic": None, "peak_source": f"{sms} SMs x 128 FP32 lanes x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
+        "algorithmic": f"{INSTR_PP} instr per p-p x {st['n_pp']} + {INSTR_PC} per p-c x {st['n_pc']}",
+        "achieved_tflops": (FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]) / (wms * 1e-3) / 1e12,
+        "kernel_ms": wms, "kernel_share_of_step": wms * args.steps / total_ms,
+        "frac_at_observed_clock": (achieved / (sms * 128 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
+    }
+    line = {
+        "metric": "regular_force_particles_per_s", "value": value, "unit": "particles/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "n": n, "r_out": w.r_out, "r_in": w.r_in, "theta": w.theta, "key_bits": 63,
+                   "nleaf": 16, "ncrit": 64, "l2": "flushed between timed iterations (512 MiB write)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "interactions_per_s": n_int * world / (wms * 1e-3), "interactions_per_step": n_int,
+        "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n,
+        "ms_build": float(np.mean(build_ms)), "ms_sort": float(np.mean(sort_ms)), "ms_force": float(np.mean(force_ms)), "ms_walk": wms,
+        "nodes": st["n_nodes"], "groups": st["n_groups"], "neighbours_total": st["nb_total"], "neighbours_max": st["nb_max"],
+        "e2e": {"value": e2e_value, "unit": "particles/s", "ms_per_step": e2e_ms_max / args.steps,
+                "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n + 8 * (n + 1) + 4 * int(nb_total)},
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        r = oracle_sample_run(w, 4000 if n >= 500000 else 100000)
+        line["cpu_baseline"] = {
+            "value": r["particles_per_s"], "unit": "particles/s", "cores": r["cores"], "kind": "oracle",
+            "interactions_per_s": r["interactions_per_s"],
+            "sample": (f"full oracle tree build ({r['t_build']:.2f} s) + fp64 tree force of every {r['stride']}th group "
+                       f"({r['groups']} groups, {r['n_sample']} particles, {r['t_force']:.2f} s); extrapolated to the full N"),
+        }
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (3 = headline, Plummer 2^20)")
+    ap.add_argument("--n", type=int, default=None, help="override the particle count (debug)")
+    ap.add_argument("--theta", type=float, default=None)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    import workloads
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, workloads.make_config(args.config, n_override=args.n, theta=args.theta), rank)
+        return
+    dist = None
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    w = workloads.make_config(args.config, n_override=args.n, theta=args.theta)
+    run_ours(args, w, rank, world, local_rank, dist)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

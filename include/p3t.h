@@ -64,6 +64,7 @@ typedef struct p3t_stats {
     float   ms_force;        /* CUDA-event time of the last p3t_regular_force (a7-a11)  */
     float   ms_walk;         /* ... of its walk+force kernel alone                      */
     float   ms_sort;         /* ... of the radix sort inside the last build             */
+    int64_t launches;        /* kernels this context has launched since p3t_create      */
 } p3t_stats;
 
 /* Create a context on CUDA device `device`, enqueuing on `cuda_stream` (a cudaStream_t passed as

@@ -173,6 +173,7 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
     out->input_bad = h.bad_input;
     for (int a = 0; a < 3; ++a) out->cube_lo[a] = h.lo[a];
     out->cube_side = h.side;
+    out->launches = c->launches;
     if (rc == P3T_ECUDA) return rc;
     (void)cudaEventElapsedTime(&out->ms_build, c->ev[0], c->ev[1]);
     (void)cudaEventElapsedTime(&out->ms_sort, c->ev[2], c->ev[3]);

@@ -68,6 +68,7 @@ struct p3t_ctx {
     int coop_blocks_tree;            // co-resident grid of the tree kernel
     p3t_stats last;
     float r_out, r_in, theta;
+    int64_t launches;                // kernels launched so far
 };
 
 #define P3T_CUDA(ctx, call)                                                              \

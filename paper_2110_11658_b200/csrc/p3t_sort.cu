@@ -220,6 +220,7 @@ int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pm)
     k_cube<<<blocks, 256, 0, ctx->stream>>>(pm, n, INFO(ctx));
     k_keys<<<blocks, 256, 0, ctx->stream>>>(pm, n, ctx->bits, INFO(ctx), P<uint64_t>(ctx->keys[0]));
     P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 2;
     return P3T_OK;
 }
 
@@ -240,6 +241,7 @@ int p3t_launch_sort(p3t_ctx* ctx)
         if (p == 0) k_scatter<true><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
         else        k_scatter<false><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
         cur ^= 1;
+        ctx->launches += 3;
     }
     P3T_CUDA(ctx, cudaGetLastError());
     // an even number of passes leaves the result in buffer 0
@@ -255,5 +257,6 @@ int p3t_launch_permute(p3t_ctx* ctx, const float4* pm)
     const int n = (int)ctx->n;
     k_permute<<<(n + 255) / 256, 256, 0, ctx->stream>>>(pm, P<uint32_t>(ctx->idx[0]), n, P<float4>(ctx->spm));
     P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 1;
     return P3T_OK;
 }

@@ -331,5 +331,6 @@ int p3t_launch_tree(p3t_ctx* ctx)
     P3T_CUDA(ctx, cudaMemsetAsync(ctx->gflag.p, 0, (size_t)ctx->n + 32, ctx->stream));
     void* args[] = { &A };
     P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void*)k_tree, dim3(ctx->coop_blocks_tree), dim3(TREE_THREADS), args, 0, ctx->stream));
+    ctx->launches += 1;
     return P3T_OK;
 }

@@ -530,5 +530,6 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
+    ctx->launches += 7;
     return P3T_OK;
 }

@@ -1,0 +1,371 @@
+"""GPU parity: libp3t.so (through its C-ABI binding) against the fp64 CPU oracle, element by element
+on the same seeded inputs.  Bars (north_star; norms: DESIGN.md R15):
+  * Morton keys, sort order, octree cells, groups, p-p / p-c list lengths, neighbour CSR: bit-exact;
+  * fp32 node moments: bit-equal except for O(1) values (<= 1e-6 relative);
+  * tree force vs the CPU tree with the same opening rule: 1e-6 relative (L2 norm over all particles,
+    per-particle median and p99, and max of |da| / sum_j |a_ij|);
+  * tree force vs eq. 3 direct summation at theta = 0.4: median < 2e-3, p99 < 2e-2.
+Every GPU call goes through paper_2110_11658_b200 (ctypes over include/p3t.h)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+NLEAF, NCRIT = 16, 64
+
+
+@pytest.fixture(scope="module")
+def p3t():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2110_11658_b200 as m
+    m.lib()                                   # fails loudly if libp3t.so is missing
+    return m
+
+
+def _cuda(pm):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(pm, dtype=np.float32)).cuda()
+
+
+def _rel(a, ref):
+    return np.linalg.norm(a - ref, axis=1) / np.linalg.norm(ref, axis=1)
+
+
+def check_build(ctx, T, pm, bits):
+    """a1-a6 bit-exact against the oracle tree T."""
+    st = ctx.stats()
+    lo, side = T.cube()
+    assert np.array_equal(np.asarray(st["cube_lo"], np.float32), lo) and st["cube_side"] == side
+    ok, oo = T.keys(); gk, go = ctx.keys()
+    assert np.array_equal(ok, gk), "Morton keys differ"
+    assert np.array_equal(oo, go), "sort order differs"
+    assert (st["n_nodes"], st["n_leaves"], st["max_level"], st["n_groups"]) == (T.n_nodes, T.n_leaves, T.max_level, T.n_groups)
+    on, gn = T.nodes(), ctx.nodes()
+    for k in ("level", "begin", "end", "first_child", "n_child"):
+        assert np.array_equal(on[k], gn[k]), f"node field {k} differs"
+    og, gg = T.groups(), ctx.groups()
+    assert np.array_equal(og["begin"], gg["begin"]) and np.array_equal(og["end"], gg["end"])
+    om, gm = T.moments(), ctx.moments()
+    assert np.array_equal(om["clo"], gm["clo"]) and np.array_equal(om["chi"], gm["chi"])     # exact min/max
+    l = side / 2.0 ** on["level"].astype(np.float64)
+    mass = om["com_m"][:, 3].astype(np.float64)
+    # moments: fp64 sums in another order, rounded once to fp32: equal up to rare 1-ulp flips
+    assert np.abs(gm["com_m"][:, :3].astype(np.float64) - om["com_m"][:, :3]).max() <= 1e-6 * side
+    assert np.abs(gm["com_m"][:, 3] / om["com_m"][:, 3] - 1).max() <= 2e-7
+    scale_q = np.maximum(np.abs(om["quad"]).max(axis=1), 1e-300)
+    qerr = np.abs(gm["quad"].astype(np.float64) - om["quad"]).max(axis=1)
+    assert np.all(qerr <= 1e-5 * np.maximum(scale_q, 1e-7 * mass * l * l))
+    assert np.abs(gm["delta"].astype(np.float64) - om["delta"]).max() <= 1e-6 * side
+    n_flip = sum(int(np.count_nonzero(gm[k] != om[k])) for k in ("com_m", "delta"))
+    assert n_flip <= 2 + T.n_nodes // 100000, f"{n_flip} COM/delta values differ in the last bit"
+
+
+def check_force(ctx, T, w, pot_mode=0, group_ids=None, theta=None, per_particle=True):
+    th = w.theta if theta is None else theta
+    out = ctx.regular_force(w.r_out, w.r_in, th, pot_mode)
+    a = out.cpu().numpy().astype(np.float64)
+    f = T.force(w.r_out, w.r_in, th, pot_mode, group_ids=group_ids, want_abs=True)
+    ref = f["acc_pot"]
+    m = ~np.isnan(ref[:, 0])
+    npp, npc = ctx.list_lengths()
+    sel = slice(None) if group_ids is None else group_ids
+    assert np.array_equal(npp[sel], f["npp"]) and np.array_equal(npc[sel], f["npc"]), "interaction lists differ"
+    da = np.linalg.norm(a[m, :3] - ref[m, :3], axis=1)
+    na = np.linalg.norm(ref[m, :3], axis=1)
+    ok = na > 0
+    assert np.linalg.norm(a[m, :3] - ref[m, :3]) <= 1e-6 * np.linalg.norm(ref[m, :3])
+    if per_particle and ok.sum() > 10:
+        rel = da[ok] / na[ok]
+        assert np.median(rel) <= 1e-6 and np.percentile(rel, 99) <= 1e-6
+    cond = f["abs_sum"][m]
+    assert np.all(da <= 1e-6 * cond + 1e-30), (da / np.maximum(cond, 1e-300)).max()
+    # potential: same terms, one more rounding each
+    pa = np.abs(a[m, 3] - ref[m, 3])
+    assert np.all(pa <= 2e-6 * np.abs(ref[m, 3]) + 1e-30)
+    return a, f
+
+
+def check_neighbours(ctx, w, targets=None):
+    off, idx = ctx.neighbours()
+    off = off.cpu().numpy(); idx = idx.cpu().numpy()
+    assert off[0] == 0 and off[-1] == idx.shape[0] and np.all(np.diff(off) >= 0)
+    ooff, oidx = oracle.neighbours(w.pos_mass, w.r_out, targets=targets)
+    if targets is None:
+        assert np.array_equal(ooff, off) and np.array_equal(oidx, idx), "neighbour CSR differs"
+    else:
+        for t, i in enumerate(targets):
+            assert np.array_equal(oidx[ooff[t]:ooff[t + 1]], idx[off[i]:off[i + 1]]), f"row {i} differs"
+    return off, idx
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bits", [63, 30])
+def test_config1_everything(p3t, cfg1, bits):
+    """BASELINE config 1 (Plummer 16k, equal masses): every stage, full oracle."""
+    w = cfg1
+    T = oracle.Tree(w.pos_mass, bits, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), bits)
+        check_build(ctx, T, w.pos_mass, bits)
+        a, f = check_force(ctx, T, w, 0)
+        check_neighbours(ctx, w)
+        st = ctx.stats()
+        g = T.groups(); cnt = (g["end"] - g["begin"]).astype(np.int64)
+        assert st["n_pp"] == int((f["npp"] * cnt).sum()) and st["n_pc"] == int((f["npc"] * cnt).sum())
+        # against eq. 3 by direct summation (north_star bound)
+        d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
+        err = _rel(a[:, :3], d["acc_reg"])
+        assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2
+        assert np.abs(a[:, 3] / d["phi_reg"] - 1).max() < 1e-3
+        # unsplit Newtonian potential
+        a1, _ = check_force(ctx, T, w, 1)
+        assert np.abs(a1[:, 3] / d["phi_newt"] - 1).max() < 1e-3
+        assert np.array_equal(a1[:, :3], a[:, :3])              # the acceleration does not depend on pot_mode
+        # run-to-run determinism: identical bits
+        b = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).cpu().numpy().astype(np.float64)
+        assert np.array_equal(a, b)
+
+
+def test_config2_kroupa_full(p3t):
+    """BASELINE config 2 (Plummer 131072, Kroupa masses): full tree parity, sampled direct sum."""
+    w = workloads.make_config(2)
+    T = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        check_build(ctx, T, w.pos_mass, 63)
+        a, _ = check_force(ctx, T, w, 0)
+        tg = workloads.sample_targets(w.n, 4096)
+        check_neighbours(ctx, w, targets=tg)
+        d = oracle.direct(w.pos_mass, w.r_out, w.r_in, targets=tg)
+        err = _rel(a[tg, :3], d["acc_reg"])
+        assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2
+        off, idx = ctx.neighbours()
+        off = off.cpu().numpy(); idx = idx.cpu().numpy()
+        # invariants that hold at any size: symmetric, no self, rows strictly ascending
+        rows = np.repeat(np.arange(w.n), np.diff(off))
+        assert np.all(rows != idx)
+        assert np.all((np.diff(idx) > 0) | (np.diff(rows) > 0))
+        fwd = set(zip(rows.tolist(), idx.tolist()))
+        assert all((j, i) in fwd for i, j in list(fwd)[:20000])
+        assert off[-1] % 2 == 0
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_1m(p3t, cfg):
+    """BASELINE configs 3 (Plummer 2^20, headline) and 4 (King W0=9, 2^20) at full size, in the launch
+    configuration bench.py times: build bit-exact against the full oracle tree; forces on sampled groups
+    the oracle walks one by one; direct sum and neighbour rows on sampled targets."""
+    w = workloads.make_config(cfg)
+    T = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        check_build(ctx, T, w.pos_mass, 63)
+        gi = np.arange(0, T.n_groups, max(1, T.n_groups // 1500), dtype=np.int64)
+        a, _ = check_force(ctx, T, w, 0, group_ids=gi)
+        tg = workloads.sample_targets(w.n, 1024)
+        off, idx = check_neighbours(ctx, w, targets=tg)
+        d = oracle.direct(w.pos_mass, w.r_out, w.r_in, targets=tg)
+        err = _rel(a[tg, :3], d["acc_reg"])
+        assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2
+        st = ctx.stats()
+        assert st["nb_total"] == off[-1]
+        mean_nb = off[-1] / w.n
+        # P9: Plummer mean count ~ N (r_out/a)^3 15 pi/256 = 1.84 (a little more with truncation); King core is dense
+        assert (1.7 < mean_nb < 2.1) if cfg == 3 else (10 < mean_nb < 25)
+        assert np.all(np.isfinite(a))
+
+
+@pytest.mark.parametrize("theta", [0.3, 0.5, 0.7])
+def test_config5_theta_sweep_4m(p3t, theta):
+    """BASELINE config 5 (Plummer 4 194 304, equal masses), opening-angle sweep: sampled groups against
+    the CPU tree, sampled targets against the direct sum."""
+    w = workloads.make_config(5, theta=theta)
+    T = _tree5(w)
+    ctx = _ctx5(p3t, w)
+    gi = np.arange(0, T.n_groups, max(1, T.n_groups // 300), dtype=np.int64)
+    a, _ = check_force(ctx, T, w, 0, group_ids=gi, theta=theta)
+    tg = workloads.sample_targets(w.n, 128)
+    d = oracle.direct(w.pos_mass, w.r_out, w.r_in, targets=tg)
+    err = _rel(a[tg, :3], d["acc_reg"])
+    assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2
+    if theta == 0.3:
+        check_neighbours(ctx, w, targets=tg)
+
+
+_C5 = {}
+
+
+def _tree5(w):
+    if "T" not in _C5:
+        _C5["T"] = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    return _C5["T"]
+
+
+def _ctx5(p3t, w):
+    if "ctx" not in _C5:
+        ctx = p3t.Context(0)
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        check_build(ctx, _tree5(w), w.pos_mass, 63)
+        _C5["ctx"] = ctx
+    return _C5["ctx"]
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nleaf,ncrit", [(8, 32), (16, 16), (1, 1), (32, 64)])
+def test_tree_parameters(p3t, nleaf, ncrit):
+    w = workloads.make_config(1, n_override=5001)            # ragged: not a multiple of 32 or of the sort tile
+    T = oracle.Tree(w.pos_mass, 63, nleaf, ncrit)
+    with p3t.Context(0, nleaf=nleaf, ncrit=ncrit) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        check_build(ctx, T, w.pos_mass, 63)
+        check_force(ctx, T, w, 0)
+        check_neighbours(ctx, w)
+
+
+def test_theta_to_zero_is_direct_sum(p3t):
+    """theta = 0 reduces the tree code to a direct-N code."""
+    w = workloads.make_config(1, n_override=3000)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        a = ctx.regular_force(w.r_out, w.r_in, 1e-3, 0).cpu().numpy().astype(np.float64)
+        npp, npc = ctx.list_lengths()
+        assert np.all(npc == 0) and np.all(npp == w.n)
+        d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
+        err = _rel(a[:, :3], d["acc_reg"])
+        assert err.max() < 2e-6 and np.median(err) < 2e-7
+        assert np.abs(a[:, 3] / d["phi_reg"] - 1).max() < 1e-6
+        check_neighbours(ctx, w)
+
+
+def test_two_bodies_in_each_zone(p3t):
+    """P2 on the GPU: |a| = m W / r^2 towards the partner (PAPER.md:66 zones, eq. 6)."""
+    r_out, r_in = 0.05, 0.005
+    with p3t.Context(0) as ctx:
+        for r in (0.001, 0.005, 0.0051, 0.02, 0.0275, 0.049, 0.05, 0.051, 0.3):
+            pm = np.array([[0.1, 0.2, 0.3, 0.25], [0.1 + r, 0.2, 0.3, 0.75]], dtype=np.float32)
+            ctx.build_tree(_cuda(pm), 63)
+            a = ctx.regular_force(r_out, r_in, 0.4, 0).cpu().numpy().astype(np.float64)
+            d = oracle.direct(pm, float(np.float32(r_out)), float(np.float32(r_in)))
+            rr = float(pm[1, 0]) - float(pm[0, 0])
+            Wv = oracle.W((rr - float(np.float32(r_in))) / (float(np.float32(r_out)) - float(np.float32(r_in))))
+            assert abs(a[0, 0] - 0.75 * Wv / rr ** 2) <= 2e-6 * 0.75 / rr ** 2
+            assert abs(a[1, 0] + 0.25 * Wv / rr ** 2) <= 2e-6 * 0.25 / rr ** 2
+            assert np.abs(a[:, :3] - d["acc_reg"]).max() <= 2e-6 * 0.75 / rr ** 2
+            assert np.abs(a[:, 3] - d["phi_reg"]).max() <= 2e-6 * np.abs(d["phi_reg"]).max()
+            off, idx = ctx.neighbours()
+            want = [1, 0] if np.float32(pm[1, 0] - pm[0, 0]) ** 2 < np.float32(r_out) ** 2 else []
+            assert idx.cpu().tolist() == want
+
+
+def test_degenerate_inputs(p3t):
+    with p3t.Context(0) as ctx:
+        # N = 1
+        pm = np.array([[1.0, 2.0, 3.0, 1.0]], dtype=np.float32)
+        ctx.build_tree(_cuda(pm), 63)
+        a = ctx.regular_force(0.05, 0.005, 0.4).cpu().numpy()
+        assert np.all(a == 0)
+        off, idx = ctx.neighbours()
+        assert off.cpu().tolist() == [0, 0] and idx.numel() == 0
+        # all particles coincident (reading R8): no force, phi_R = sum m psi(r_in), everybody is a neighbour
+        n = 100
+        pm = np.tile(np.array([[0.5, -0.25, 2.0, 0.01]], dtype=np.float32), (n, 1))
+        T = oracle.Tree(pm, 63, NLEAF, NCRIT)
+        ctx.build_tree(_cuda(pm), 63)
+        check_build(ctx, T, pm, 63)
+        a = ctx.regular_force(0.05, 0.005, 0.4).cpu().numpy().astype(np.float64)
+        assert np.all(a[:, :3] == 0)
+        psi_in = oracle.psi(0.0, float(np.float32(0.05)), float(np.float32(0.005)))
+        assert np.allclose(a[:, 3], (n - 1) * float(np.float32(0.01)) * psi_in, rtol=2e-6)
+        off, idx = ctx.neighbours()
+        assert np.all(np.diff(off.cpu().numpy()) == n - 1)
+        a1 = ctx.regular_force(0.05, 0.005, 0.4, 1).cpu().numpy()
+        assert np.all(a1 == 0)                                  # Newtonian potential skips r = 0 pairs
+        # collinear, and r_out larger than the whole system
+        n = 777
+        pm = np.zeros((n, 4), dtype=np.float32)
+        pm[:, 0] = np.linspace(-1, 1, n) ** 3; pm[:, 3] = 1.0 / n
+
+        class W: pass
+        w = W(); w.pos_mass = pm; w.r_out = 5.0; w.r_in = 0.5; w.theta = 0.4; w.n = n
+        T = oracle.Tree(pm, 63, NLEAF, NCRIT)
+        ctx.build_tree(_cuda(pm), 63)
+        check_build(ctx, T, pm, 63)
+        # symmetric line: the net force nearly cancels for the inner particles, so only the conditioned norms apply
+        check_force(ctx, T, w, 0, per_particle=False)
+        off, idx = check_neighbours(ctx, w)
+        assert off[-1] == n * (n - 1)
+        nb6 = ctx.neighbours_nbody6(n)
+        assert np.all(nb6[:, 0] == n - 1) and nb6[0, 1] == 2 and nb6[5, 1] == 1 and nb6[0, n - 1] == n
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.neighbours_nbody6(10)
+        assert e.value.code == p3t.ERANGE
+
+
+def test_error_codes(p3t):
+    import torch
+    with p3t.Context(0) as ctx:
+        out = torch.empty((4, 4), dtype=torch.float32, device="cuda")
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.n = 4
+            ctx.regular_force(0.05, 0.005, 0.4, out=out)
+        assert e.value.code == p3t.ESTATE
+        pm = _cuda(workloads.make_config(1, n_override=64).pos_mass)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.build_tree(pm, 42)
+        assert e.value.code == p3t.EINVAL
+        ctx.build_tree(pm, 63)
+        for bad in ((0.05, 0.05, 0.4), (0.05, -1.0, 0.4), (0.05, 0.005, 0.0), (float("nan"), 0.005, 0.4)):
+            with pytest.raises(p3t.P3TError) as e:
+                ctx.regular_force(*bad)
+            assert e.value.code == p3t.EINVAL
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.neighbours()
+        assert e.value.code == p3t.ESTATE
+        # NaN / Inf input is found by the bounding-cube reduction and reported by the next synchronising call
+        bad = pm.clone(); bad[7, 1] = float("nan")
+        ctx.build_tree(bad, 63)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.stats()
+        assert e.value.code == p3t.EINVAL
+        bad = pm.clone(); bad[3, 3] = float("inf")
+        ctx.build_tree(bad, 63)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.stats()
+        assert e.value.code == p3t.EINVAL
+        ctx.build_tree(pm, 63)                                  # the context recovers with good input
+        assert ctx.stats()["input_bad"] == 0
+
+
+def test_step_host_matches_device_path(p3t):
+    """The HOST-buffer entry point (what bench.py's e2e times) gives the same bits as the device path."""
+    w = workloads.make_config(2, n_override=40000)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        a = ctx.regular_force(w.r_out, w.r_in, w.theta).cpu().numpy()
+        off, idx = ctx.neighbours()
+        off = off.cpu().numpy(); idx = idx.cpu().numpy()
+        nb_off = np.empty(w.n + 1, dtype=np.int64); nb_idx = np.empty(idx.shape[0] + 10, dtype=np.int32)
+        acc, _, _, total = ctx.step_host(w.pos_mass, w.r_out, w.r_in, w.theta, nb_offsets=nb_off, nb_indices=nb_idx)
+        assert total == idx.shape[0]
+        assert np.array_equal(acc, a) and np.array_equal(nb_off, off) and np.array_equal(nb_idx[:total], idx)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.step_host(w.pos_mass, w.r_out, w.r_in, w.theta, nb_offsets=nb_off, nb_indices=nb_idx[:5])
+        assert e.value.code == p3t.ERANGE
+
+
+def test_theta_and_radii_change_without_rebuild(p3t, cfg1):
+    w = cfg1
+    T = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        for theta, ro in ((0.7, 0.05), (0.3, 0.02), (0.5, 0.11)):
+            class W: pass
+            v = W(); v.pos_mass = w.pos_mass; v.n = w.n; v.theta = theta
+            v.r_out = float(np.float32(ro)); v.r_in = float(np.float32(0.1 * ro))
+            check_force(ctx, T, v, 0)
+            check_neighbours(ctx, v, targets=workloads.sample_targets(w.n, 2000))
