@@ -14,8 +14,11 @@
 #define WALK_THREADS (WALK_WARPS * 32)
 #define STACK_CAP    512                  // per-warp node stack in shared memory; deeper entries spill
 #define SPILL_CAP    8192                 // per-warp spill (global memory), entries
-#define PC_TILE      32                   // cells evaluated per flush
-#define PP_TILE      64                   // particles evaluated per flush
+#define PC_TILE      32                   // cells: a flush is due at this fill level
+#define PP_TILE      64                   // particles: likewise
+#define PC_CAP       (PC_TILE + 32)       // one walk iteration appends at most 32 cells
+#define PP_CAP       (PP_TILE + 32)       // leaf particles are appended in chunks of at most 32
+#define FAR_AWAY     1.0e18f              // position of the zero-mass padding entries of a tile
 
 struct walk_consts {
     float rout2, rin2, r_in, inv_delta;   // inv_delta = 1 / (r_out - r_in)
@@ -43,13 +46,14 @@ struct walk_args {
     walk_consts K;
 };
 
-struct warp_smem {
-    int    stack[STACK_CAP];
-    float4 pc_com[PC_TILE + 32];
-    float4 pc_q0[PC_TILE + 32];
-    float2 pc_q1[PC_TILE + 32];
-    float4 pp_pos[PP_TILE + 32];
-    int    pp_j[PP_TILE + 32];
+// Per-warp list tiles, structure-of-arrays so that two (LDS.64) or four (LDS.128) consecutive
+// entries arrive as the packed operands of the f32x2 instructions below.
+// pc rows: 0-2 COM, 3 M, 4-9 MINUS the traceless quadrupole (xx yy zz xy xz yz).
+struct __align__(16) warp_smem {
+    int   stack[STACK_CAP];
+    float pc[10][PC_CAP];
+    float pp[4][PP_CAP];        // x y z m
+    int   ppj[PP_CAP];          // sorted position of the source
 };
 
 __device__ __forceinline__ float rsqrt_approx(float x)
@@ -58,6 +62,18 @@ __device__ __forceinline__ float rsqrt_approx(float x)
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+
+// ---- packed fp32 pairs: Blackwell's FADD2 / FMUL2 / FFMA2 (PTX add/mul/fma.rn.f32x2) retire two
+// IEEE-rn fp32 operations per lane and issue slot; measured on B200 they reach the same
+// 128 lanes/clk/SM as FFMA with half the issue slots, which is what an issue-bound loop needs.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float f2lo(f2 v) { float a; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }
+__device__ __forceinline__ float f2hi(f2 v) { float b; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
 // eq. 6, 0 < x < 1: W = x^4 (35 - 84 x + 70 x^2 - 20 x^3); evaluated through the
 // symmetry W(x) = 1 - W(1 - x) above x = 1/2 so that fp32 Horner never cancels.
@@ -77,9 +93,13 @@ __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float
     return -W * rinv - K.k140 * integral;
 }
 
+// NS target slots per lane.  Every accumulator is a packed pair: .lo sums the even list entries,
+// .hi the odd ones.  ph accumulates MINUS the potential of the far terms; the rare near-zone terms
+// (cutoff branch) go to the scalar n* accumulators with their true sign.
 template <int NS> struct target {
     float x[NS], y[NS], z[NS];
-    float ax[NS], ay[NS], az[NS], ph[NS];        // fp32 partial sums of the current tile
+    f2    ax[NS], ay[NS], az[NS], ph[NS];        // fp32 partial sums of the current tile
+    float nax[NS], nay[NS], naz[NS], nph[NS];
     double dax[NS], day[NS], daz[NS], dph[NS];   // fp64 masters (R-S9)
     int   id[NS];                                // sorted position of the target, -1 = no target
     long long cur[NS];                           // neighbour write cursor (MODE 1) / count (MODE 0)
@@ -87,82 +107,196 @@ template <int NS> struct target {
 
 template <int NS> __device__ __forceinline__ void fold(target<NS>& T)
 {
+    const f2 zero = pk(0.0f, 0.0f);
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        T.dax[s] += (double)T.ax[s]; T.day[s] += (double)T.ay[s]; T.daz[s] += (double)T.az[s]; T.dph[s] += (double)T.ph[s];
-        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = 0.0f;
+        T.dax[s] += (double)((f2lo(T.ax[s]) + f2hi(T.ax[s])) + T.nax[s]);
+        T.day[s] += (double)((f2lo(T.ay[s]) + f2hi(T.ay[s])) + T.nay[s]);
+        T.daz[s] += (double)((f2lo(T.az[s]) + f2hi(T.az[s])) + T.naz[s]);
+        T.dph[s] += (double)(T.nph[s] - (f2lo(T.ph[s]) + f2hi(T.ph[s])));
+        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = zero;
+        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
     }
 }
 
-// R-S8 particle-cell: monopole + traceless quadrupole, r = x_i - COM
-//   phi = -M/R - (1/2) r.Q.r / R^5 ;  a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7
+// R-S8 particle-cell, monopole + traceless quadrupole, two cells per packed operation.
+// With d = COM - x_i (= -r), Q' = -Q (stored negated in the tile), R = |d|:
+//   q' = d.Q'.d / R^5,  -phi = M/R - q'/2,  a = (M/R - (5/2) q') d / R^2 + (Q'.d) / R^5
+// which is a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7 of R-S8: 33 packed operations per pair.
+template <int NS> __device__ __forceinline__ void pc_pair(target<NS>& T, f2 cx, f2 cy, f2 cz, f2 cm,
+                                                          f2 qxx, f2 qyy, f2 qzz, f2 qxy, f2 qxz, f2 qyz)
+{
+    const f2 mhalf = pk(-0.5f, -0.5f), m52 = pk(-2.5f, -2.5f);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const f2 dx = sub2(cx, pk(T.x[s], T.x[s])), dy = sub2(cy, pk(T.y[s], T.y[s])), dz = sub2(cz, pk(T.z[s], T.z[s]));
+        const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
+        const f2 ri2 = mul2(ri, ri);
+        const f2 qx = fma2(qxz, dz, fma2(qxy, dy, mul2(qxx, dx)));
+        const f2 qy = fma2(qyz, dz, fma2(qyy, dy, mul2(qxy, dx)));
+        const f2 qz = fma2(qzz, dz, fma2(qyz, dy, mul2(qxz, dx)));
+        const f2 dqd = fma2(dz, qz, fma2(dy, qy, mul2(dx, qx)));
+        const f2 ri3 = mul2(ri2, ri), ri5 = mul2(ri3, ri2);
+        const f2 mono = mul2(cm, ri);
+        const f2 q5 = mul2(dqd, ri5);
+        T.ph[s] = fma2(mhalf, q5, add2(T.ph[s], mono));
+        const f2 cr = mul2(fma2(m52, q5, mono), ri2);
+        T.ax[s] = fma2(qx, ri5, fma2(cr, dx, T.ax[s]));
+        T.ay[s] = fma2(qy, ri5, fma2(cr, dy, T.ay[s]));
+        T.az[s] = fma2(qz, ri5, fma2(cr, dz, T.az[s]));
+    }
+}
+
+// cnt is a multiple of 4 (the tail of a list is padded with zero-mass cells FAR_AWAY)
 template <int NS> __device__ __forceinline__ void eval_pc(target<NS>& T, const warp_smem& S, int cnt)
 {
-#pragma unroll 2
-    for (int e = 0; e < cnt; ++e) {
-        const float4 cm = S.pc_com[e], q0 = S.pc_q0[e];
-        const float2 q1 = S.pc_q1[e];
+#pragma unroll 1
+    for (int e = 0; e < cnt; e += 4) {
+        ulonglong2 v[10];
 #pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            const float rx = T.x[s] - cm.x, ry = T.y[s] - cm.y, rz = T.z[s] - cm.z;
-            const float R2 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));
-            const float ri = rsqrt_approx(R2), ri2 = ri * ri;
-            const float qx = fmaf(q1.x, rz, fmaf(q0.w, ry, q0.x * rx));      // (Q r)_x = xx rx + xy ry + xz rz
-            const float qy = fmaf(q1.y, rz, fmaf(q0.y, ry, q0.w * rx));      // xy rx + yy ry + yz rz
-            const float qz = fmaf(q0.z, rz, fmaf(q1.y, ry, q1.x * rx));      // xz rx + yz ry + zz rz
-            const float rqr = fmaf(rz, qz, fmaf(ry, qy, rx * qx));
-            const float ri3 = ri2 * ri, ri5 = ri3 * ri2;
-            const float mono = cm.w * ri;                                      // M / R
-            const float quad = 0.5f * rqr * ri5;                               // (1/2) rQr / R^5
-            T.ph[s] -= mono + quad;
-            const float cr = -(mono + 5.0f * quad) * ri2;                      // -(M/R^3 + (5/2) rQr/R^7)
-            T.ax[s] += fmaf(cr, rx, qx * ri5);
-            T.ay[s] += fmaf(cr, ry, qy * ri5);
-            T.az[s] += fmaf(cr, rz, qz * ri5);
-        }
+        for (int k = 0; k < 10; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&S.pc[k][e]);
+        pc_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
+        pc_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
     }
 }
 
-// R10 + eq. 6: particle-particle with cutoff; MODE 0 counts neighbours only, MODE 1 also emits
+// Two sources per packed operation: the far zone (d2 >= r_out^2, W = 1, pure Newtonian) of the
+// p-p list, branch-free.  d2 follows R10 bit for bit (sub, mul, fma, fma; all rn).  A near pair is
+// masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
+// by the lane is returned so that the caller knows whether the tile needs the near pass.
+template <int NS>
+__device__ __forceinline__ float pp_far_pair(target<NS>& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
+{
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const f2 dx = sub2(px, pk(T.x[s], T.x[s])), dy = sub2(py, pk(T.y[s], T.y[s])), dz = sub2(pz, pk(T.z[s], T.z[s]));
+        const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        const float d2a = f2lo(d2), d2b = f2hi(d2);
+        dmin = fminf(dmin, fminf(d2a, d2b));
+        const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
+        const f2 mri = mul2(pm, ri);
+        const f2 f = mul2(mri, mul2(ri, ri));
+        T.ph[s] = add2(T.ph[s], mri);
+        T.ax[s] = fma2(f, dx, T.ax[s]); T.ay[s] = fma2(f, dy, T.ay[s]); T.az[s] = fma2(f, dz, T.az[s]);
+    }
+    return dmin;
+}
+
+// R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission (MODE 1) or count (MODE 0) and the
+// cutoff-weighted pair term.  Scalar pass over a tile, run only by warps whose tile came within
+// r_out of one of their targets (about one tile in eight).
 template <int NS, int MODE>
-__device__ __forceinline__ void eval_pp(target<NS>& T, const warp_smem& S, int cnt, const walk_args& A)
+__device__ __forceinline__ void pp_near_pass(target<NS>& T, const warp_smem& S, int cnt, const walk_args& A)
 {
     const walk_consts& K = A.K;
-#pragma unroll 2
+#pragma unroll 1
     for (int e = 0; e < cnt; ++e) {
-        const float4 p = S.pp_pos[e];
+        const float px = S.pp[0][e], py = S.pp[1][e], pz = S.pp[2][e];
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
-            const float dx = __fsub_rn(p.x, T.x[s]), dy = __fsub_rn(p.y, T.y[s]), dz = __fsub_rn(p.z, T.z[s]);
+            const float dx = __fsub_rn(px, T.x[s]), dy = __fsub_rn(py, T.y[s]), dz = __fsub_rn(pz, T.z[s]);
             const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
             if (d2 < K.rout2) {
-                const int j = S.pp_j[e];
-                if (T.id[s] >= 0 && j != T.id[s]) {                  // self excluded by index
+                const int j = S.ppj[e];
+                if (T.id[s] >= 0 && j != T.id[s]) {                  // self excluded by index; idle lanes
                     if (MODE == 1) A.nbraw[T.cur[s]] = (int32_t)A.order[j];
                     T.cur[s]++;
                     if (MODE == 1) {
+                        const float m = S.pp[3][e];
                         if (d2 > K.rin2) {
                             const float ri = rsqrt_approx(d2), r = d2 * ri;
                             const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
                             const float W = cutoff_W(x);
-                            const float f = p.w * W * ri * ri * ri;
-                            T.ax[s] = fmaf(f, dx, T.ax[s]); T.ay[s] = fmaf(f, dy, T.ay[s]); T.az[s] = fmaf(f, dz, T.az[s]);
-                            T.ph[s] += K.pot_mode == 0 ? p.w * cutoff_psi(K, x, W, ri) : -p.w * ri;
+                            const float f = m * W * ri * ri * ri;
+                            T.nax[s] = fmaf(f, dx, T.nax[s]); T.nay[s] = fmaf(f, dy, T.nay[s]); T.naz[s] = fmaf(f, dz, T.naz[s]);
+                            T.nph[s] += K.pot_mode == 0 ? m * cutoff_psi(K, x, W, ri) : -m * ri;
                         } else if (K.pot_mode == 0) {
-                            T.ph[s] = fmaf(p.w, K.psi_in, T.ph[s]);    // inside r_in: constant psi(r_in), also r = 0 (R8)
+                            T.nph[s] = fmaf(m, K.psi_in, T.nph[s]);    // inside r_in: constant psi(r_in), also r = 0 (R8)
                         } else if (d2 > 0.0f) {
-                            T.ph[s] -= p.w * rsqrt_approx(d2);
+                            T.nph[s] -= m * rsqrt_approx(d2);
                         }
                     }
                 }
-            } else if (MODE == 1) {
-                const float ri = rsqrt_approx(d2);
-                const float mr = p.w * ri, mr3 = mr * ri * ri;
-                T.ph[s] -= mr;
-                T.ax[s] = fmaf(mr3, dx, T.ax[s]); T.ay[s] = fmaf(mr3, dy, T.ay[s]); T.az[s] = fmaf(mr3, dz, T.az[s]);
             }
         }
     }
+}
+
+// cnt is a multiple of 4 (tail padded with zero-mass particles FAR_AWAY, index -1)
+template <int NS, int MODE>
+__device__ __forceinline__ void eval_pp(target<NS>& T, const warp_smem& S, int cnt, const walk_args& A)
+{
+    if (MODE == 1) {
+        float dmin = INFINITY;
+#pragma unroll 1
+        for (int e = 0; e < cnt; e += 4) {
+            ulonglong2 v[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&S.pp[k][e]);
+            dmin = pp_far_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
+            dmin = pp_far_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
+        }
+        if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
+    }
+    pp_near_pass<NS, MODE>(T, S, cnt, A);     // the count pass (MODE 0) walks only cells within r_out
+}
+
+// pad the p-c tile from `fill` up to the next multiple of 4 with zero-mass cells; returns that multiple
+__device__ __forceinline__ int pad_pc(warp_smem& S, int fill, int lane)
+{
+    const int n4 = (fill + 3) & ~3;
+    if (lane < n4 - fill) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) S.pc[k][fill + lane] = k < 3 ? FAR_AWAY : 0.0f;
+    }
+    __syncwarp();
+    return n4;
+}
+__device__ __forceinline__ int pad_pp(warp_smem& S, int fill, int lane)
+{
+    const int n4 = (fill + 3) & ~3;
+    if (lane < n4 - fill) {
+        S.pp[0][fill + lane] = S.pp[1][fill + lane] = S.pp[2][fill + lane] = FAR_AWAY;
+        S.pp[3][fill + lane] = 0.0f; S.ppj[fill + lane] = -1;
+    }
+    __syncwarp();
+    return n4;
+}
+// after the first n4 entries (multiple of 4) were evaluated, move the 0..3 left over to the front
+__device__ __forceinline__ int shift_pc(warp_smem& S, int fill, int n4, int lane)
+{
+    const int rest = fill - n4;
+    float t[10];
+    if (lane < rest) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) t[k] = S.pc[k][n4 + lane];
+    }
+    __syncwarp();
+    if (lane < rest) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) S.pc[k][lane] = t[k];
+    }
+    __syncwarp();
+    return rest;
+}
+__device__ __forceinline__ int shift_pp(warp_smem& S, int fill, int n4, int lane)
+{
+    const int rest = fill - n4;
+    float t[4]; int j = 0;
+    if (lane < rest) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) t[k] = S.pp[k][n4 + lane];
+        j = S.ppj[n4 + lane];
+    }
+    __syncwarp();
+    if (lane < rest) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) S.pp[k][lane] = t[k];
+        S.ppj[lane] = j;
+    }
+    __syncwarp();
+    return rest;
 }
 
 __device__ __forceinline__ int stack_get(const warp_smem& S, const int32_t* spill, int i)
@@ -190,7 +324,8 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
         const bool v = i < ge;
         const float4 p = v ? A.spm[i] : pfirst;
         T.x[s] = p.x; T.y[s] = p.y; T.z[s] = p.z;
-        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = 0.0f;
+        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = pk(0.0f, 0.0f);
+        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
         T.dax[s] = T.day[s] = T.daz[s] = T.dph[s] = 0.0;
         T.id[s] = v ? i : -1;
         T.cur[s] = 0;
@@ -209,104 +344,108 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
     int top = 1, npc = 0, npp = 0, fill_pc = 0, fill_pp = 0, overflow = 0;
     if (lane == 0) S.stack[0] = 0;
     __syncwarp();
-    while (top > 0) {
-        const int take = min(top, 32);
-        top -= take;
-        const bool valid = lane < take;
-        int node = 0;
-        if (valid) node = stack_get(S, spill, top + lane);
-        bool open = false;
+    // One more pass after the stack has emptied flushes the list tails, so that each evaluation
+    // loop exists once in the code (instruction-cache footprint).
+    for (bool more = true; more;) {
+        more = top > 0;
+        uint32_t lm = 0;                 // lanes holding an opened leaf
         int2 link = make_int2(0, 0);
-        float4 com = make_float4(0, 0, 0, 0);
-        if (valid) {
-            com = A.ncom[node];
-            const float4 lo = A.nlo[node], hi = A.nhi[node];
-            link = A.nlink[node];
-            // R-S7, every operation one fp32 rounding
-            const float ex = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], com.x)), __fsub_rn(com.x, ghi[0]));
-            const float ey = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], com.y)), __fsub_rn(com.y, ghi[1]));
-            const float ez = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], com.z)), __fsub_rn(com.z, ghi[2]));
-            const float fx = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], hi.x)), __fsub_rn(lo.x, ghi[0]));
-            const float fy = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], hi.y)), __fsub_rn(lo.y, ghi[1]));
-            const float fz = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], hi.z)), __fsub_rn(lo.z, ghi[2]));
-            const float d2 = fmaf(ez, ez, fmaf(ey, ey, __fmul_rn(ex, ex)));
-            const float b2 = fmaf(fz, fz, fmaf(fy, fy, __fmul_rn(fx, fx)));
-            const float u = __fadd_rn(s_lt[__float_as_int(hi.w)], lo.w);
-            const float rc2 = __fmul_rn(u, u);
-            const bool near = b2 < K.rout2;
-            open = MODE == 1 ? ((d2 < rc2) || near) : near;
-        }
-        const bool inner = valid && open && link.y > 0;
-        const bool leaf  = valid && open && link.y < 0;
-        const bool acc   = MODE == 1 && valid && !open;
-        // children of opened internal cells go on the stack
-        {
-            int c = inner ? link.y : 0, x = c;
+        if (more) {
+            const int take = min(top, 32);
+            top -= take;
+            const bool valid = lane < take;
+            int node = 0;
+            if (valid) node = stack_get(S, spill, top + lane);
+            bool open = false;
+            float4 com = make_float4(0, 0, 0, 0);
+            if (valid) {
+                com = A.ncom[node];
+                const float4 lo = A.nlo[node], hi = A.nhi[node];
+                link = A.nlink[node];
+                // R-S7, every operation one fp32 rounding
+                const float ex = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], com.x)), __fsub_rn(com.x, ghi[0]));
+                const float ey = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], com.y)), __fsub_rn(com.y, ghi[1]));
+                const float ez = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], com.z)), __fsub_rn(com.z, ghi[2]));
+                const float fx = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], hi.x)), __fsub_rn(lo.x, ghi[0]));
+                const float fy = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], hi.y)), __fsub_rn(lo.y, ghi[1]));
+                const float fz = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], hi.z)), __fsub_rn(lo.z, ghi[2]));
+                const float d2 = fmaf(ez, ez, fmaf(ey, ey, __fmul_rn(ex, ex)));
+                const float b2 = fmaf(fz, fz, fmaf(fy, fy, __fmul_rn(fx, fx)));
+                const float u = __fadd_rn(s_lt[__float_as_int(hi.w)], lo.w);
+                const float rc2 = __fmul_rn(u, u);
+                const bool near = b2 < K.rout2;
+                open = MODE == 1 ? ((d2 < rc2) || near) : near;
+            }
+            const bool inner = valid && open && link.y > 0;
+            const bool leaf  = valid && open && link.y < 0;
+            const bool acc   = MODE == 1 && valid && !open;
+            // children of opened internal cells go on the stack
+            {
+                int c = inner ? link.y : 0, x = c;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-            const int total = __shfl_sync(0xffffffffu, x, 31);
-            if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
-            int w = top + x - c;
-            for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
-            top += total;
-        }
-        // accepted cells go on the particle-cell tile
-        if (MODE == 1) {
-            const uint32_t m = __ballot_sync(0xffffffffu, acc);
-            if (acc) {
-                const int w = fill_pc + __popc(m & lt_mask);
-                S.pc_com[w] = com; S.pc_q0[w] = A.nq0[node]; S.pc_q1[w] = A.nq1[node];
+                for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+                const int total = __shfl_sync(0xffffffffu, x, 31);
+                if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
+                int w = top + x - c;
+                for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
+                top += total;
             }
-            fill_pc += __popc(m);
-            npc += __popc(m);
-        }
-        // opened leaves: their particles go on the particle-particle tile
-        uint32_t lm = __ballot_sync(0xffffffffu, leaf);
-        __syncwarp();
-        while (lm) {
-            const int src = __ffs(lm) - 1;
-            lm &= lm - 1;
-            const int lb = __shfl_sync(0xffffffffu, link.x, src);
-            const int lc = -__shfl_sync(0xffffffffu, link.y, src);
-            npp += lc;
-            for (int o = 0; o < lc; o += 32) {
-                const int m = min(32, lc - o);
-                if (lane < m) { S.pp_pos[fill_pp + lane] = A.spm[lb + o + lane]; S.pp_j[fill_pp + lane] = lb + o + lane; }
-                fill_pp += m;
-                __syncwarp();
-                if (fill_pp >= PP_TILE) {
-                    eval_pp<NS, MODE>(T, S, PP_TILE, A);
-                    if (MODE == 1) fold(T);
-                    __syncwarp();
-                    const int rest = fill_pp - PP_TILE;
-                    float4 tp; int tj;
-                    if (lane < rest) { tp = S.pp_pos[PP_TILE + lane]; tj = S.pp_j[PP_TILE + lane]; }
-                    __syncwarp();
-                    if (lane < rest) { S.pp_pos[lane] = tp; S.pp_j[lane] = tj; }
-                    fill_pp = rest;
-                    __syncwarp();
+            // accepted cells go on the particle-cell tile
+            if (MODE == 1) {
+                const uint32_t m = __ballot_sync(0xffffffffu, acc);
+                if (acc) {
+                    const int w = fill_pc + __popc(m & lt_mask);
+                    const float4 q0 = A.nq0[node]; const float2 q1 = A.nq1[node];
+                    S.pc[0][w] = com.x; S.pc[1][w] = com.y; S.pc[2][w] = com.z; S.pc[3][w] = com.w;
+                    S.pc[4][w] = -q0.x; S.pc[5][w] = -q0.y; S.pc[6][w] = -q0.z; S.pc[7][w] = -q0.w;
+                    S.pc[8][w] = -q1.x; S.pc[9][w] = -q1.y;
                 }
+                fill_pc += __popc(m);
+                npc += __popc(m);
             }
+            lm = __ballot_sync(0xffffffffu, leaf);
         }
-        if (MODE == 1 && fill_pc >= PC_TILE) {
-            __syncwarp();
-            eval_pc<NS>(T, S, PC_TILE);
+        __syncwarp();
+        // opened leaves: their particles go on the particle-particle tile, 32 at a time
+        int src_b = 0, src_left = 0;
+        for (;;) {
+            if (src_left == 0 && lm != 0) {
+                const int src = __ffs(lm) - 1;
+                lm &= lm - 1;
+                src_b = __shfl_sync(0xffffffffu, link.x, src);
+                src_left = -__shfl_sync(0xffffffffu, link.y, src);
+                npp += src_left;
+            }
+            if (src_left > 0) {
+                const int m = min(32, src_left);
+                if (lane < m) {
+                    const float4 p = A.spm[src_b + lane];
+                    const int w = fill_pp + lane;
+                    S.pp[0][w] = p.x; S.pp[1][w] = p.y; S.pp[2][w] = p.z; S.pp[3][w] = p.w; S.ppj[w] = src_b + lane;
+                }
+                fill_pp += m; src_b += m; src_left -= m;
+                __syncwarp();
+            }
+            const bool drained = src_left == 0 && lm == 0;
+            const bool last = !more && drained;
+            if (fill_pp >= PP_TILE || (last && fill_pp > 0)) {
+                const int n4 = last ? pad_pp(S, fill_pp, lane) : (fill_pp & ~3);
+                eval_pp<NS, MODE>(T, S, n4, A);
+                if (MODE == 1) fold(T);
+                __syncwarp();
+                fill_pp = last ? 0 : shift_pp(S, fill_pp, n4, lane);
+            }
+            if (drained) break;
+        }
+        if (MODE == 1 && (fill_pc >= PC_TILE || (!more && fill_pc > 0))) {
+            const int n4 = more ? (fill_pc & ~3) : pad_pc(S, fill_pc, lane);
+            eval_pc<NS>(T, S, n4);
             fold(T);
             __syncwarp();
-            const int rest = fill_pc - PC_TILE;
-            float4 a, b; float2 c;
-            if (lane < rest) { a = S.pc_com[PC_TILE + lane]; b = S.pc_q0[PC_TILE + lane]; c = S.pc_q1[PC_TILE + lane]; }
-            __syncwarp();
-            if (lane < rest) { S.pc_com[lane] = a; S.pc_q0[lane] = b; S.pc_q1[lane] = c; }
-            fill_pc = rest;
+            fill_pc = more ? shift_pc(S, fill_pc, n4, lane) : 0;
         }
         __syncwarp();
     }
-    // tails
-    __syncwarp();
-    if (fill_pp > 0) { eval_pp<NS, MODE>(T, S, fill_pp, A); if (MODE == 1) fold(T); }
-    if (MODE == 1 && fill_pc > 0) { eval_pc<NS>(T, S, fill_pc); fold(T); }
-    __syncwarp();
 
     // a11: results to the caller's order
 #pragma unroll
