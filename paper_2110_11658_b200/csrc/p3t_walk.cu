@@ -9,6 +9,7 @@
 // DESIGN.md R-S7 (opening rule, bit-specified fp32), R-S8 (evaluation), R-S9 (accumulation),
 // R10 (neighbour predicate, bit-specified fp32).
 #include "p3t_internal.cuh"
+#include <stdlib.h>
 
 #define WALK_WARPS   4                    // warps per CTA, each walks its own groups
 #define WALK_THREADS (WALK_WARPS * 32)
@@ -44,6 +45,7 @@ struct walk_args {
     int32_t* spill;
     p3t_devinfo* info;
     walk_consts K;
+    int dbg;
 };
 
 // Per-warp list tiles, structure-of-arrays so that two (LDS.64) or four (LDS.128) consecutive
@@ -98,7 +100,9 @@ __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float
 // (cutoff branch) go to the scalar n* accumulators with their true sign.
 template <int NS> struct target {
     float x[NS], y[NS], z[NS];
-    f2    ax[NS], ay[NS], az[NS], ph[NS];        // fp32 partial sums of the current tile
+    f2    ph[NS];                                // fp32 partial sums of the current tile: -potential (packed)
+    float axe[NS], aye[NS], aze[NS];             // acceleration from the even list entries ...
+    float axo[NS], ayo[NS], azo[NS];             // ... and from the odd ones (scalar FFMAs, see pc_pair)
     float nax[NS], nay[NS], naz[NS], nph[NS];
     double dax[NS], day[NS], daz[NS], dph[NS];   // fp64 masters (R-S9)
     int   id[NS];                                // sorted position of the target, -1 = no target
@@ -110,11 +114,12 @@ template <int NS> __device__ __forceinline__ void fold(target<NS>& T)
     const f2 zero = pk(0.0f, 0.0f);
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        T.dax[s] += (double)((f2lo(T.ax[s]) + f2hi(T.ax[s])) + T.nax[s]);
-        T.day[s] += (double)((f2lo(T.ay[s]) + f2hi(T.ay[s])) + T.nay[s]);
-        T.daz[s] += (double)((f2lo(T.az[s]) + f2hi(T.az[s])) + T.naz[s]);
+        T.dax[s] += (double)((T.axe[s] + T.axo[s]) + T.nax[s]);
+        T.day[s] += (double)((T.aye[s] + T.ayo[s]) + T.nay[s]);
+        T.daz[s] += (double)((T.aze[s] + T.azo[s]) + T.naz[s]);
         T.dph[s] += (double)(T.nph[s] - (f2lo(T.ph[s]) + f2hi(T.ph[s])));
-        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = zero;
+        T.ph[s] = zero;
+        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
         T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
     }
 }
@@ -142,9 +147,12 @@ template <int NS> __device__ __forceinline__ void pc_pair(target<NS>& T, f2 cx, 
         const f2 q5 = mul2(dqd, ri5);
         T.ph[s] = fma2(mhalf, q5, add2(T.ph[s], mono));
         const f2 cr = mul2(fma2(m52, q5, mono), ri2);
-        T.ax[s] = fma2(qx, ri5, fma2(cr, dx, T.ax[s]));
-        T.ay[s] = fma2(qy, ri5, fma2(cr, dy, T.ay[s]));
-        T.az[s] = fma2(qz, ri5, fma2(cr, dz, T.az[s]));
+        // An FFMA2 with three distinct register-pair operands occupies the pipe for 3 cycles (measured:
+        // operand bandwidth), two scalar FFMAs for 2: the accumulations are issued on the halves.
+        const float crl = f2lo(cr), crh = f2hi(cr), r5l = f2lo(ri5), r5h = f2hi(ri5);
+        T.axe[s] = fmaf(f2lo(qx), r5l, fmaf(crl, f2lo(dx), T.axe[s])); T.axo[s] = fmaf(f2hi(qx), r5h, fmaf(crh, f2hi(dx), T.axo[s]));
+        T.aye[s] = fmaf(f2lo(qy), r5l, fmaf(crl, f2lo(dy), T.aye[s])); T.ayo[s] = fmaf(f2hi(qy), r5h, fmaf(crh, f2hi(dy), T.ayo[s]));
+        T.aze[s] = fmaf(f2lo(qz), r5l, fmaf(crl, f2lo(dz), T.aze[s])); T.azo[s] = fmaf(f2hi(qz), r5h, fmaf(crh, f2hi(dz), T.azo[s]));
     }
 }
 
@@ -178,7 +186,10 @@ __device__ __forceinline__ float pp_far_pair(target<NS>& T, f2 px, f2 py, f2 pz,
         const f2 mri = mul2(pm, ri);
         const f2 f = mul2(mri, mul2(ri, ri));
         T.ph[s] = add2(T.ph[s], mri);
-        T.ax[s] = fma2(f, dx, T.ax[s]); T.ay[s] = fma2(f, dy, T.ay[s]); T.az[s] = fma2(f, dz, T.az[s]);
+        const float fl = f2lo(f), fh = f2hi(f);
+        T.axe[s] = fmaf(fl, f2lo(dx), T.axe[s]); T.axo[s] = fmaf(fh, f2hi(dx), T.axo[s]);
+        T.aye[s] = fmaf(fl, f2lo(dy), T.aye[s]); T.ayo[s] = fmaf(fh, f2hi(dy), T.ayo[s]);
+        T.aze[s] = fmaf(fl, f2lo(dz), T.aze[s]); T.azo[s] = fmaf(fh, f2hi(dz), T.azo[s]);
     }
     return dmin;
 }
@@ -324,7 +335,8 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
         const bool v = i < ge;
         const float4 p = v ? A.spm[i] : pfirst;
         T.x[s] = p.x; T.y[s] = p.y; T.z[s] = p.z;
-        T.ax[s] = T.ay[s] = T.az[s] = T.ph[s] = pk(0.0f, 0.0f);
+        T.ph[s] = pk(0.0f, 0.0f);
+        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
         T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
         T.dax[s] = T.day[s] = T.daz[s] = T.dph[s] = 0.0;
         T.id[s] = v ? i : -1;
@@ -348,8 +360,8 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
     // loop exists once in the code (instruction-cache footprint).
     for (bool more = true; more;) {
         more = top > 0;
-        uint32_t lm = 0;                 // lanes holding an opened leaf
         int2 link = make_int2(0, 0);
+        int lc_incl = 0, lc_excl = 0, src_total = 0;
         if (more) {
             const int take = min(top, 32);
             top -= take;
@@ -357,11 +369,13 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
             int node = 0;
             if (valid) node = stack_get(S, spill, top + lane);
             bool open = false;
-            float4 com = make_float4(0, 0, 0, 0);
+            float4 com = make_float4(0, 0, 0, 0), q0 = com;
+            float2 q1 = make_float2(0, 0);
             if (valid) {
                 com = A.ncom[node];
                 const float4 lo = A.nlo[node], hi = A.nhi[node];
                 link = A.nlink[node];
+                if (MODE == 1) { q0 = A.nq0[node]; q1 = A.nq1[node]; }   // with the node, not after the test: one L2 round trip
                 // R-S7, every operation one fp32 rounding
                 const float ex = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], com.x)), __fsub_rn(com.x, ghi[0]));
                 const float ey = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], com.y)), __fsub_rn(com.y, ghi[1]));
@@ -395,7 +409,6 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
                 const uint32_t m = __ballot_sync(0xffffffffu, acc);
                 if (acc) {
                     const int w = fill_pc + __popc(m & lt_mask);
-                    const float4 q0 = A.nq0[node]; const float2 q1 = A.nq1[node];
                     S.pc[0][w] = com.x; S.pc[1][w] = com.y; S.pc[2][w] = com.z; S.pc[3][w] = com.w;
                     S.pc[4][w] = -q0.x; S.pc[5][w] = -q0.y; S.pc[6][w] = -q0.z; S.pc[7][w] = -q0.w;
                     S.pc[8][w] = -q1.x; S.pc[9][w] = -q1.y;
@@ -403,34 +416,43 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
                 fill_pc += __popc(m);
                 npc += __popc(m);
             }
-            lm = __ballot_sync(0xffffffffu, leaf);
+            // opened leaves: inclusive scan of their particle counts, so that the copy below can
+            // take 32 particles per round whatever the leaf sizes are
+            lc_incl = leaf ? -link.y : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, lc_incl, o); if (lane >= o) lc_incl += y; }
+            src_total = __shfl_sync(0xffffffffu, lc_incl, 31);
+            lc_excl = lc_incl - (leaf ? -link.y : 0);
+            npp += src_total;
         }
         __syncwarp();
-        // opened leaves: their particles go on the particle-particle tile, 32 at a time
-        int src_b = 0, src_left = 0;
-        for (;;) {
-            if (src_left == 0 && lm != 0) {
-                const int src = __ffs(lm) - 1;
-                lm &= lm - 1;
-                src_b = __shfl_sync(0xffffffffu, link.x, src);
-                src_left = -__shfl_sync(0xffffffffu, link.y, src);
-                npp += src_left;
-            }
-            if (src_left > 0) {
-                const int m = min(32, src_left);
-                if (lane < m) {
-                    const float4 p = A.spm[src_b + lane];
-                    const int w = fill_pp + lane;
-                    S.pp[0][w] = p.x; S.pp[1][w] = p.y; S.pp[2][w] = p.z; S.pp[3][w] = p.w; S.ppj[w] = src_b + lane;
+        // particle k of this iteration's opened leaves belongs to the first lane whose inclusive
+        // count exceeds k (binary search by shuffle); 32 particles per round go on the p-p tile
+        for (int k0 = 0;; k0 += 32) {
+            const int m = min(32, src_total - k0);
+            if (m > 0) {
+                const int k = k0 + lane;
+                int pos = 0;
+#pragma unroll
+                for (int st = 16; st > 0; st >>= 1) {
+                    const int v = __shfl_sync(0xffffffffu, lc_incl, pos + st - 1);
+                    if (v <= k) pos += st;
                 }
-                fill_pp += m; src_b += m; src_left -= m;
+                pos = min(pos, 31);
+                const int j = __shfl_sync(0xffffffffu, link.x, pos) + (k - __shfl_sync(0xffffffffu, lc_excl, pos));
+                if (lane < m) {
+                    const float4 p = A.spm[j];
+                    const int w = fill_pp + lane;
+                    S.pp[0][w] = p.x; S.pp[1][w] = p.y; S.pp[2][w] = p.z; S.pp[3][w] = p.w; S.ppj[w] = j;
+                }
+                fill_pp += m;
                 __syncwarp();
             }
-            const bool drained = src_left == 0 && lm == 0;
+            const bool drained = k0 + 32 >= src_total;
             const bool last = !more && drained;
             if (fill_pp >= PP_TILE || (last && fill_pp > 0)) {
                 const int n4 = last ? pad_pp(S, fill_pp, lane) : (fill_pp & ~3);
-                eval_pp<NS, MODE>(T, S, n4, A);
+                if (!(A.dbg & 2)) eval_pp<NS, MODE>(T, S, n4, A);
                 if (MODE == 1) fold(T);
                 __syncwarp();
                 fill_pp = last ? 0 : shift_pp(S, fill_pp, n4, lane);
@@ -439,7 +461,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
         }
         if (MODE == 1 && (fill_pc >= PC_TILE || (!more && fill_pc > 0))) {
             const int n4 = more ? (fill_pc & ~3) : pad_pc(S, fill_pc, lane);
-            eval_pc<NS>(T, S, n4);
+            for (int rep = (A.dbg & 1) ? 0 : ((A.dbg & 8) ? 2 : 1); rep > 0; --rep) eval_pc<NS>(T, S, n4);
             fold(T);
             __syncwarp();
             fill_pc = more ? shift_pc(S, fill_pc, n4, lane) : 0;
@@ -467,7 +489,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(WALK_THREADS) k_walk(walk_args A)
+__global__ void __launch_bounds__(WALK_THREADS, 4) k_walk(walk_args A)
 {
     __shared__ warp_smem smem[WALK_WARPS];
     __shared__ float s_lt[24];
@@ -627,7 +649,8 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
         if (per_sm[0] < 1) per_sm[0] = 1;
         if (per_sm[1] < 1) per_sm[1] = 1;
     }
-    const int blocks0 = per_sm[0] * ctx->num_sms, blocks1 = per_sm[1] * ctx->num_sms;
+    int blocks0 = per_sm[0] * ctx->num_sms, blocks1 = per_sm[1] * ctx->num_sms;
+    if (getenv("P3T_CTAS")) blocks1 = atoi(getenv("P3T_CTAS")) * ctx->num_sms;
     const int maxblocks = blocks0 > blocks1 ? blocks0 : blocks1;
     int rc;
     if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)maxblocks * WALK_WARPS * SPILL_CAP * sizeof(int32_t)))) return rc;
@@ -644,6 +667,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.nbcount = P<int32_t>(ctx->nbcount); A.nboff = P<int64_t>(ctx->nboff);
     A.nbraw = nullptr; A.out = acc_pot; A.spill = P<int32_t>(ctx->spill); A.info = INFO(ctx);
     make_consts(A.K, r_out, r_in, theta, pot_mode);
+    A.dbg = getenv("P3T_DBG") ? atoi(getenv("P3T_DBG")) : 0;
 
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
     k_force_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx));
