@@ -62,6 +62,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
     int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
     if (rc == P3T_OK) rc = p3t_tree_init(c);
+    if (rc == P3T_OK) rc = p3t_walk_init(c);
     if (rc != P3T_OK) { p3t_destroy(c); return rc; }
     *out = c;
     return P3T_OK;
@@ -74,7 +75,7 @@ int p3t_destroy(p3t_ctx* c)
     cudaStreamSynchronize(c->stream);
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp,
-                        &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill,
+                        &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill, &c->pcpool, &c->pppool, &c->glist,
                         &c->info, &c->stage_in, &c->stage_out };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);

@@ -1,0 +1,553 @@
+// p3t_force.cu -- steps a8-a11: particle-cell and particle-particle regular force with
+// the cutoff of eq. 6 and neighbour-list emission fused in, results
+// scattered to the caller's particle order; plus the neighbour CSR bookkeeping (a10).
+//
+//   F_R,i = sum_j m_j W(x_ij) (x_j - x_i) / r_ij^3,  W = 1 - K,  x = (r - r_in)/(r_out - r_in)
+//   (eq. 1, 3, 4, 6, 8-10; attractive sign: DESIGN.md R1)
+//
+// One warp evaluates one target group (<= 64 particles, one or two target slots per lane) against
+// the interaction lists that k_walk<WALK_LISTS> left in HBM.  32 list entries at a time are gathered
+// (node / particle data, L2-resident) into a double-buffered structure-of-arrays tile in shared
+// memory while the previous tile is being evaluated, so the FP32 pipe never waits for the walk.
+// Rules: DESIGN.md R-S8 (evaluation), R-S9 (accumulation), R10 (neighbour predicate, bit-specified).
+#include "p3t_internal.cuh"
+#include <stdio.h>
+#include <stdlib.h>
+#include <math.h>
+
+#define FORCE_WARPS   4
+#define FORCE_THREADS (FORCE_WARPS * 32)
+#define TILE          32                  // list entries per tile
+#define FAR_AWAY      1.0e18f             // position of the zero-mass padding entries of a tile
+
+struct walk_consts {
+    float rout2, rin2, r_in, inv_delta;   // inv_delta = 1 / (r_out - r_in)
+    float psi_in;                          // psi(r_in), the constant regular pair potential inside r_in
+    float k140;                            // 140 / (r_out - r_in)
+    float s1;                              // S(1)
+    float sc[6];                           // S(t) = t (sc0 + t (sc1 + ... t sc5))
+    float rem;                             // c^3 (1+c)^3  (> 0)
+    float c;                               // r_in / (r_out - r_in)
+    float theta;
+    int   pot_mode;
+};
+
+struct force_args {
+    const float4* spm; const uint32_t* order;
+    const float4 *ncom, *nq0; const float2* nq1;
+    const int32_t* gbegin;
+    const uint4* glist;
+    const int32_t *pcpool, *pppool;
+    const int64_t* nboff;       // per ORIGINAL id
+    int32_t* nbraw;             // out: unsorted rows
+    float4* out;                // out: acc_pot, original order
+    p3t_devinfo* info;
+    walk_consts K;
+};
+
+// Per-warp list tiles, double-buffered, structure-of-arrays so that two (LDS.64) or four (LDS.128)
+// consecutive entries arrive as the packed operands of the f32x2 instructions below.
+// pc rows: 0-2 COM, 3 M, 4-9 MINUS the traceless quadrupole (xx yy zz xy xz yz).
+struct __align__(16) tile_smem {
+    float pc[2][10][TILE];
+    float pp[2][4][TILE];       // x y z m
+    int   ppj[2][TILE];         // sorted position of the source, -1 = padding
+};
+
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---- packed fp32 pairs: Blackwell's FADD2 / FMUL2 / FFMA2 (PTX add/mul/fma.rn.f32x2) retire two
+// IEEE-rn fp32 operations per lane and issue slot; measured on B200 they reach the same
+// 128 lanes/clk/SM as FFMA with half the issue slots, which is what an issue-bound loop needs.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float f2lo(f2 v) { float a; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }
+__device__ __forceinline__ float f2hi(f2 v) { float b; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+// eq. 6, 0 < x < 1: W = x^4 (35 - 84 x + 70 x^2 - 20 x^3); evaluated through the
+// symmetry W(x) = 1 - W(1 - x) above x = 1/2 so that fp32 Horner never cancels.
+__device__ __forceinline__ float cutoff_W(float x)
+{
+    float t = x > 0.5f ? 1.0f - x : x;
+    float t2 = t * t;
+    float w = t2 * t2 * (35.0f + t * (-84.0f + t * (70.0f - 20.0f * t)));
+    return x > 0.5f ? 1.0f - w : w;
+}
+
+// regular pair potential for r_in < r < r_out (R6): -W/r - (140/D) int_x^1 t^3(1-t)^3/(t+c) dt
+__device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float W, float rinv)
+{
+    float sx = x * (K.sc[0] + x * (K.sc[1] + x * (K.sc[2] + x * (K.sc[3] + x * (K.sc[4] + x * K.sc[5])))));
+    float integral = (K.s1 - sx) - K.rem * __logf((1.0f + K.c) / (x + K.c));
+    return -W * rinv - K.k140 * integral;
+}
+
+// NS target slots per lane.  Every accumulator is a packed pair: .lo sums the even list entries,
+// .hi the odd ones.  ph accumulates MINUS the potential of the far terms; the rare near-zone terms
+// (cutoff branch) go to the scalar n* accumulators with their true sign.
+template <int NS> struct target {
+    float x[NS], y[NS], z[NS];
+    f2    ph[NS];                                // fp32 partial sums of the current tile: -potential (packed)
+    float axe[NS], aye[NS], aze[NS];             // acceleration from the even list entries ...
+    float axo[NS], ayo[NS], azo[NS];             // ... and from the odd ones (scalar FFMAs, see pc_pair)
+    float nax[NS], nay[NS], naz[NS], nph[NS];
+    double dax[NS], day[NS], daz[NS], dph[NS];   // fp64 masters (R-S9)
+    int   id[NS];                                // sorted position of the target, -1 = no target
+    long long cur[NS];                           // neighbour write cursor
+};
+
+template <int NS> __device__ __forceinline__ void fold(target<NS>& T)
+{
+    const f2 zero = pk(0.0f, 0.0f);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        T.dax[s] += (double)((T.axe[s] + T.axo[s]) + T.nax[s]);
+        T.day[s] += (double)((T.aye[s] + T.ayo[s]) + T.nay[s]);
+        T.daz[s] += (double)((T.aze[s] + T.azo[s]) + T.naz[s]);
+        T.dph[s] += (double)(T.nph[s] - (f2lo(T.ph[s]) + f2hi(T.ph[s])));
+        T.ph[s] = zero;
+        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
+        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
+    }
+}
+
+// R-S8 particle-cell, monopole + traceless quadrupole, two cells per packed operation.
+// With d = COM - x_i (= -r), Q' = -Q (stored negated in the tile), R = |d|:
+//   q' = d.Q'.d / R^5,  -phi = M/R - q'/2,  a = (M/R - (5/2) q') d / R^2 + (Q'.d) / R^5
+// which is a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7 of R-S8: 33 packed operations per pair.
+template <int NS> __device__ __forceinline__ void pc_pair(target<NS>& T, f2 cx, f2 cy, f2 cz, f2 cm,
+                                                          f2 qxx, f2 qyy, f2 qzz, f2 qxy, f2 qxz, f2 qyz)
+{
+    const f2 mhalf = pk(-0.5f, -0.5f), m52 = pk(-2.5f, -2.5f);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const f2 dx = sub2(cx, pk(T.x[s], T.x[s])), dy = sub2(cy, pk(T.y[s], T.y[s])), dz = sub2(cz, pk(T.z[s], T.z[s]));
+        const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
+        const f2 ri2 = mul2(ri, ri);
+        const f2 qx = fma2(qxz, dz, fma2(qxy, dy, mul2(qxx, dx)));
+        const f2 qy = fma2(qyz, dz, fma2(qyy, dy, mul2(qxy, dx)));
+        const f2 qz = fma2(qzz, dz, fma2(qyz, dy, mul2(qxz, dx)));
+        const f2 dqd = fma2(dz, qz, fma2(dy, qy, mul2(dx, qx)));
+        const f2 ri3 = mul2(ri2, ri), ri5 = mul2(ri3, ri2);
+        const f2 mono = mul2(cm, ri);
+        const f2 q5 = mul2(dqd, ri5);
+        T.ph[s] = fma2(mhalf, q5, add2(T.ph[s], mono));
+        const f2 cr = mul2(fma2(m52, q5, mono), ri2);
+        // An FFMA2 with three distinct register-pair operands occupies the pipe for 3 cycles (measured:
+        // operand bandwidth), two scalar FFMAs for 2: the accumulations are issued on the halves.
+        const float crl = f2lo(cr), crh = f2hi(cr), r5l = f2lo(ri5), r5h = f2hi(ri5);
+        T.axe[s] = fmaf(f2lo(qx), r5l, fmaf(crl, f2lo(dx), T.axe[s])); T.axo[s] = fmaf(f2hi(qx), r5h, fmaf(crh, f2hi(dx), T.axo[s]));
+        T.aye[s] = fmaf(f2lo(qy), r5l, fmaf(crl, f2lo(dy), T.aye[s])); T.ayo[s] = fmaf(f2hi(qy), r5h, fmaf(crh, f2hi(dy), T.ayo[s]));
+        T.aze[s] = fmaf(f2lo(qz), r5l, fmaf(crl, f2lo(dz), T.aze[s])); T.azo[s] = fmaf(f2hi(qz), r5h, fmaf(crh, f2hi(dz), T.azo[s]));
+    }
+}
+
+// cnt is a multiple of 4 (the tail of a list is padded with zero-mass cells FAR_AWAY)
+template <int NS> __device__ __forceinline__ void eval_pc(target<NS>& T, const float (*pc)[TILE], int cnt)
+{
+#pragma unroll 1
+    for (int e = 0; e < cnt; e += 4) {
+        ulonglong2 v[10];
+#pragma unroll
+        for (int k = 0; k < 10; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&pc[k][e]);
+        pc_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
+        pc_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
+    }
+}
+
+// Two sources per packed operation: the far zone (d2 >= r_out^2, W = 1, pure Newtonian) of the
+// p-p list, branch-free.  d2 follows R10 bit for bit (sub, mul, fma, fma; all rn).  A near pair is
+// masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
+// by the lane is returned so that the caller knows whether the tile needs the near pass.
+template <int NS>
+__device__ __forceinline__ float pp_far_pair(target<NS>& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
+{
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const f2 dx = sub2(px, pk(T.x[s], T.x[s])), dy = sub2(py, pk(T.y[s], T.y[s])), dz = sub2(pz, pk(T.z[s], T.z[s]));
+        const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        const float d2a = f2lo(d2), d2b = f2hi(d2);
+        dmin = fminf(dmin, fminf(d2a, d2b));
+        const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
+        const f2 mri = mul2(pm, ri);
+        const f2 f = mul2(mri, mul2(ri, ri));
+        T.ph[s] = add2(T.ph[s], mri);
+        const float fl = f2lo(f), fh = f2hi(f);
+        T.axe[s] = fmaf(fl, f2lo(dx), T.axe[s]); T.axo[s] = fmaf(fh, f2hi(dx), T.axo[s]);
+        T.aye[s] = fmaf(fl, f2lo(dy), T.aye[s]); T.ayo[s] = fmaf(fh, f2hi(dy), T.ayo[s]);
+        T.aze[s] = fmaf(fl, f2lo(dz), T.aze[s]); T.azo[s] = fmaf(fh, f2hi(dz), T.azo[s]);
+    }
+    return dmin;
+}
+
+// R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission and the
+// cutoff-weighted pair term.  Scalar pass over a tile, run only by warps whose tile came within
+// r_out of one of their targets (about one tile in eight).
+template <int NS>
+__device__ __forceinline__ void pp_near_pass(target<NS>& T, const float (*pp)[TILE], const int* ppj, int cnt, const force_args& A)
+{
+    const walk_consts& K = A.K;
+#pragma unroll 1
+    for (int e = 0; e < cnt; ++e) {
+        const float px = pp[0][e], py = pp[1][e], pz = pp[2][e];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float dx = __fsub_rn(px, T.x[s]), dy = __fsub_rn(py, T.y[s]), dz = __fsub_rn(pz, T.z[s]);
+            const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
+            if (d2 < K.rout2) {
+                const int j = ppj[e];
+                if (T.id[s] >= 0 && j != T.id[s]) {                  // self excluded by index; idle lanes
+                    A.nbraw[T.cur[s]++] = (int32_t)A.order[j];
+                    {
+                        const float m = pp[3][e];
+                        if (d2 > K.rin2) {
+                            const float ri = rsqrt_approx(d2), r = d2 * ri;
+                            const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
+                            const float W = cutoff_W(x);
+                            const float f = m * W * ri * ri * ri;
+                            T.nax[s] = fmaf(f, dx, T.nax[s]); T.nay[s] = fmaf(f, dy, T.nay[s]); T.naz[s] = fmaf(f, dz, T.naz[s]);
+                            T.nph[s] += K.pot_mode == 0 ? m * cutoff_psi(K, x, W, ri) : -m * ri;
+                        } else if (K.pot_mode == 0) {
+                            T.nph[s] = fmaf(m, K.psi_in, T.nph[s]);    // inside r_in: constant psi(r_in), also r = 0 (R8)
+                        } else if (d2 > 0.0f) {
+                            T.nph[s] -= m * rsqrt_approx(d2);
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+// cnt is a multiple of 4 (tail padded with zero-mass particles FAR_AWAY, index -1)
+template <int NS>
+__device__ __forceinline__ void eval_pp(target<NS>& T, const float (*pp)[TILE], const int* ppj, int cnt, const force_args& A)
+{
+    {
+        float dmin = INFINITY;
+#pragma unroll 1
+        for (int e = 0; e < cnt; e += 4) {
+            ulonglong2 v[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&pp[k][e]);
+            dmin = pp_far_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
+            dmin = pp_far_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
+        }
+        if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
+    }
+    pp_near_pass<NS>(T, pp, ppj, cnt, A);
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// one target group against its two lists
+// ---------------------------------------------------------------------------------------------
+struct pc_regs { float v[10]; };
+struct pp_regs { float x, y, z, m; int j; };
+
+__device__ __forceinline__ pc_regs load_pc(const force_args& A, const int32_t* ids, int e, int n)
+{
+    pc_regs r;
+    if (e < n) {
+        const int id = ids[e];
+        const float4 c = A.ncom[id], q0 = A.nq0[id]; const float2 q1 = A.nq1[id];
+        r.v[0] = c.x; r.v[1] = c.y; r.v[2] = c.z; r.v[3] = c.w;
+        r.v[4] = -q0.x; r.v[5] = -q0.y; r.v[6] = -q0.z; r.v[7] = -q0.w; r.v[8] = -q1.x; r.v[9] = -q1.y;
+    } else {                                   // padding: a zero-mass cell far away contributes exactly 0
+#pragma unroll
+        for (int k = 0; k < 10; ++k) r.v[k] = k < 3 ? FAR_AWAY : 0.0f;
+    }
+    return r;
+}
+__device__ __forceinline__ pp_regs load_pp(const force_args& A, const int32_t* ids, int e, int n)
+{
+    pp_regs r;
+    if (e < n) { r.j = ids[e]; const float4 p = A.spm[r.j]; r.x = p.x; r.y = p.y; r.z = p.z; r.m = p.w; }
+    else { r.x = r.y = r.z = FAR_AWAY; r.m = 0.0f; r.j = -1; }
+    return r;
+}
+
+template <int NS>
+__device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, int ge)
+{
+    const int lane = threadIdx.x & 31;
+    target<NS> T;
+    const float4 pfirst = A.spm[gb];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const int i = gb + s * 32 + lane;
+        const bool v = i < ge;
+        const float4 p = v ? A.spm[i] : pfirst;
+        T.x[s] = p.x; T.y[s] = p.y; T.z[s] = p.z;
+        T.ph[s] = pk(0.0f, 0.0f);
+        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
+        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
+        T.dax[s] = T.day[s] = T.daz[s] = T.dph[s] = 0.0;
+        T.id[s] = v ? i : -1;
+        T.cur[s] = v ? A.nboff[A.order[i]] : 0;
+    }
+    const uint4 rec = A.glist[g];
+    // ---- a8: particle-cell list ----
+    {
+        const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
+        const int n = (int)rec.y, nt = (n + TILE - 1) / TILE;
+        if (nt > 0) {
+            pc_regs r = load_pc(A, ids, lane, n);
+#pragma unroll
+            for (int k = 0; k < 10; ++k) S.pc[0][k][lane] = r.v[k];
+            __syncwarp();
+            for (int t = 0; t < nt; ++t) {
+                const bool more = t + 1 < nt;
+                if (more) r = load_pc(A, ids, (t + 1) * TILE + lane, n);      // in flight during the evaluation
+                eval_pc<NS>(T, S.pc[t & 1], TILE);
+                fold(T);
+                if (more) {
+#pragma unroll
+                    for (int k = 0; k < 10; ++k) S.pc[(t + 1) & 1][k][lane] = r.v[k];
+                }
+                __syncwarp();
+            }
+        }
+    }
+    // ---- a9: particle-particle list (cutoff, neighbour emission) ----
+    {
+        const int32_t* ids = A.pppool + ((long long)rec.z << 5);
+        const int n = (int)rec.w, nt = (n + TILE - 1) / TILE;
+        if (nt > 0) {
+            pp_regs r = load_pp(A, ids, lane, n);
+            S.pp[0][0][lane] = r.x; S.pp[0][1][lane] = r.y; S.pp[0][2][lane] = r.z; S.pp[0][3][lane] = r.m; S.ppj[0][lane] = r.j;
+            __syncwarp();
+            for (int t = 0; t < nt; ++t) {
+                const bool more = t + 1 < nt;
+                const int b = t & 1, nbuf = b ^ 1;
+                if (more) r = load_pp(A, ids, (t + 1) * TILE + lane, n);
+                eval_pp<NS>(T, S.pp[b], S.ppj[b], TILE, A);
+                if (b) fold(T);                                           // every 64 particles
+                if (more) { S.pp[nbuf][0][lane] = r.x; S.pp[nbuf][1][lane] = r.y; S.pp[nbuf][2][lane] = r.z; S.pp[nbuf][3][lane] = r.m; S.ppj[nbuf][lane] = r.j; }
+                __syncwarp();
+            }
+            fold(T);
+        }
+    }
+    // ---- a11: results to the caller's order ----
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        if (T.id[s] < 0) continue;
+        A.out[A.order[T.id[s]]] = make_float4((float)T.dax[s], (float)T.day[s], (float)T.daz[s], (float)T.dph[s]);
+    }
+}
+
+__global__ void __launch_bounds__(FORCE_THREADS, 4) k_force(force_args A)
+{
+    __shared__ tile_smem smem[FORCE_WARPS];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    tile_smem& S = smem[w];
+    const int ng = A.info->n_groups;
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = (int)atomicAdd(&A.info->group_cursor3, 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ng) break;
+        const int gb = A.gbegin[g], ge = A.gbegin[g + 1];
+        if (ge - gb > 32) force_group<2>(A, S, g, gb, ge);
+        else              force_group<1>(A, S, g, gb, ge);
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a10  neighbour CSR: exclusive scan of the per-particle counts (original order) -> int64 offsets
+// ---------------------------------------------------------------------------------------------
+#define SCAN_TILE 4096
+
+__global__ void __launch_bounds__(256) k_nb_blocksum(const int32_t* __restrict__ cnt, int n, long long* __restrict__ bsum,
+                                                     p3t_devinfo* info)
+{
+    __shared__ long long s_sum[8];
+    __shared__ int s_max[8];
+    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * 16;
+    long long t = 0; int mx = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { int i = base + k; int v = i < n ? cnt[i] : 0; t += v; mx = max(mx, v); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { t += __shfl_xor_sync(0xffffffffu, t, o); mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
+    if ((threadIdx.x & 31) == 0) { s_sum[threadIdx.x >> 5] = t; s_max[threadIdx.x >> 5] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < 8; ++k) { t += s_sum[k]; mx = max(mx, s_max[k]); }
+        bsum[blockIdx.x] = t;
+        atomicMax(&info->nb_max, mx);
+    }
+}
+
+__global__ void __launch_bounds__(1024) k_nb_scansums(long long* __restrict__ bsum, int nb, long long* __restrict__ off_n,
+                                                      p3t_devinfo* info)
+{
+    __shared__ long long s_w[32];
+    __shared__ long long s_run;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_run = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nb; b0 += 1024) {
+        const int b = b0 + threadIdx.x;
+        long long v = b < nb ? bsum[b] : 0, x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { long long y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) s_w[w] = x;
+        __syncthreads();
+        long long add = s_run, tot = 0;
+        for (int k = 0; k < 32; ++k) { long long t = s_w[k]; if (k < w) add += t; tot += t; }
+        if (b < nb) bsum[b] = add + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) s_run += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { *off_n = s_run; info->nb_total = (unsigned long long)s_run; }
+}
+
+__global__ void __launch_bounds__(256) k_nb_offsets(const int32_t* __restrict__ cnt, int n, const long long* __restrict__ bsum,
+                                                    long long* __restrict__ off)
+{
+    __shared__ long long s_w[8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * 16;
+    int v[16]; long long t = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { int i = base + k; v[k] = i < n ? cnt[i] : 0; t += v[k]; }
+    long long x = t;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { long long y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) s_w[w] = x;
+    __syncthreads();
+    long long run = bsum[blockIdx.x] + x - t;
+    for (int k = 0; k < w; ++k) run += s_w[k];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { int i = base + k; if (i < n) off[i] = run; run += v[k]; }
+}
+
+// rows ascending in original id: rank sort (ids inside a row are distinct), out of place.
+// Each lane sorts its own short row; rows longer than 16 are done by the whole warp.
+__global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
+                                                     int32_t* __restrict__ idx, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    long long b = 0; int len = 0;
+    if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
+    if (len <= 16) {
+        for (int a = 0; a < len; ++a) {
+            const int v = raw[b + a]; int r = 0;
+            for (int c = 0; c < len; ++c) r += raw[b + c] < v;
+            idx[b + r] = v;
+        }
+    }
+    uint32_t m = __ballot_sync(0xffffffffu, len > 16);
+    while (m) {
+        const int src = __ffs(m) - 1; m &= m - 1;
+        const long long rb = __shfl_sync(0xffffffffu, b, src);
+        const int rl = __shfl_sync(0xffffffffu, len, src);
+        for (int a = lane; a < rl; a += 32) {
+            const int v = raw[rb + a]; int r = 0;
+            for (int c = 0; c < rl; ++c) r += raw[rb + c] < v;
+            idx[rb + r] = v;
+        }
+    }
+}
+
+
+static void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode)
+{
+    // fp32 thresholds exactly as DESIGN.md R10 states them: one fp32 product each
+    volatile float ro2 = r_out * r_out, ri2 = r_in * r_in;
+    K.rout2 = ro2; K.rin2 = ri2; K.r_in = r_in;
+    const double D = (double)r_out - (double)r_in, c = (double)r_in / D, c1 = 1.0 + c;
+    K.inv_delta = (float)(1.0 / D);
+    K.k140 = (float)(140.0 / D);
+    // t^3 (1-t)^3 = (t + c) (b5 t^5 + ... + b0) - c^3 (1+c)^3   (synthetic division at t = -c)
+    const double b[6] = { c * c * c1 * c1 * c1, -c * c1 * c1 * c1, c1 * c1 * c1, -(3.0 + 3.0 * c + c * c), 3.0 + c, -1.0 };
+    double s1 = 0.0;
+    for (int k = 0; k < 6; ++k) { K.sc[k] = (float)(b[k] / (k + 1)); s1 += b[k] / (k + 1); }
+    K.s1 = (float)s1;
+    K.rem = (float)(c * c * c * c1 * c1 * c1);
+    K.c = (float)c;
+    // psi(r_in) = -(140/D) [ S(1) + rem ln((1+c)/c) ... ] with W(0) = 0; here the remainder enters with a minus sign
+    K.psi_in = (float)(-(140.0 / D) * (s1 - c * c * c * c1 * c1 * c1 * log(c1 / c)));
+    K.theta = theta;
+    K.pot_mode = pot_mode;
+}
+
+
+int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot)
+{
+    const int n = (int)ctx->n;
+    static int per_sm = 0;
+    if (!per_sm) {
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force, FORCE_THREADS, 0));
+        if (per_sm < 1) per_sm = 1;
+    }
+    int rc;
+    const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
+    if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->nboff, ((size_t)n + 1) * 8))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->nbcur, (size_t)nsb * 8 + 64))) return rc;
+
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
+    // a10, sizes: neighbour counts (range search only) -> CSR offsets, so that the lists can be written in place
+    if ((rc = p3t_launch_walk_count(ctx, r_out, theta))) return rc;
+    k_nb_blocksum<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), INFO(ctx));
+    k_nb_scansums<<<1, 1024, 0, ctx->stream>>>(P<long long>(ctx->nbcur), nsb, P<long long>(ctx->nboff) + n, INFO(ctx));
+    k_nb_offsets<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), P<long long>(ctx->nboff));
+    P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 3;
+    // a7: interaction lists
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
+    if ((rc = p3t_launch_walk_lists(ctx, r_out, theta))) return rc;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
+    // the one host synchronisation of this call: the neighbour total sizes the list buffers, and the
+    // walk reports whether its list pools were large enough (if not it is repeated, normally only on
+    // the first call of a context)
+    p3t_devinfo h;
+    for (int attempt = 0;; ++attempt) {
+        P3T_CUDA(ctx, cudaMemcpyAsync(&h, ctx->info.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (!h.pool_overflow) break;
+        if (attempt >= 4) { snprintf(ctx->err, sizeof(ctx->err), "interaction-list pools still too small after %d attempts", attempt); return P3T_ECUDA; }
+        ctx->pool_cap_pc = (((long long)h.need_pc + h.need_pc / 4 + 16384) + 31) & ~31ll;
+        ctx->pool_cap_pp = (((long long)h.need_pp + h.need_pp / 4 + 16384) + 31) & ~31ll;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
+        if ((rc = p3t_launch_walk_lists(ctx, r_out, theta))) return rc;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
+    }
+    const long long total = (long long)h.nb_total;
+    ctx->nb_total_host = total;
+    if ((rc = p3t_reserve(ctx, &ctx->nbidx, (size_t)total * 4 + 64))) return rc;
+    p3t_buf* raw = &ctx->stage_out;      // unsorted rows share the host-staging scratch
+    if ((rc = p3t_reserve(ctx, raw, (size_t)total * 4 + 64))) return rc;
+
+    force_args A;
+    A.spm = P<float4>(ctx->spm); A.order = P<uint32_t>(ctx->idx[0]);
+    A.ncom = P<float4>(ctx->ncom); A.nq0 = P<float4>(ctx->nq0); A.nq1 = P<float2>(ctx->nq1);
+    A.gbegin = P<int32_t>(ctx->gbegin); A.glist = P<uint4>(ctx->glist);
+    A.pcpool = P<int32_t>(ctx->pcpool); A.pppool = P<int32_t>(ctx->pppool);
+    A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
+    A.out = acc_pot; A.info = INFO(ctx);
+    make_consts(A.K, r_out, r_in, theta, pot_mode);
+    // a8, a9, a11: the force kernel
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
+    k_force<<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
+    k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    P3T_CUDA(ctx, cudaGetLastError());
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
+    ctx->launches += 2;
+    return P3T_OK;
+}

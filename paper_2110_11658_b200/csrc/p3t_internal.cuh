@@ -26,10 +26,13 @@ struct p3t_devinfo {
     int32_t  level_begin[24]; // first node of each level; level_begin[max_level+1] = n_nodes
     uint32_t group_cursor;   // dynamic group scheduler of the walk kernels
     uint32_t group_cursor2;
+    uint32_t group_cursor3;
     unsigned long long n_pp, n_pc, n_pp_list, n_pc_list;
     unsigned long long nb_total;
     int32_t  nb_max;
     int32_t  stack_overflow;
+    int32_t  pool_overflow;  // a walker warp ran out of list space (the call is repeated with larger pools)
+    uint32_t need_pc, need_pp; // largest per-warp list space used, in entries
     uint32_t minmax[6];      // order-preserving uint encodings of min xyz / max xyz
 };
 
@@ -59,6 +62,10 @@ struct p3t_ctx {
     p3t_buf nbcount, nboff, nbidx;   // neighbour CSR: counts (sorted order) -> offsets (original order), indices
     p3t_buf nbcur;                   // int64 per sorted particle: write cursor base
     p3t_buf spill;                   // walk stack spill
+    p3t_buf pcpool, pppool;          // interaction lists: node ids / sorted particle positions, per-warp regions
+    p3t_buf glist;                   // uint4 per group: pc offset/32, n_pc, pp offset/32, n_pp
+    int64_t pool_cap_pc, pool_cap_pp;// entries per walker warp (multiples of 32)
+    int64_t walk_warps_max, walk_list_warps;
     p3t_buf info;                    // p3t_devinfo
     p3t_buf stage_in, stage_out;     // p3t_step_host staging
     int64_t nb_total_host;           // valid after p3t_neighbours
@@ -90,5 +97,9 @@ int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
 // p3t_tree.cu : a4-a6
 int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
-// p3t_walk.cu : a7-a11
+// p3t_walk.cu : a7 (interaction lists), a10 (neighbour counts)
+int p3t_walk_init(p3t_ctx* ctx);
+int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta);
+int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta);
+// p3t_force.cu : a8-a11
 int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot);

@@ -1,314 +1,54 @@
-// p3t_walk.cu -- steps a7-a11: group tree walk, particle-cell and
-// particle-particle regular force with the cutoff of eq. 6 and neighbour-list
-// emission fused in, scatter of the results to the caller's particle order.
+// p3t_walk.cu -- steps a7 and a10: the group tree walk.
 //
-//   F_R,i = sum_j m_j W(x_ij) (x_j - x_i) / r_ij^3,  W = 1 - K,  x = (r - r_in)/(r_out - r_in)
-//   (eq. 1, 3, 4, 6, 8-10; attractive sign: DESIGN.md R1)
+// One warp walks one target group (R-S5) breadth-first: 32 cells per iteration, one per lane, the
+// opening rule R-S7 evaluated in bit-specified fp32, ballot / popc compaction, a shared-memory
+// stack with a global spill.  Two kernels share the traversal:
 //
-// One warp walks one target group (<= 64 particles, two target slots per lane).  Rules:
-// DESIGN.md R-S7 (opening rule, bit-specified fp32), R-S8 (evaluation), R-S9 (accumulation),
-// R10 (neighbour predicate, bit-specified fp32).
+//   k_walk<WALK_COUNT>  walks only the cells within r_out of the group box and counts, per target,
+//                       the neighbours d2 < r_out^2 (R10): the sizes of the CSR rows (a10).
+//   k_walk<WALK_LISTS>  the full walk (a7).  It evaluates nothing: accepted cells (node ids) and the
+//                       particles of opened leaves (sorted positions) are appended to the group's
+//                       interaction lists in HBM.  The force kernel (p3t_force.cu) streams them.
+//
+// Why the lists go through HBM on B200: the walk is a serial, latency-bound pointer chase that
+// needs few registers and many resident warps; the force evaluation is an FP32-pipe-bound stream
+// that needs many registers.  Fused in one kernel (this library's first version) the two phases of
+// a warp alternate and the FP32 pipe idles for 30-40 % of the time (profiles/r01_*).  Writing
+// 4 bytes per interaction-list entry costs 0.57 GB of HBM traffic at N = 2^20 (< 0.2 ms at the
+// measured 6.5 TB/s) and lets either kernel run at its own occupancy.
+// The paper gives no detail of this stage ("the BONSAI library").
 #include "p3t_internal.cuh"
 #include <stdlib.h>
 
-#define WALK_WARPS   4                    // warps per CTA, each walks its own groups
+#define WALK_WARPS   8
 #define WALK_THREADS (WALK_WARPS * 32)
-#define STACK_CAP    512                  // per-warp node stack in shared memory; deeper entries spill
+#define STACK_CAP    384                  // per-warp node stack in shared memory; deeper entries spill
 #define SPILL_CAP    8192                 // per-warp spill (global memory), entries
-#define PC_TILE      32                   // cells: a flush is due at this fill level
-#define PP_TILE      64                   // particles: likewise
-#define PC_CAP       (PC_TILE + 32)       // one walk iteration appends at most 32 cells
-#define PP_CAP       (PP_TILE + 32)       // leaf particles are appended in chunks of at most 32
-#define FAR_AWAY     1.0e18f              // position of the zero-mass padding entries of a tile
-
-struct walk_consts {
-    float rout2, rin2, r_in, inv_delta;   // inv_delta = 1 / (r_out - r_in)
-    float psi_in;                          // psi(r_in), the constant regular pair potential inside r_in
-    float k140;                            // 140 / (r_out - r_in)
-    float s1;                              // S(1)
-    float sc[6];                           // S(t) = t (sc0 + t (sc1 + ... t sc5))
-    float rem;                             // c^3 (1+c)^3  (> 0)
-    float c;                               // r_in / (r_out - r_in)
-    float theta;
-    int   pot_mode;
-};
+#define WALK_COUNT   0
+#define WALK_LISTS   1
 
 struct walk_args {
     const float4* spm; const uint32_t* order;
-    const float4 *ncom, *nlo, *nhi, *nq0; const float2* nq1; const int2* nlink;
+    const float4 *ncom, *nlo, *nhi; const int2* nlink;
     const int32_t* gbegin;
     int32_t *gnpp, *gnpc;
-    int32_t* nbcount;           // MODE 0 out: per ORIGINAL id
-    const int64_t* nboff;       // MODE 1 in:  per ORIGINAL id
-    int32_t* nbraw;             // MODE 1 out: unsorted rows
-    float4* out;                // MODE 1 out: acc_pot, original order
+    int32_t* nbcount;           // WALK_COUNT out: per ORIGINAL id
+    int32_t *pcpool, *pppool;   // WALK_LISTS out
+    uint4* glist;               // WALK_LISTS out
+    long long cap_pc, cap_pp;   // list space per warp, entries (multiples of 32)
     int32_t* spill;
     p3t_devinfo* info;
-    walk_consts K;
-    int dbg;
+    float rout2, theta;
 };
 
-// Per-warp list tiles, structure-of-arrays so that two (LDS.64) or four (LDS.128) consecutive
-// entries arrive as the packed operands of the f32x2 instructions below.
-// pc rows: 0-2 COM, 3 M, 4-9 MINUS the traceless quadrupole (xx yy zz xy xz yz).
 struct __align__(16) warp_smem {
     int   stack[STACK_CAP];
-    float pc[10][PC_CAP];
-    float pp[4][PP_CAP];        // x y z m
-    int   ppj[PP_CAP];          // sorted position of the source
+    int   pcid[64];             // WALK_LISTS: accepted node ids waiting for a 32-wide store
+    int   ppid[64];             // WALK_LISTS: sorted positions of leaf particles, likewise
 };
-
-__device__ __forceinline__ float rsqrt_approx(float x)
-{
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-// ---- packed fp32 pairs: Blackwell's FADD2 / FMUL2 / FFMA2 (PTX add/mul/fma.rn.f32x2) retire two
-// IEEE-rn fp32 operations per lane and issue slot; measured on B200 they reach the same
-// 128 lanes/clk/SM as FFMA with half the issue slots, which is what an issue-bound loop needs.
-typedef unsigned long long f2;
-__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float f2lo(f2 v) { float a; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(a) : "l"(v)); return a; }
-__device__ __forceinline__ float f2hi(f2 v) { float b; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(b) : "l"(v)); return b; }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-
-// eq. 6, 0 < x < 1: W = x^4 (35 - 84 x + 70 x^2 - 20 x^3); evaluated through the
-// symmetry W(x) = 1 - W(1 - x) above x = 1/2 so that fp32 Horner never cancels.
-__device__ __forceinline__ float cutoff_W(float x)
-{
-    float t = x > 0.5f ? 1.0f - x : x;
-    float t2 = t * t;
-    float w = t2 * t2 * (35.0f + t * (-84.0f + t * (70.0f - 20.0f * t)));
-    return x > 0.5f ? 1.0f - w : w;
-}
-
-// regular pair potential for r_in < r < r_out (R6): -W/r - (140/D) int_x^1 t^3(1-t)^3/(t+c) dt
-__device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float W, float rinv)
-{
-    float sx = x * (K.sc[0] + x * (K.sc[1] + x * (K.sc[2] + x * (K.sc[3] + x * (K.sc[4] + x * K.sc[5])))));
-    float integral = (K.s1 - sx) - K.rem * __logf((1.0f + K.c) / (x + K.c));
-    return -W * rinv - K.k140 * integral;
-}
-
-// NS target slots per lane.  Every accumulator is a packed pair: .lo sums the even list entries,
-// .hi the odd ones.  ph accumulates MINUS the potential of the far terms; the rare near-zone terms
-// (cutoff branch) go to the scalar n* accumulators with their true sign.
-template <int NS> struct target {
-    float x[NS], y[NS], z[NS];
-    f2    ph[NS];                                // fp32 partial sums of the current tile: -potential (packed)
-    float axe[NS], aye[NS], aze[NS];             // acceleration from the even list entries ...
-    float axo[NS], ayo[NS], azo[NS];             // ... and from the odd ones (scalar FFMAs, see pc_pair)
-    float nax[NS], nay[NS], naz[NS], nph[NS];
-    double dax[NS], day[NS], daz[NS], dph[NS];   // fp64 masters (R-S9)
-    int   id[NS];                                // sorted position of the target, -1 = no target
-    long long cur[NS];                           // neighbour write cursor (MODE 1) / count (MODE 0)
+struct __align__(16) count_smem {   // WALK_COUNT: positions of the leaf particles of one round
+    float x[32], y[32], z[32]; int j[32];
 };
-
-template <int NS> __device__ __forceinline__ void fold(target<NS>& T)
-{
-    const f2 zero = pk(0.0f, 0.0f);
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        T.dax[s] += (double)((T.axe[s] + T.axo[s]) + T.nax[s]);
-        T.day[s] += (double)((T.aye[s] + T.ayo[s]) + T.nay[s]);
-        T.daz[s] += (double)((T.aze[s] + T.azo[s]) + T.naz[s]);
-        T.dph[s] += (double)(T.nph[s] - (f2lo(T.ph[s]) + f2hi(T.ph[s])));
-        T.ph[s] = zero;
-        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
-        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
-    }
-}
-
-// R-S8 particle-cell, monopole + traceless quadrupole, two cells per packed operation.
-// With d = COM - x_i (= -r), Q' = -Q (stored negated in the tile), R = |d|:
-//   q' = d.Q'.d / R^5,  -phi = M/R - q'/2,  a = (M/R - (5/2) q') d / R^2 + (Q'.d) / R^5
-// which is a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7 of R-S8: 33 packed operations per pair.
-template <int NS> __device__ __forceinline__ void pc_pair(target<NS>& T, f2 cx, f2 cy, f2 cz, f2 cm,
-                                                          f2 qxx, f2 qyy, f2 qzz, f2 qxy, f2 qxz, f2 qyz)
-{
-    const f2 mhalf = pk(-0.5f, -0.5f), m52 = pk(-2.5f, -2.5f);
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const f2 dx = sub2(cx, pk(T.x[s], T.x[s])), dy = sub2(cy, pk(T.y[s], T.y[s])), dz = sub2(cz, pk(T.z[s], T.z[s]));
-        const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
-        const f2 ri2 = mul2(ri, ri);
-        const f2 qx = fma2(qxz, dz, fma2(qxy, dy, mul2(qxx, dx)));
-        const f2 qy = fma2(qyz, dz, fma2(qyy, dy, mul2(qxy, dx)));
-        const f2 qz = fma2(qzz, dz, fma2(qyz, dy, mul2(qxz, dx)));
-        const f2 dqd = fma2(dz, qz, fma2(dy, qy, mul2(dx, qx)));
-        const f2 ri3 = mul2(ri2, ri), ri5 = mul2(ri3, ri2);
-        const f2 mono = mul2(cm, ri);
-        const f2 q5 = mul2(dqd, ri5);
-        T.ph[s] = fma2(mhalf, q5, add2(T.ph[s], mono));
-        const f2 cr = mul2(fma2(m52, q5, mono), ri2);
-        // An FFMA2 with three distinct register-pair operands occupies the pipe for 3 cycles (measured:
-        // operand bandwidth), two scalar FFMAs for 2: the accumulations are issued on the halves.
-        const float crl = f2lo(cr), crh = f2hi(cr), r5l = f2lo(ri5), r5h = f2hi(ri5);
-        T.axe[s] = fmaf(f2lo(qx), r5l, fmaf(crl, f2lo(dx), T.axe[s])); T.axo[s] = fmaf(f2hi(qx), r5h, fmaf(crh, f2hi(dx), T.axo[s]));
-        T.aye[s] = fmaf(f2lo(qy), r5l, fmaf(crl, f2lo(dy), T.aye[s])); T.ayo[s] = fmaf(f2hi(qy), r5h, fmaf(crh, f2hi(dy), T.ayo[s]));
-        T.aze[s] = fmaf(f2lo(qz), r5l, fmaf(crl, f2lo(dz), T.aze[s])); T.azo[s] = fmaf(f2hi(qz), r5h, fmaf(crh, f2hi(dz), T.azo[s]));
-    }
-}
-
-// cnt is a multiple of 4 (the tail of a list is padded with zero-mass cells FAR_AWAY)
-template <int NS> __device__ __forceinline__ void eval_pc(target<NS>& T, const warp_smem& S, int cnt)
-{
-#pragma unroll 1
-    for (int e = 0; e < cnt; e += 4) {
-        ulonglong2 v[10];
-#pragma unroll
-        for (int k = 0; k < 10; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&S.pc[k][e]);
-        pc_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
-        pc_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
-    }
-}
-
-// Two sources per packed operation: the far zone (d2 >= r_out^2, W = 1, pure Newtonian) of the
-// p-p list, branch-free.  d2 follows R10 bit for bit (sub, mul, fma, fma; all rn).  A near pair is
-// masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
-// by the lane is returned so that the caller knows whether the tile needs the near pass.
-template <int NS>
-__device__ __forceinline__ float pp_far_pair(target<NS>& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
-{
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const f2 dx = sub2(px, pk(T.x[s], T.x[s])), dy = sub2(py, pk(T.y[s], T.y[s])), dz = sub2(pz, pk(T.z[s], T.z[s]));
-        const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        const float d2a = f2lo(d2), d2b = f2hi(d2);
-        dmin = fminf(dmin, fminf(d2a, d2b));
-        const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
-        const f2 mri = mul2(pm, ri);
-        const f2 f = mul2(mri, mul2(ri, ri));
-        T.ph[s] = add2(T.ph[s], mri);
-        const float fl = f2lo(f), fh = f2hi(f);
-        T.axe[s] = fmaf(fl, f2lo(dx), T.axe[s]); T.axo[s] = fmaf(fh, f2hi(dx), T.axo[s]);
-        T.aye[s] = fmaf(fl, f2lo(dy), T.aye[s]); T.ayo[s] = fmaf(fh, f2hi(dy), T.ayo[s]);
-        T.aze[s] = fmaf(fl, f2lo(dz), T.aze[s]); T.azo[s] = fmaf(fh, f2hi(dz), T.azo[s]);
-    }
-    return dmin;
-}
-
-// R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission (MODE 1) or count (MODE 0) and the
-// cutoff-weighted pair term.  Scalar pass over a tile, run only by warps whose tile came within
-// r_out of one of their targets (about one tile in eight).
-template <int NS, int MODE>
-__device__ __forceinline__ void pp_near_pass(target<NS>& T, const warp_smem& S, int cnt, const walk_args& A)
-{
-    const walk_consts& K = A.K;
-#pragma unroll 1
-    for (int e = 0; e < cnt; ++e) {
-        const float px = S.pp[0][e], py = S.pp[1][e], pz = S.pp[2][e];
-#pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            const float dx = __fsub_rn(px, T.x[s]), dy = __fsub_rn(py, T.y[s]), dz = __fsub_rn(pz, T.z[s]);
-            const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
-            if (d2 < K.rout2) {
-                const int j = S.ppj[e];
-                if (T.id[s] >= 0 && j != T.id[s]) {                  // self excluded by index; idle lanes
-                    if (MODE == 1) A.nbraw[T.cur[s]] = (int32_t)A.order[j];
-                    T.cur[s]++;
-                    if (MODE == 1) {
-                        const float m = S.pp[3][e];
-                        if (d2 > K.rin2) {
-                            const float ri = rsqrt_approx(d2), r = d2 * ri;
-                            const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
-                            const float W = cutoff_W(x);
-                            const float f = m * W * ri * ri * ri;
-                            T.nax[s] = fmaf(f, dx, T.nax[s]); T.nay[s] = fmaf(f, dy, T.nay[s]); T.naz[s] = fmaf(f, dz, T.naz[s]);
-                            T.nph[s] += K.pot_mode == 0 ? m * cutoff_psi(K, x, W, ri) : -m * ri;
-                        } else if (K.pot_mode == 0) {
-                            T.nph[s] = fmaf(m, K.psi_in, T.nph[s]);    // inside r_in: constant psi(r_in), also r = 0 (R8)
-                        } else if (d2 > 0.0f) {
-                            T.nph[s] -= m * rsqrt_approx(d2);
-                        }
-                    }
-                }
-            }
-        }
-    }
-}
-
-// cnt is a multiple of 4 (tail padded with zero-mass particles FAR_AWAY, index -1)
-template <int NS, int MODE>
-__device__ __forceinline__ void eval_pp(target<NS>& T, const warp_smem& S, int cnt, const walk_args& A)
-{
-    if (MODE == 1) {
-        float dmin = INFINITY;
-#pragma unroll 1
-        for (int e = 0; e < cnt; e += 4) {
-            ulonglong2 v[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&S.pp[k][e]);
-            dmin = pp_far_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
-            dmin = pp_far_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
-        }
-        if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
-    }
-    pp_near_pass<NS, MODE>(T, S, cnt, A);     // the count pass (MODE 0) walks only cells within r_out
-}
-
-// pad the p-c tile from `fill` up to the next multiple of 4 with zero-mass cells; returns that multiple
-__device__ __forceinline__ int pad_pc(warp_smem& S, int fill, int lane)
-{
-    const int n4 = (fill + 3) & ~3;
-    if (lane < n4 - fill) {
-#pragma unroll
-        for (int k = 0; k < 10; ++k) S.pc[k][fill + lane] = k < 3 ? FAR_AWAY : 0.0f;
-    }
-    __syncwarp();
-    return n4;
-}
-__device__ __forceinline__ int pad_pp(warp_smem& S, int fill, int lane)
-{
-    const int n4 = (fill + 3) & ~3;
-    if (lane < n4 - fill) {
-        S.pp[0][fill + lane] = S.pp[1][fill + lane] = S.pp[2][fill + lane] = FAR_AWAY;
-        S.pp[3][fill + lane] = 0.0f; S.ppj[fill + lane] = -1;
-    }
-    __syncwarp();
-    return n4;
-}
-// after the first n4 entries (multiple of 4) were evaluated, move the 0..3 left over to the front
-__device__ __forceinline__ int shift_pc(warp_smem& S, int fill, int n4, int lane)
-{
-    const int rest = fill - n4;
-    float t[10];
-    if (lane < rest) {
-#pragma unroll
-        for (int k = 0; k < 10; ++k) t[k] = S.pc[k][n4 + lane];
-    }
-    __syncwarp();
-    if (lane < rest) {
-#pragma unroll
-        for (int k = 0; k < 10; ++k) S.pc[k][lane] = t[k];
-    }
-    __syncwarp();
-    return rest;
-}
-__device__ __forceinline__ int shift_pp(warp_smem& S, int fill, int n4, int lane)
-{
-    const int rest = fill - n4;
-    float t[4]; int j = 0;
-    if (lane < rest) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) t[k] = S.pp[k][n4 + lane];
-        j = S.ppj[n4 + lane];
-    }
-    __syncwarp();
-    if (lane < rest) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) S.pp[k][lane] = t[k];
-        S.ppj[lane] = j;
-    }
-    __syncwarp();
-    return rest;
-}
 
 __device__ __forceinline__ int stack_get(const warp_smem& S, const int32_t* spill, int i)
 {
@@ -319,29 +59,38 @@ __device__ __forceinline__ void stack_put(warp_smem& S, int32_t* spill, int i, i
     if (i < STACK_CAP) S.stack[i] = v; else spill[i - STACK_CAP] = v;
 }
 
-template <int NS, int MODE>
-__device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int g, int gb, int ge,
-                           const float* s_lt /* [24] fl(l/theta) per level */)
+// ids wait in a 64-entry staging row; once 32 are there they leave as one coalesced 128-byte store.
+// ptr counts entries even when the region is full, so that the host learns the space needed.
+__device__ __forceinline__ void list_flush(int* stage, int& fill, int32_t* pool, long long& ptr, long long end, int lane, int& ovf)
+{
+    if (fill >= 32) {
+        if (ptr + 32 <= end) pool[ptr + lane] = stage[lane]; else ovf = 1;
+        ptr += 32;
+        const int v = stage[32 + lane];
+        __syncwarp();
+        stage[lane] = v;
+        fill -= 32;
+        __syncwarp();
+    }
+}
+
+template <int MODE>
+__device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int32_t* spill, int g, int gb, int ge,
+                           const float* s_lt /* [24] fl(l/theta) per level */,
+                           long long& pc_ptr, long long pc_end, long long& pp_ptr, long long pp_end)
 {
     const int lane = threadIdx.x & 31;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const walk_consts& K = A.K;
-    target<NS> T;
+    // targets: two slots per lane (P3T_MAX_NCRIT = 64); the group box is the exact fp32 min/max
+    float tx[2], ty[2], tz[2]; int tid[2], cnt[2] = { 0, 0 };
     float glo[3] = { INFINITY, INFINITY, INFINITY }, ghi[3] = { -INFINITY, -INFINITY, -INFINITY };
     const float4 pfirst = A.spm[gb];
 #pragma unroll
-    for (int s = 0; s < NS; ++s) {
+    for (int s = 0; s < 2; ++s) {
         const int i = gb + s * 32 + lane;
         const bool v = i < ge;
         const float4 p = v ? A.spm[i] : pfirst;
-        T.x[s] = p.x; T.y[s] = p.y; T.z[s] = p.z;
-        T.ph[s] = pk(0.0f, 0.0f);
-        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
-        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
-        T.dax[s] = T.day[s] = T.daz[s] = T.dph[s] = 0.0;
-        T.id[s] = v ? i : -1;
-        T.cur[s] = 0;
-        if (MODE == 1 && v) T.cur[s] = A.nboff[A.order[i]];
+        tx[s] = p.x; ty[s] = p.y; tz[s] = p.z; tid[s] = v ? i : -1;
         glo[0] = fminf(glo[0], p.x); glo[1] = fminf(glo[1], p.y); glo[2] = fminf(glo[2], p.z);
         ghi[0] = fmaxf(ghi[0], p.x); ghi[1] = fmaxf(ghi[1], p.y); ghi[2] = fmaxf(ghi[2], p.z);
     }
@@ -353,346 +102,234 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, int32_t* spill, int
             ghi[a] = fmaxf(ghi[a], __shfl_xor_sync(0xffffffffu, ghi[a], o));
         }
 
-    int top = 1, npc = 0, npp = 0, fill_pc = 0, fill_pp = 0, overflow = 0;
+    // every group's lists start on a 32-entry (128-byte) boundary
+    const long long pc_begin = pc_ptr, pp_begin = pp_ptr;
+    int top = 1, npc = 0, npp = 0, fill_pc = 0, fill_pp = 0, overflow = 0, ovf = 0;
     if (lane == 0) S.stack[0] = 0;
     __syncwarp();
-    // One more pass after the stack has emptied flushes the list tails, so that each evaluation
-    // loop exists once in the code (instruction-cache footprint).
-    for (bool more = true; more;) {
-        more = top > 0;
+    while (top > 0) {
+        const int take = min(top, 32);
+        top -= take;
+        const bool valid = lane < take;
+        int node = 0;
+        if (valid) node = stack_get(S, spill, top + lane);
+        bool open = false;
         int2 link = make_int2(0, 0);
-        int lc_incl = 0, lc_excl = 0, src_total = 0;
-        if (more) {
-            const int take = min(top, 32);
-            top -= take;
-            const bool valid = lane < take;
-            int node = 0;
-            if (valid) node = stack_get(S, spill, top + lane);
-            bool open = false;
-            float4 com = make_float4(0, 0, 0, 0), q0 = com;
-            float2 q1 = make_float2(0, 0);
-            if (valid) {
-                com = A.ncom[node];
-                const float4 lo = A.nlo[node], hi = A.nhi[node];
-                link = A.nlink[node];
-                if (MODE == 1) { q0 = A.nq0[node]; q1 = A.nq1[node]; }   // with the node, not after the test: one L2 round trip
-                // R-S7, every operation one fp32 rounding
+        if (valid) {
+            const float4 com = A.ncom[node];
+            const float4 lo = A.nlo[node], hi = A.nhi[node];
+            link = A.nlink[node];
+            // R-S7, every operation one fp32 rounding
+            const float fx = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], hi.x)), __fsub_rn(lo.x, ghi[0]));
+            const float fy = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], hi.y)), __fsub_rn(lo.y, ghi[1]));
+            const float fz = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], hi.z)), __fsub_rn(lo.z, ghi[2]));
+            const float b2 = fmaf(fz, fz, fmaf(fy, fy, __fmul_rn(fx, fx)));
+            open = b2 < A.rout2;
+            if (MODE == WALK_LISTS) {
                 const float ex = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], com.x)), __fsub_rn(com.x, ghi[0]));
                 const float ey = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], com.y)), __fsub_rn(com.y, ghi[1]));
                 const float ez = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], com.z)), __fsub_rn(com.z, ghi[2]));
-                const float fx = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], hi.x)), __fsub_rn(lo.x, ghi[0]));
-                const float fy = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], hi.y)), __fsub_rn(lo.y, ghi[1]));
-                const float fz = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], hi.z)), __fsub_rn(lo.z, ghi[2]));
                 const float d2 = fmaf(ez, ez, fmaf(ey, ey, __fmul_rn(ex, ex)));
-                const float b2 = fmaf(fz, fz, fmaf(fy, fy, __fmul_rn(fx, fx)));
                 const float u = __fadd_rn(s_lt[__float_as_int(hi.w)], lo.w);
-                const float rc2 = __fmul_rn(u, u);
-                const bool near = b2 < K.rout2;
-                open = MODE == 1 ? ((d2 < rc2) || near) : near;
+                open = open || d2 < __fmul_rn(u, u);
             }
-            const bool inner = valid && open && link.y > 0;
-            const bool leaf  = valid && open && link.y < 0;
-            const bool acc   = MODE == 1 && valid && !open;
-            // children of opened internal cells go on the stack
-            {
-                int c = inner ? link.y : 0, x = c;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-                const int total = __shfl_sync(0xffffffffu, x, 31);
-                if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
-                int w = top + x - c;
-                for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
-                top += total;
-            }
-            // accepted cells go on the particle-cell tile
-            if (MODE == 1) {
-                const uint32_t m = __ballot_sync(0xffffffffu, acc);
-                if (acc) {
-                    const int w = fill_pc + __popc(m & lt_mask);
-                    S.pc[0][w] = com.x; S.pc[1][w] = com.y; S.pc[2][w] = com.z; S.pc[3][w] = com.w;
-                    S.pc[4][w] = -q0.x; S.pc[5][w] = -q0.y; S.pc[6][w] = -q0.z; S.pc[7][w] = -q0.w;
-                    S.pc[8][w] = -q1.x; S.pc[9][w] = -q1.y;
-                }
-                fill_pc += __popc(m);
-                npc += __popc(m);
-            }
-            // opened leaves: inclusive scan of their particle counts, so that the copy below can
-            // take 32 particles per round whatever the leaf sizes are
-            lc_incl = leaf ? -link.y : 0;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, lc_incl, o); if (lane >= o) lc_incl += y; }
-            src_total = __shfl_sync(0xffffffffu, lc_incl, 31);
-            lc_excl = lc_incl - (leaf ? -link.y : 0);
-            npp += src_total;
         }
-        __syncwarp();
-        // particle k of this iteration's opened leaves belongs to the first lane whose inclusive
-        // count exceeds k (binary search by shuffle); 32 particles per round go on the p-p tile
-        for (int k0 = 0;; k0 += 32) {
-            const int m = min(32, src_total - k0);
-            if (m > 0) {
-                const int k = k0 + lane;
-                int pos = 0;
+        const bool inner = valid && open && link.y > 0;
+        const bool leaf  = valid && open && link.y < 0;
+        const bool acc   = MODE == WALK_LISTS && valid && !open;
+        // children of opened internal cells go on the stack
+        {
+            int c = inner ? link.y : 0, x = c;
 #pragma unroll
-                for (int st = 16; st > 0; st >>= 1) {
-                    const int v = __shfl_sync(0xffffffffu, lc_incl, pos + st - 1);
-                    if (v <= k) pos += st;
-                }
-                pos = min(pos, 31);
-                const int j = __shfl_sync(0xffffffffu, link.x, pos) + (k - __shfl_sync(0xffffffffu, lc_excl, pos));
-                if (lane < m) {
-                    const float4 p = A.spm[j];
-                    const int w = fill_pp + lane;
-                    S.pp[0][w] = p.x; S.pp[1][w] = p.y; S.pp[2][w] = p.z; S.pp[3][w] = p.w; S.ppj[w] = j;
-                }
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            const int total = __shfl_sync(0xffffffffu, x, 31);
+            if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
+            int w = top + x - c;
+            for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
+            top += total;
+        }
+        // accepted cells: their ids go on the particle-cell list
+        if (MODE == WALK_LISTS) {
+            const uint32_t m = __ballot_sync(0xffffffffu, acc);
+            if (acc) S.pcid[fill_pc + __popc(m & lt_mask)] = node;
+            fill_pc += __popc(m);
+            npc += __popc(m);
+            __syncwarp();
+            list_flush(S.pcid, fill_pc, A.pcpool, pc_ptr, pc_end, lane, ovf);
+        }
+        // opened leaves: inclusive scan of their particle counts; particle k of this iteration's leaves
+        // belongs to the first lane whose inclusive count exceeds k (binary search by shuffle)
+        int lc_incl = leaf ? -link.y : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, lc_incl, o); if (lane >= o) lc_incl += y; }
+        const int src_total = __shfl_sync(0xffffffffu, lc_incl, 31);
+        const int lc_excl = lc_incl - (leaf ? -link.y : 0);
+        npp += src_total;
+        for (int k0 = 0; k0 < src_total; k0 += 32) {
+            const int m = min(32, src_total - k0);
+            const int k = k0 + lane;
+            int pos = 0;
+#pragma unroll
+            for (int st = 16; st > 0; st >>= 1) {
+                const int v = __shfl_sync(0xffffffffu, lc_incl, pos + st - 1);
+                if (v <= k) pos += st;
+            }
+            pos = min(pos, 31);
+            const int j = __shfl_sync(0xffffffffu, link.x, pos) + (k - __shfl_sync(0xffffffffu, lc_excl, pos));
+            if (MODE == WALK_LISTS) {
+                if (lane < m) S.ppid[fill_pp + lane] = j;
                 fill_pp += m;
                 __syncwarp();
-            }
-            const bool drained = k0 + 32 >= src_total;
-            const bool last = !more && drained;
-            if (fill_pp >= PP_TILE || (last && fill_pp > 0)) {
-                const int n4 = last ? pad_pp(S, fill_pp, lane) : (fill_pp & ~3);
-                if (!(A.dbg & 2)) eval_pp<NS, MODE>(T, S, n4, A);
-                if (MODE == 1) fold(T);
+                list_flush(S.ppid, fill_pp, A.pppool, pp_ptr, pp_end, lane, ovf);
+            } else {
+                // R10 neighbour predicate, bit-specified fp32, for the 32 particles of this round
+                if (lane < m) { const float4 p = A.spm[j]; C->x[lane] = p.x; C->y[lane] = p.y; C->z[lane] = p.z; C->j[lane] = j; }
                 __syncwarp();
-                fill_pp = last ? 0 : shift_pp(S, fill_pp, n4, lane);
+                for (int e = 0; e < m; ++e) {
+                    const float px = C->x[e], py = C->y[e], pz = C->z[e]; const int pj = C->j[e];
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        const float dx = __fsub_rn(px, tx[s]), dy = __fsub_rn(py, ty[s]), dz = __fsub_rn(pz, tz[s]);
+                        const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
+                        cnt[s] += (d2 < A.rout2 && pj != tid[s]) ? 1 : 0;          // self excluded by index
+                    }
+                }
+                __syncwarp();
             }
-            if (drained) break;
-        }
-        if (MODE == 1 && (fill_pc >= PC_TILE || (!more && fill_pc > 0))) {
-            const int n4 = more ? (fill_pc & ~3) : pad_pc(S, fill_pc, lane);
-            for (int rep = (A.dbg & 1) ? 0 : ((A.dbg & 8) ? 2 : 1); rep > 0; --rep) eval_pc<NS>(T, S, n4);
-            fold(T);
-            __syncwarp();
-            fill_pc = more ? shift_pc(S, fill_pc, n4, lane) : 0;
         }
         __syncwarp();
     }
 
-    // a11: results to the caller's order
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        if (T.id[s] < 0) continue;
-        const uint32_t orig = A.order[T.id[s]];
-        if (MODE == 1) A.out[orig] = make_float4((float)T.dax[s], (float)T.day[s], (float)T.daz[s], (float)T.dph[s]);
-        else A.nbcount[orig] = (int32_t)T.cur[s];
-    }
-    if (lane == 0) {
-        if (MODE == 1) {
+    if (MODE == WALK_LISTS) {
+        // tails, padded to the 32-entry boundary (the force kernel masks by n_pc / n_pp)
+        if (fill_pc > 0) { fill_pc = 32; list_flush(S.pcid, fill_pc, A.pcpool, pc_ptr, pc_end, lane, ovf); }
+        if (fill_pp > 0) { fill_pp = 32; list_flush(S.ppid, fill_pp, A.pppool, pp_ptr, pp_end, lane, ovf); }
+        if (lane == 0) {
+            A.glist[g] = make_uint4((uint32_t)(pc_begin >> 5), (uint32_t)npc, (uint32_t)(pp_begin >> 5), (uint32_t)npp);
             A.gnpp[g] = npp; A.gnpc[g] = npc;
-            const unsigned long long cnt = (unsigned long long)(ge - gb);
-            atomicAdd(&A.info->n_pp, cnt * npp); atomicAdd(&A.info->n_pc, cnt * npc);
+            const unsigned long long c = (unsigned long long)(ge - gb);
+            atomicAdd(&A.info->n_pp, c * npp); atomicAdd(&A.info->n_pc, c * npc);
             atomicAdd(&A.info->n_pp_list, (unsigned long long)npp); atomicAdd(&A.info->n_pc_list, (unsigned long long)npc);
+            if (ovf) atomicOr(&A.info->pool_overflow, 1);
         }
-        if (overflow) atomicOr(&A.info->stack_overflow, 1);
+    } else {
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+            if (tid[s] >= 0) A.nbcount[A.order[tid[s]]] = cnt[s];
     }
+    if (lane == 0 && overflow) atomicOr(&A.info->stack_overflow, 1);
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(WALK_THREADS, 4) k_walk(walk_args A)
+__global__ void __launch_bounds__(WALK_THREADS) k_walk(walk_args A)
 {
     __shared__ warp_smem smem[WALK_WARPS];
+    __shared__ count_smem csm[MODE == WALK_COUNT ? WALK_WARPS : 1];
     __shared__ float s_lt[24];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x < 24) s_lt[threadIdx.x] = __fdiv_rn(ldexpf(A.info->side, -(int)threadIdx.x), A.K.theta);
+    if (threadIdx.x < 24) s_lt[threadIdx.x] = __fdiv_rn(ldexpf(A.info->side, -(int)threadIdx.x), A.theta);
     __syncthreads();
     warp_smem& S = smem[w];
-    int32_t* spill = A.spill + (size_t)(blockIdx.x * WALK_WARPS + w) * SPILL_CAP;
+    const long long wg = (long long)blockIdx.x * WALK_WARPS + w;
+    int32_t* spill = A.spill + wg * SPILL_CAP;
+    long long pc_ptr = wg * A.cap_pc, pp_ptr = wg * A.cap_pp;
+    const long long pc_base = pc_ptr, pp_base = pp_ptr, pc_end = pc_ptr + A.cap_pc, pp_end = pp_ptr + A.cap_pp;
     const int ng = A.info->n_groups;
-    uint32_t* cursor = MODE == 1 ? &A.info->group_cursor : &A.info->group_cursor2;
+    uint32_t* cursor = MODE == WALK_LISTS ? &A.info->group_cursor : &A.info->group_cursor2;
     for (;;) {
         int g = 0;
         if (lane == 0) g = (int)atomicAdd(cursor, 1u);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ng) break;
-        const int gb = A.gbegin[g], ge = A.gbegin[g + 1];
-        if (ge - gb > 32) walk_group<2, MODE>(A, S, spill, g, gb, ge, s_lt);
-        else              walk_group<1, MODE>(A, S, spill, g, gb, ge, s_lt);
+        walk_group<MODE>(A, S, &csm[MODE == WALK_COUNT ? w : 0], spill, g, A.gbegin[g], A.gbegin[g + 1], s_lt, pc_ptr, pc_end, pp_ptr, pp_end);
         __syncwarp();
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// a10  neighbour CSR: exclusive scan of the per-particle counts (original order) -> int64 offsets
-// ---------------------------------------------------------------------------------------------
-#define SCAN_TILE 4096
-
-__global__ void __launch_bounds__(256) k_nb_blocksum(const int32_t* __restrict__ cnt, int n, long long* __restrict__ bsum,
-                                                     p3t_devinfo* info)
-{
-    __shared__ long long s_sum[8];
-    __shared__ int s_max[8];
-    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * 16;
-    long long t = 0; int mx = 0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) { int i = base + k; int v = i < n ? cnt[i] : 0; t += v; mx = max(mx, v); }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { t += __shfl_xor_sync(0xffffffffu, t, o); mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o)); }
-    if ((threadIdx.x & 31) == 0) { s_sum[threadIdx.x >> 5] = t; s_max[threadIdx.x >> 5] = mx; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int k = 1; k < 8; ++k) { t += s_sum[k]; mx = max(mx, s_max[k]); }
-        bsum[blockIdx.x] = t;
-        atomicMax(&info->nb_max, mx);
+    if (MODE == WALK_LISTS && lane == 0) {
+        atomicMax(&A.info->need_pc, (uint32_t)min(pc_ptr - pc_base, 0xffffffffll));
+        atomicMax(&A.info->need_pp, (uint32_t)min(pp_ptr - pp_base, 0xffffffffll));
     }
 }
 
-__global__ void __launch_bounds__(1024) k_nb_scansums(long long* __restrict__ bsum, int nb, long long* __restrict__ off_n,
-                                                      p3t_devinfo* info)
+__global__ void k_walk_reset(p3t_devinfo* info, int mode)
 {
-    __shared__ long long s_w[32];
-    __shared__ long long s_run;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_run = 0;
-    __syncthreads();
-    for (int b0 = 0; b0 < nb; b0 += 1024) {
-        const int b = b0 + threadIdx.x;
-        long long v = b < nb ? bsum[b] : 0, x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { long long y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-        if (lane == 31) s_w[w] = x;
-        __syncthreads();
-        long long add = s_run, tot = 0;
-        for (int k = 0; k < 32; ++k) { long long t = s_w[k]; if (k < w) add += t; tot += t; }
-        if (b < nb) bsum[b] = add + x - v;
-        __syncthreads();
-        if (threadIdx.x == 0) s_run += tot;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) { *off_n = s_run; info->nb_total = (unsigned long long)s_run; }
-}
-
-__global__ void __launch_bounds__(256) k_nb_offsets(const int32_t* __restrict__ cnt, int n, const long long* __restrict__ bsum,
-                                                    long long* __restrict__ off)
-{
-    __shared__ long long s_w[8];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int base = blockIdx.x * SCAN_TILE + threadIdx.x * 16;
-    int v[16]; long long t = 0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) { int i = base + k; v[k] = i < n ? cnt[i] : 0; t += v[k]; }
-    long long x = t;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { long long y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-    if (lane == 31) s_w[w] = x;
-    __syncthreads();
-    long long run = bsum[blockIdx.x] + x - t;
-    for (int k = 0; k < w; ++k) run += s_w[k];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) { int i = base + k; if (i < n) off[i] = run; run += v[k]; }
-}
-
-// rows ascending in original id: rank sort (ids inside a row are distinct), out of place.
-// Each lane sorts its own short row; rows longer than 16 are done by the whole warp.
-__global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
-                                                     int32_t* __restrict__ idx, int n)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
-    long long b = 0; int len = 0;
-    if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
-    if (len <= 16) {
-        for (int a = 0; a < len; ++a) {
-            const int v = raw[b + a]; int r = 0;
-            for (int c = 0; c < len; ++c) r += raw[b + c] < v;
-            idx[b + r] = v;
-        }
-    }
-    uint32_t m = __ballot_sync(0xffffffffu, len > 16);
-    while (m) {
-        const int src = __ffs(m) - 1; m &= m - 1;
-        const long long rb = __shfl_sync(0xffffffffu, b, src);
-        const int rl = __shfl_sync(0xffffffffu, len, src);
-        for (int a = lane; a < rl; a += 32) {
-            const int v = raw[rb + a]; int r = 0;
-            for (int c = 0; c < rl; ++c) r += raw[rb + c] < v;
-            idx[rb + r] = v;
-        }
+    if (mode == WALK_COUNT) { info->group_cursor2 = 0; info->nb_total = 0ull; info->nb_max = 0; }
+    else {
+        info->group_cursor = 0; info->group_cursor3 = 0;
+        info->n_pp = info->n_pc = info->n_pp_list = info->n_pc_list = 0ull;
+        info->pool_overflow = 0; info->need_pc = 0; info->need_pp = 0;
     }
 }
 
-__global__ void k_force_reset(p3t_devinfo* info)
+static int walk_blocks(p3t_ctx* ctx, int mode, int* out)
 {
-    info->group_cursor = 0; info->group_cursor2 = 0;
-    info->n_pp = info->n_pc = info->n_pp_list = info->n_pc_list = 0ull;
-    info->nb_total = 0ull; info->nb_max = 0;
-}
-
-// ---------------------------------------------------------------------------------------------
-static void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode)
-{
-    // fp32 thresholds exactly as DESIGN.md R10 states them: one fp32 product each
-    volatile float ro2 = r_out * r_out, ri2 = r_in * r_in;
-    K.rout2 = ro2; K.rin2 = ri2; K.r_in = r_in;
-    const double D = (double)r_out - (double)r_in, c = (double)r_in / D, c1 = 1.0 + c;
-    K.inv_delta = (float)(1.0 / D);
-    K.k140 = (float)(140.0 / D);
-    // t^3 (1-t)^3 = (t + c) (b5 t^5 + ... + b0) - c^3 (1+c)^3   (synthetic division at t = -c)
-    const double b[6] = { c * c * c1 * c1 * c1, -c * c1 * c1 * c1, c1 * c1 * c1, -(3.0 + 3.0 * c + c * c), 3.0 + c, -1.0 };
-    double s1 = 0.0;
-    for (int k = 0; k < 6; ++k) { K.sc[k] = (float)(b[k] / (k + 1)); s1 += b[k] / (k + 1); }
-    K.s1 = (float)s1;
-    K.rem = (float)(c * c * c * c1 * c1 * c1);
-    K.c = (float)c;
-    // psi(r_in) = -(140/D) [ S(1) + rem ln((1+c)/c) ... ] with W(0) = 0; here the remainder enters with a minus sign
-    K.psi_in = (float)(-(140.0 / D) * (s1 - c * c * c * c1 * c1 * c1 * log(c1 / c)));
-    K.theta = theta;
-    K.pot_mode = pot_mode;
-}
-
-int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot)
-{
-    const int n = (int)ctx->n;
     static int per_sm[2] = { 0, 0 };
-    if (!per_sm[0]) {
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], k_walk<0>, WALK_THREADS, 0));
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], k_walk<1>, WALK_THREADS, 0));
-        if (per_sm[0] < 1) per_sm[0] = 1;
-        if (per_sm[1] < 1) per_sm[1] = 1;
+    if (!per_sm[mode]) {
+        if (mode == WALK_COUNT) P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], k_walk<WALK_COUNT>, WALK_THREADS, 0));
+        else                    P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], k_walk<WALK_LISTS>, WALK_THREADS, 0));
+        if (per_sm[mode] < 1) per_sm[mode] = 1;
     }
-    int blocks0 = per_sm[0] * ctx->num_sms, blocks1 = per_sm[1] * ctx->num_sms;
-    if (getenv("P3T_CTAS")) blocks1 = atoi(getenv("P3T_CTAS")) * ctx->num_sms;
-    const int maxblocks = blocks0 > blocks1 ? blocks0 : blocks1;
-    int rc;
-    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)maxblocks * WALK_WARPS * SPILL_CAP * sizeof(int32_t)))) return rc;
-    const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
-    if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;
-    if ((rc = p3t_reserve(ctx, &ctx->nboff, ((size_t)n + 1) * 8))) return rc;
-    if ((rc = p3t_reserve(ctx, &ctx->nbcur, (size_t)nsb * 8 + 64))) return rc;
+    *out = per_sm[mode] * ctx->num_sms;
+    return P3T_OK;
+}
 
-    walk_args A;
+static void fill_args(p3t_ctx* ctx, walk_args& A, float r_out, float theta)
+{
     A.spm = P<float4>(ctx->spm); A.order = P<uint32_t>(ctx->idx[0]);
-    A.ncom = P<float4>(ctx->ncom); A.nlo = P<float4>(ctx->nlo); A.nhi = P<float4>(ctx->nhi);
-    A.nq0 = P<float4>(ctx->nq0); A.nq1 = P<float2>(ctx->nq1); A.nlink = P<int2>(ctx->nlink);
+    A.ncom = P<float4>(ctx->ncom); A.nlo = P<float4>(ctx->nlo); A.nhi = P<float4>(ctx->nhi); A.nlink = P<int2>(ctx->nlink);
     A.gbegin = P<int32_t>(ctx->gbegin); A.gnpp = P<int32_t>(ctx->gnpp); A.gnpc = P<int32_t>(ctx->gnpc);
-    A.nbcount = P<int32_t>(ctx->nbcount); A.nboff = P<int64_t>(ctx->nboff);
-    A.nbraw = nullptr; A.out = acc_pot; A.spill = P<int32_t>(ctx->spill); A.info = INFO(ctx);
-    make_consts(A.K, r_out, r_in, theta, pot_mode);
-    A.dbg = getenv("P3T_DBG") ? atoi(getenv("P3T_DBG")) : 0;
+    A.nbcount = P<int32_t>(ctx->nbcount);
+    A.pcpool = P<int32_t>(ctx->pcpool); A.pppool = P<int32_t>(ctx->pppool); A.glist = P<uint4>(ctx->glist);
+    A.cap_pc = ctx->pool_cap_pc; A.cap_pp = ctx->pool_cap_pp;
+    A.spill = P<int32_t>(ctx->spill); A.info = INFO(ctx);
+    volatile float ro2 = r_out * r_out;           // one fp32 product, as R10 states it
+    A.rout2 = ro2; A.theta = theta;
+}
 
-    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
-    k_force_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx));
-    // pass 1 (range search only): neighbour counts, so that the lists can be written in place
-    k_walk<0><<<blocks0, WALK_THREADS, 0, ctx->stream>>>(A);
-    k_nb_blocksum<<<nsb, 256, 0, ctx->stream>>>(A.nbcount, n, P<long long>(ctx->nbcur), INFO(ctx));
-    k_nb_scansums<<<1, 1024, 0, ctx->stream>>>(P<long long>(ctx->nbcur), nsb, P<long long>(ctx->nboff) + n, INFO(ctx));
-    k_nb_offsets<<<nsb, 256, 0, ctx->stream>>>(A.nbcount, n, P<long long>(ctx->nbcur), P<long long>(ctx->nboff));
+// a10, first half: neighbour counts per ORIGINAL id into ctx->nbcount
+int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta)
+{
+    int blocks, rc;
+    if ((rc = walk_blocks(ctx, WALK_COUNT, &blocks))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)ctx->walk_warps_max * SPILL_CAP * sizeof(int32_t)))) return rc;
+    walk_args A; fill_args(ctx, A, r_out, theta);
+    k_walk_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx), WALK_COUNT);
+    k_walk<WALK_COUNT><<<blocks, WALK_THREADS, 0, ctx->stream>>>(A);
     P3T_CUDA(ctx, cudaGetLastError());
-    // the list buffers are sized from the total: the one host synchronisation of this call
-    long long total = 0;
-    P3T_CUDA(ctx, cudaMemcpyAsync(&total, P<long long>(ctx->nboff) + n, 8, cudaMemcpyDeviceToHost, ctx->stream));
-    P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    ctx->nb_total_host = total;
-    if ((rc = p3t_reserve(ctx, &ctx->nbidx, (size_t)total * 4 + 64))) return rc;
-    p3t_buf* raw = &ctx->stage_out;      // unsorted rows share the host-staging scratch
-    if ((rc = p3t_reserve(ctx, raw, (size_t)total * 4 + 64))) return rc;
-    A.nbraw = P<int32_t>(*raw);
-    // pass 2: walk + force + emission
-    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
-    k_walk<1><<<blocks1, WALK_THREADS, 0, ctx->stream>>>(A);
-    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
-    k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    ctx->launches += 2;
+    return P3T_OK;
+}
+
+// a7: interaction lists.  Sizes the pools on first use (and after an overflow, from the measured need).
+int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta)
+{
+    int blocks, rc;
+    if ((rc = walk_blocks(ctx, WALK_LISTS, &blocks))) return rc;
+    const long long warps = (long long)blocks * WALK_WARPS;
+    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)ctx->walk_warps_max * SPILL_CAP * sizeof(int32_t)))) return rc;
+    if (ctx->pool_cap_pc == 0) {
+        // first call: a guess from the group count (lists of the paper's workloads hold 4-8 thousand
+        // cells and 1-3 thousand particles at theta = 0.4); corrected below if it was too small
+        const long long ng = (ctx->n + 31) / 32;
+        ctx->pool_cap_pc = ((ng * 6000 / warps + 16384) + 31) & ~31ll;
+        ctx->pool_cap_pp = ((ng * 3000 / warps + 16384) + 31) & ~31ll;
+    }
+    if ((rc = p3t_reserve(ctx, &ctx->pcpool, (size_t)(warps * ctx->pool_cap_pc) * 4))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->pppool, (size_t)(warps * ctx->pool_cap_pp) * 4))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->glist, ((size_t)ctx->n + 1) * sizeof(uint4)))) return rc;
+    walk_args A; fill_args(ctx, A, r_out, theta);
+    k_walk_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx), WALK_LISTS);
+    k_walk<WALK_LISTS><<<blocks, WALK_THREADS, 0, ctx->stream>>>(A);
     P3T_CUDA(ctx, cudaGetLastError());
-    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
-    ctx->launches += 7;
+    ctx->launches += 2;
+    ctx->walk_list_warps = warps;
+    return P3T_OK;
+}
+
+int p3t_walk_init(p3t_ctx* ctx)
+{
+    int b0, b1, rc;
+    if ((rc = walk_blocks(ctx, WALK_COUNT, &b0))) return rc;
+    if ((rc = walk_blocks(ctx, WALK_LISTS, &b1))) return rc;
+    ctx->walk_warps_max = (long long)(b0 > b1 ? b0 : b1) * WALK_WARPS;
     return P3T_OK;
 }
