@@ -252,29 +252,38 @@ __device__ __forceinline__ void eval_pp(target<NS>& T, const float (*pp)[TILE], 
 // ---------------------------------------------------------------------------------------------
 // one target group against its two lists
 // ---------------------------------------------------------------------------------------------
-struct pc_regs { float v[10]; };
-struct pp_regs { float x, y, z, m; int j; };
+// Software pipeline of the list stream: the ids of tile t+2 and the node / particle data of tile
+// t+1 are in flight while tile t is evaluated; nothing is consumed before the evaluation is over
+// (the quadrupole is negated on its way to shared memory, not at the load).
+struct pc_regs { float4 c, q0; float2 q1; };
+struct pp_regs { float4 p; int j; };
 
-__device__ __forceinline__ pc_regs load_pc(const force_args& A, const int32_t* ids, int e, int n)
+__device__ __forceinline__ int load_id(const int32_t* ids, int e, int n) { return e < n ? ids[e] : -1; }
+
+__device__ __forceinline__ pc_regs gather_pc(const force_args& A, int id)
 {
     pc_regs r;
-    if (e < n) {
-        const int id = ids[e];
-        const float4 c = A.ncom[id], q0 = A.nq0[id]; const float2 q1 = A.nq1[id];
-        r.v[0] = c.x; r.v[1] = c.y; r.v[2] = c.z; r.v[3] = c.w;
-        r.v[4] = -q0.x; r.v[5] = -q0.y; r.v[6] = -q0.z; r.v[7] = -q0.w; r.v[8] = -q1.x; r.v[9] = -q1.y;
-    } else {                                   // padding: a zero-mass cell far away contributes exactly 0
-#pragma unroll
-        for (int k = 0; k < 10; ++k) r.v[k] = k < 3 ? FAR_AWAY : 0.0f;
+    if (id >= 0) { r.c = A.ncom[id]; r.q0 = A.nq0[id]; r.q1 = A.nq1[id]; }
+    else {                                     // padding: a zero-mass cell far away contributes exactly 0
+        r.c = make_float4(FAR_AWAY, FAR_AWAY, FAR_AWAY, 0.0f); r.q0 = make_float4(0, 0, 0, 0); r.q1 = make_float2(0, 0);
     }
     return r;
 }
-__device__ __forceinline__ pp_regs load_pp(const force_args& A, const int32_t* ids, int e, int n)
+__device__ __forceinline__ void store_pc(float (*pc)[TILE], int lane, const pc_regs& r)
 {
-    pp_regs r;
-    if (e < n) { r.j = ids[e]; const float4 p = A.spm[r.j]; r.x = p.x; r.y = p.y; r.z = p.z; r.m = p.w; }
-    else { r.x = r.y = r.z = FAR_AWAY; r.m = 0.0f; r.j = -1; }
+    pc[0][lane] = r.c.x; pc[1][lane] = r.c.y; pc[2][lane] = r.c.z; pc[3][lane] = r.c.w;
+    pc[4][lane] = -r.q0.x; pc[5][lane] = -r.q0.y; pc[6][lane] = -r.q0.z; pc[7][lane] = -r.q0.w;
+    pc[8][lane] = -r.q1.x; pc[9][lane] = -r.q1.y;
+}
+__device__ __forceinline__ pp_regs gather_pp(const force_args& A, int id)
+{
+    pp_regs r; r.j = id;
+    if (id >= 0) r.p = A.spm[id]; else r.p = make_float4(FAR_AWAY, FAR_AWAY, FAR_AWAY, 0.0f);
     return r;
+}
+__device__ __forceinline__ void store_pp(float (*pp)[TILE], int* ppj, int lane, const pp_regs& r)
+{
+    pp[0][lane] = r.p.x; pp[1][lane] = r.p.y; pp[2][lane] = r.p.z; pp[3][lane] = r.p.w; ppj[lane] = r.j;
 }
 
 template <int NS>
@@ -302,19 +311,17 @@ __device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, in
         const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
         const int n = (int)rec.y, nt = (n + TILE - 1) / TILE;
         if (nt > 0) {
-            pc_regs r = load_pc(A, ids, lane, n);
-#pragma unroll
-            for (int k = 0; k < 10; ++k) S.pc[0][k][lane] = r.v[k];
+            pc_regs r = gather_pc(A, load_id(ids, lane, n));
+            int idn = load_id(ids, TILE + lane, n);
+            store_pc(S.pc[0], lane, r);
             __syncwarp();
             for (int t = 0; t < nt; ++t) {
                 const bool more = t + 1 < nt;
-                if (more) r = load_pc(A, ids, (t + 1) * TILE + lane, n);      // in flight during the evaluation
+                if (more) r = gather_pc(A, idn);
+                idn = load_id(ids, (t + 2) * TILE + lane, n);
                 eval_pc<NS>(T, S.pc[t & 1], TILE);
                 fold(T);
-                if (more) {
-#pragma unroll
-                    for (int k = 0; k < 10; ++k) S.pc[(t + 1) & 1][k][lane] = r.v[k];
-                }
+                if (more) store_pc(S.pc[(t + 1) & 1], lane, r);
                 __syncwarp();
             }
         }
@@ -324,16 +331,18 @@ __device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, in
         const int32_t* ids = A.pppool + ((long long)rec.z << 5);
         const int n = (int)rec.w, nt = (n + TILE - 1) / TILE;
         if (nt > 0) {
-            pp_regs r = load_pp(A, ids, lane, n);
-            S.pp[0][0][lane] = r.x; S.pp[0][1][lane] = r.y; S.pp[0][2][lane] = r.z; S.pp[0][3][lane] = r.m; S.ppj[0][lane] = r.j;
+            pp_regs r = gather_pp(A, load_id(ids, lane, n));
+            int idn = load_id(ids, TILE + lane, n);
+            store_pp(S.pp[0], S.ppj[0], lane, r);
             __syncwarp();
             for (int t = 0; t < nt; ++t) {
                 const bool more = t + 1 < nt;
-                const int b = t & 1, nbuf = b ^ 1;
-                if (more) r = load_pp(A, ids, (t + 1) * TILE + lane, n);
+                const int b = t & 1;
+                if (more) r = gather_pp(A, idn);
+                idn = load_id(ids, (t + 2) * TILE + lane, n);
                 eval_pp<NS>(T, S.pp[b], S.ppj[b], TILE, A);
                 if (b) fold(T);                                           // every 64 particles
-                if (more) { S.pp[nbuf][0][lane] = r.x; S.pp[nbuf][1][lane] = r.y; S.pp[nbuf][2][lane] = r.z; S.pp[nbuf][3][lane] = r.m; S.ppj[nbuf][lane] = r.j; }
+                if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
             }
             fold(T);
