@@ -17,6 +17,7 @@
 
 #define FORCE_WARPS   4
 #define FORCE_THREADS (FORCE_WARPS * 32)
+#define FORCE_CTAS_PER_SM 5
 #define TILE          32                  // list entries per tile
 #define FAR_AWAY      1.0e18f             // position of the zero-mass padding entries of a tile
 
@@ -52,6 +53,7 @@ struct __align__(16) tile_smem {
     float pc[2][10][TILE];
     float pp[2][4][TILE];       // x y z m
     int   ppj[2][TILE];         // sorted position of the source, -1 = padding
+    int   nbrow[32];            // per target of the item: neighbours already written to its CSR row
 };
 
 __device__ __forceinline__ float rsqrt_approx(float x)
@@ -91,77 +93,74 @@ __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float
     return -W * rinv - K.k140 * integral;
 }
 
-// NS target slots per lane.  Every accumulator is a packed pair: .lo sums the even list entries,
-// .hi the odd ones.  ph accumulates MINUS the potential of the far terms; the rare near-zone terms
-// (cutoff branch) go to the scalar n* accumulators with their true sign.
-template <int NS> struct target {
-    float x[NS], y[NS], z[NS];
-    f2    ph[NS];                                // fp32 partial sums of the current tile: -potential (packed)
-    float axe[NS], aye[NS], aze[NS];             // acceleration from the even list entries ...
-    float axo[NS], ayo[NS], azo[NS];             // ... and from the odd ones (scalar FFMAs, see pc_pair)
-    float nax[NS], nay[NS], naz[NS], nph[NS];
-    double dax[NS], day[NS], daz[NS], dph[NS];   // fp64 masters (R-S9)
-    int   id[NS];                                // sorted position of the target, -1 = no target
-    long long cur[NS];                           // neighbour write cursor
+// One work item = up to 32 targets of one group (a group of 33..64 particles makes two items that
+// stream the same lists).  An item with c <= 16 targets gives every target k = 2, 4 or 8 lanes
+// ("parts"): lane = target * k + part, and part p evaluates the 4-entry blocks p, p + k, ... of every
+// tile, so that a half-empty item costs half the time instead of idling half the lanes.  The parts
+// of a target are summed by shuffles at the end.
+//
+// Every accumulator is a pair: .lo / e sums the even list entries, .hi / o the odd ones.  ph
+// accumulates MINUS the potential of the far terms; the rare near-zone terms (cutoff branch) go to
+// the scalar n* accumulators with their true sign.
+struct target {
+    float x, y, z;
+    f2    ph;                                    // fp32 partial sums since the last fold
+    float axe, aye, aze, axo, ayo, azo;          // scalar FFMAs: see pc_pair
+    float nax, nay, naz, nph;
+    double dax, day, daz, dph;                   // fp64 masters (R-S9)
+    int   id;                                    // sorted position of the target, -1 = idle lane
+    int   slot;                                  // index of the target inside the item (row of the neighbour cursor)
 };
 
-template <int NS> __device__ __forceinline__ void fold(target<NS>& T)
+__device__ __forceinline__ void fold(target& T)
 {
-    const f2 zero = pk(0.0f, 0.0f);
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        T.dax[s] += (double)((T.axe[s] + T.axo[s]) + T.nax[s]);
-        T.day[s] += (double)((T.aye[s] + T.ayo[s]) + T.nay[s]);
-        T.daz[s] += (double)((T.aze[s] + T.azo[s]) + T.naz[s]);
-        T.dph[s] += (double)(T.nph[s] - (f2lo(T.ph[s]) + f2hi(T.ph[s])));
-        T.ph[s] = zero;
-        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
-        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
-    }
+    T.dax += (double)((T.axe + T.axo) + T.nax);
+    T.day += (double)((T.aye + T.ayo) + T.nay);
+    T.daz += (double)((T.aze + T.azo) + T.naz);
+    T.dph += (double)(T.nph - (f2lo(T.ph) + f2hi(T.ph)));
+    T.ph = pk(0.0f, 0.0f);
+    T.axe = T.aye = T.aze = T.axo = T.ayo = T.azo = 0.0f;
+    T.nax = T.nay = T.naz = T.nph = 0.0f;
 }
 
 // R-S8 particle-cell, monopole + traceless quadrupole, two cells per packed operation.
 // With d = COM - x_i (= -r), Q' = -Q (stored negated in the tile), R = |d|:
 //   q' = d.Q'.d / R^5,  -phi = M/R - q'/2,  a = (M/R - (5/2) q') d / R^2 + (Q'.d) / R^5
-// which is a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7 of R-S8: 33 packed operations per pair.
-template <int NS> __device__ __forceinline__ void pc_pair(target<NS>& T, f2 cx, f2 cy, f2 cz, f2 cm,
-                                                          f2 qxx, f2 qyy, f2 qzz, f2 qxy, f2 qxz, f2 qyz)
+// which is a = -M r/R^3 + Q.r/R^5 - (5/2)(r.Q.r) r/R^7 of R-S8.
+__device__ __forceinline__ void pc_pair(target& T, f2 cx, f2 cy, f2 cz, f2 cm, f2 qxx, f2 qyy, f2 qzz, f2 qxy, f2 qxz, f2 qyz)
 {
     const f2 mhalf = pk(-0.5f, -0.5f), m52 = pk(-2.5f, -2.5f);
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const f2 dx = sub2(cx, pk(T.x[s], T.x[s])), dy = sub2(cy, pk(T.y[s], T.y[s])), dz = sub2(cz, pk(T.z[s], T.z[s]));
-        const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
-        const f2 ri2 = mul2(ri, ri);
-        const f2 qx = fma2(qxz, dz, fma2(qxy, dy, mul2(qxx, dx)));
-        const f2 qy = fma2(qyz, dz, fma2(qyy, dy, mul2(qxy, dx)));
-        const f2 qz = fma2(qzz, dz, fma2(qyz, dy, mul2(qxz, dx)));
-        const f2 dqd = fma2(dz, qz, fma2(dy, qy, mul2(dx, qx)));
-        const f2 ri3 = mul2(ri2, ri), ri5 = mul2(ri3, ri2);
-        const f2 mono = mul2(cm, ri);
-        const f2 q5 = mul2(dqd, ri5);
-        T.ph[s] = fma2(mhalf, q5, add2(T.ph[s], mono));
-        const f2 cr = mul2(fma2(m52, q5, mono), ri2);
-        // An FFMA2 with three distinct register-pair operands occupies the pipe for 3 cycles (measured:
-        // operand bandwidth), two scalar FFMAs for 2: the accumulations are issued on the halves.
-        const float crl = f2lo(cr), crh = f2hi(cr), r5l = f2lo(ri5), r5h = f2hi(ri5);
-        T.axe[s] = fmaf(f2lo(qx), r5l, fmaf(crl, f2lo(dx), T.axe[s])); T.axo[s] = fmaf(f2hi(qx), r5h, fmaf(crh, f2hi(dx), T.axo[s]));
-        T.aye[s] = fmaf(f2lo(qy), r5l, fmaf(crl, f2lo(dy), T.aye[s])); T.ayo[s] = fmaf(f2hi(qy), r5h, fmaf(crh, f2hi(dy), T.ayo[s]));
-        T.aze[s] = fmaf(f2lo(qz), r5l, fmaf(crl, f2lo(dz), T.aze[s])); T.azo[s] = fmaf(f2hi(qz), r5h, fmaf(crh, f2hi(dz), T.azo[s]));
-    }
+    const f2 dx = sub2(cx, pk(T.x, T.x)), dy = sub2(cy, pk(T.y, T.y)), dz = sub2(cz, pk(T.z, T.z));
+    const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
+    const f2 ri2 = mul2(ri, ri);
+    const f2 qx = fma2(qxz, dz, fma2(qxy, dy, mul2(qxx, dx)));
+    const f2 qy = fma2(qyz, dz, fma2(qyy, dy, mul2(qxy, dx)));
+    const f2 qz = fma2(qzz, dz, fma2(qyz, dy, mul2(qxz, dx)));
+    const f2 dqd = fma2(dz, qz, fma2(dy, qy, mul2(dx, qx)));
+    const f2 ri3 = mul2(ri2, ri), ri5 = mul2(ri3, ri2);
+    const f2 mono = mul2(cm, ri);
+    const f2 q5 = mul2(dqd, ri5);
+    T.ph = fma2(mhalf, q5, add2(T.ph, mono));
+    const f2 cr = mul2(fma2(m52, q5, mono), ri2);
+    // An FFMA2 with three distinct register-pair operands occupies the pipe for 3 cycles (measured:
+    // operand bandwidth), two scalar FFMAs for 2: the accumulations are issued on the halves.
+    const float crl = f2lo(cr), crh = f2hi(cr), r5l = f2lo(ri5), r5h = f2hi(ri5);
+    T.axe = fmaf(f2lo(qx), r5l, fmaf(crl, f2lo(dx), T.axe)); T.axo = fmaf(f2hi(qx), r5h, fmaf(crh, f2hi(dx), T.axo));
+    T.aye = fmaf(f2lo(qy), r5l, fmaf(crl, f2lo(dy), T.aye)); T.ayo = fmaf(f2hi(qy), r5h, fmaf(crh, f2hi(dy), T.ayo));
+    T.aze = fmaf(f2lo(qz), r5l, fmaf(crl, f2lo(dz), T.aze)); T.azo = fmaf(f2hi(qz), r5h, fmaf(crh, f2hi(dz), T.azo));
 }
 
-// cnt is a multiple of 4 (the tail of a list is padded with zero-mass cells FAR_AWAY)
-template <int NS> __device__ __forceinline__ void eval_pc(target<NS>& T, const float (*pc)[TILE], int cnt)
+// one tile of TILE cells; this lane takes the 4-entry blocks part, part + k, ...
+__device__ __forceinline__ void eval_pc(target& T, const float (*pc)[TILE], int part, int k)
 {
 #pragma unroll 1
-    for (int e = 0; e < cnt; e += 4) {
+    for (int e = 4 * part; e < TILE; e += 4 * k) {
         ulonglong2 v[10];
 #pragma unroll
-        for (int k = 0; k < 10; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&pc[k][e]);
-        pc_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
-        pc_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
+        for (int r = 0; r < 10; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pc[r][e]);
+        pc_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
+        pc_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
     }
 }
 
@@ -169,59 +168,53 @@ template <int NS> __device__ __forceinline__ void eval_pc(target<NS>& T, const f
 // p-p list, branch-free.  d2 follows R10 bit for bit (sub, mul, fma, fma; all rn).  A near pair is
 // masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
 // by the lane is returned so that the caller knows whether the tile needs the near pass.
-template <int NS>
-__device__ __forceinline__ float pp_far_pair(target<NS>& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
+__device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
 {
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const f2 dx = sub2(px, pk(T.x[s], T.x[s])), dy = sub2(py, pk(T.y[s], T.y[s])), dz = sub2(pz, pk(T.z[s], T.z[s]));
-        const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        const float d2a = f2lo(d2), d2b = f2hi(d2);
-        dmin = fminf(dmin, fminf(d2a, d2b));
-        const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
-        const f2 mri = mul2(pm, ri);
-        const f2 f = mul2(mri, mul2(ri, ri));
-        T.ph[s] = add2(T.ph[s], mri);
-        const float fl = f2lo(f), fh = f2hi(f);
-        T.axe[s] = fmaf(fl, f2lo(dx), T.axe[s]); T.axo[s] = fmaf(fh, f2hi(dx), T.axo[s]);
-        T.aye[s] = fmaf(fl, f2lo(dy), T.aye[s]); T.ayo[s] = fmaf(fh, f2hi(dy), T.ayo[s]);
-        T.aze[s] = fmaf(fl, f2lo(dz), T.aze[s]); T.azo[s] = fmaf(fh, f2hi(dz), T.azo[s]);
-    }
+    const f2 dx = sub2(px, pk(T.x, T.x)), dy = sub2(py, pk(T.y, T.y)), dz = sub2(pz, pk(T.z, T.z));
+    const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    const float d2a = f2lo(d2), d2b = f2hi(d2);
+    dmin = fminf(dmin, fminf(d2a, d2b));
+    const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
+    const f2 mri = mul2(pm, ri);
+    const f2 f = mul2(mri, mul2(ri, ri));
+    T.ph = add2(T.ph, mri);
+    const float fl = f2lo(f), fh = f2hi(f);
+    T.axe = fmaf(fl, f2lo(dx), T.axe); T.axo = fmaf(fh, f2hi(dx), T.axo);
+    T.aye = fmaf(fl, f2lo(dy), T.aye); T.ayo = fmaf(fh, f2hi(dy), T.ayo);
+    T.aze = fmaf(fl, f2lo(dz), T.aze); T.azo = fmaf(fh, f2hi(dz), T.azo);
     return dmin;
 }
 
-// R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission and the
-// cutoff-weighted pair term.  Scalar pass over a tile, run only by warps whose tile came within
-// r_out of one of their targets (about one tile in eight).
-template <int NS>
-__device__ __forceinline__ void pp_near_pass(target<NS>& T, const float (*pp)[TILE], const int* ppj, int cnt, const force_args& A)
+// R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission and the cutoff-weighted pair term.
+// Scalar pass over this lane's blocks of a tile, run only by warps whose tile came within r_out of
+// one of their targets (about one tile in eight).  nbrow[slot] counts the entries already written
+// to the target's CSR row (shared by the parts of a target).
+__device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
+                                             long long rowbase, int* nbrow, const force_args& A)
 {
     const walk_consts& K = A.K;
 #pragma unroll 1
-    for (int e = 0; e < cnt; ++e) {
-        const float px = pp[0][e], py = pp[1][e], pz = pp[2][e];
-#pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            const float dx = __fsub_rn(px, T.x[s]), dy = __fsub_rn(py, T.y[s]), dz = __fsub_rn(pz, T.z[s]);
+    for (int e0 = 4 * part; e0 < TILE; e0 += 4 * k) {
+#pragma unroll 1
+        for (int e = e0; e < e0 + 4; ++e) {
+            const float dx = __fsub_rn(pp[0][e], T.x), dy = __fsub_rn(pp[1][e], T.y), dz = __fsub_rn(pp[2][e], T.z);
             const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
             if (d2 < K.rout2) {
                 const int j = ppj[e];
-                if (T.id[s] >= 0 && j != T.id[s]) {                  // self excluded by index; idle lanes
-                    A.nbraw[T.cur[s]++] = (int32_t)A.order[j];
-                    {
-                        const float m = pp[3][e];
-                        if (d2 > K.rin2) {
-                            const float ri = rsqrt_approx(d2), r = d2 * ri;
-                            const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
-                            const float W = cutoff_W(x);
-                            const float f = m * W * ri * ri * ri;
-                            T.nax[s] = fmaf(f, dx, T.nax[s]); T.nay[s] = fmaf(f, dy, T.nay[s]); T.naz[s] = fmaf(f, dz, T.naz[s]);
-                            T.nph[s] += K.pot_mode == 0 ? m * cutoff_psi(K, x, W, ri) : -m * ri;
-                        } else if (K.pot_mode == 0) {
-                            T.nph[s] = fmaf(m, K.psi_in, T.nph[s]);    // inside r_in: constant psi(r_in), also r = 0 (R8)
-                        } else if (d2 > 0.0f) {
-                            T.nph[s] -= m * rsqrt_approx(d2);
-                        }
+                if (T.id >= 0 && j != T.id) {                        // self excluded by index; idle lanes
+                    A.nbraw[rowbase + atomicAdd(&nbrow[T.slot], 1)] = (int32_t)A.order[j];
+                    const float m = pp[3][e];
+                    if (d2 > K.rin2) {
+                        const float ri = rsqrt_approx(d2), r = d2 * ri;
+                        const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
+                        const float W = cutoff_W(x);
+                        const float f = m * W * ri * ri * ri;
+                        T.nax = fmaf(f, dx, T.nax); T.nay = fmaf(f, dy, T.nay); T.naz = fmaf(f, dz, T.naz);
+                        T.nph += K.pot_mode == 0 ? m * cutoff_psi(K, x, W, ri) : -m * ri;
+                    } else if (K.pot_mode == 0) {
+                        T.nph = fmaf(m, K.psi_in, T.nph);              // inside r_in: constant psi(r_in), also r = 0 (R8)
+                    } else if (d2 > 0.0f) {
+                        T.nph -= m * rsqrt_approx(d2);
                     }
                 }
             }
@@ -229,29 +222,22 @@ __device__ __forceinline__ void pp_near_pass(target<NS>& T, const float (*pp)[TI
     }
 }
 
-// cnt is a multiple of 4 (tail padded with zero-mass particles FAR_AWAY, index -1)
-template <int NS>
-__device__ __forceinline__ void eval_pp(target<NS>& T, const float (*pp)[TILE], const int* ppj, int cnt, const force_args& A)
+__device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
+                                        long long rowbase, int* nbrow, const force_args& A)
 {
-    {
-        float dmin = INFINITY;
+    float dmin = INFINITY;
 #pragma unroll 1
-        for (int e = 0; e < cnt; e += 4) {
-            ulonglong2 v[4];
+    for (int e = 4 * part; e < TILE; e += 4 * k) {
+        ulonglong2 v[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) v[k] = *reinterpret_cast<const ulonglong2*>(&pp[k][e]);
-            dmin = pp_far_pair<NS>(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
-            dmin = pp_far_pair<NS>(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
-        }
-        if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
+        for (int r = 0; r < 4; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pp[r][e]);
+        dmin = pp_far_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
+        dmin = pp_far_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
     }
-    pp_near_pass<NS>(T, pp, ppj, cnt, A);
+    if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
+    pp_near_pass(T, pp, ppj, part, k, rowbase, nbrow, A);
 }
 
-
-// ---------------------------------------------------------------------------------------------
-// one target group against its two lists
-// ---------------------------------------------------------------------------------------------
 // Software pipeline of the list stream: the ids of tile t+2 and the node / particle data of tile
 // t+1 are in flight while tile t is evaluated; nothing is consumed before the evaluation is over
 // (the quadrupole is negated on its way to shared memory, not at the load).
@@ -286,27 +272,36 @@ __device__ __forceinline__ void store_pp(float (*pp)[TILE], int* ppj, int lane, 
     pp[0][lane] = r.p.x; pp[1][lane] = r.p.y; pp[2][lane] = r.p.z; pp[3][lane] = r.p.w; ppj[lane] = r.j;
 }
 
-template <int NS>
-__device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, int ge)
+__device__ __forceinline__ double shfl_xor_double(double v, int o)
+{
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_xor_sync(0xffffffffu, lo, o); hi = __shfl_xor_sync(0xffffffffu, hi, o);
+    return __hiloint2double(hi, lo);
+}
+
+// targets [tb, te) (sorted positions, te - tb <= 32) of group g against the group's two lists
+__device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te)
 {
     const int lane = threadIdx.x & 31;
-    target<NS> T;
-    const float4 pfirst = A.spm[gb];
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const int i = gb + s * 32 + lane;
-        const bool v = i < ge;
-        const float4 p = v ? A.spm[i] : pfirst;
-        T.x[s] = p.x; T.y[s] = p.y; T.z[s] = p.z;
-        T.ph[s] = pk(0.0f, 0.0f);
-        T.axe[s] = T.aye[s] = T.aze[s] = T.axo[s] = T.ayo[s] = T.azo[s] = 0.0f;
-        T.nax[s] = T.nay[s] = T.naz[s] = T.nph[s] = 0.0f;
-        T.dax[s] = T.day[s] = T.daz[s] = T.dph[s] = 0.0;
-        T.id[s] = v ? i : -1;
-        T.cur[s] = v ? A.nboff[A.order[i]] : 0;
-    }
+    const int c = te - tb;
+    const int kshift = c > 16 ? 0 : c > 8 ? 1 : c > 4 ? 2 : 3;     // k = 1, 2, 4, 8 lanes per target
+    const int k = 1 << kshift, part = lane & (k - 1);
+    target T;
+    T.slot = lane >> kshift;
+    const bool v = T.slot < c;
+    const float4 p = A.spm[v ? tb + T.slot : tb];
+    T.x = p.x; T.y = p.y; T.z = p.z;
+    T.id = v ? tb + T.slot : -1;
+    T.dax = T.day = T.daz = T.dph = 0.0;
+    T.ph = pk(0.0f, 0.0f);
+    T.axe = T.aye = T.aze = T.axo = T.ayo = T.azo = 0.0f;
+    T.nax = T.nay = T.naz = T.nph = 0.0f;
+    const uint32_t orig = v ? A.order[T.id] : 0u;
+    const long long rowbase = v ? A.nboff[orig] : 0;
+    S.nbrow[lane] = 0;
     const uint4 rec = A.glist[g];
-    // ---- a8: particle-cell list ----
+    __syncwarp();
+    // ---- a8: particle-cell list; a lane sees TILE / k cells per tile: fold every k tiles ----
     {
         const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
         const int n = (int)rec.y, nt = (n + TILE - 1) / TILE;
@@ -319,14 +314,15 @@ __device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, in
                 const bool more = t + 1 < nt;
                 if (more) r = gather_pc(A, idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pc<NS>(T, S.pc[t & 1], TILE);
-                fold(T);
+                eval_pc(T, S.pc[t & 1], part, k);
+                if (((t + 1) & (k - 1)) == 0) fold(T);
                 if (more) store_pc(S.pc[(t + 1) & 1], lane, r);
                 __syncwarp();
             }
+            fold(T);
         }
     }
-    // ---- a9: particle-particle list (cutoff, neighbour emission) ----
+    // ---- a9: particle-particle list (cutoff, neighbour emission): fold every 2k tiles ----
     {
         const int32_t* ids = A.pppool + ((long long)rec.z << 5);
         const int n = (int)rec.w, nt = (n + TILE - 1) / TILE;
@@ -340,36 +336,40 @@ __device__ void force_group(const force_args& A, tile_smem& S, int g, int gb, in
                 const int b = t & 1;
                 if (more) r = gather_pp(A, idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pp<NS>(T, S.pp[b], S.ppj[b], TILE, A);
-                if (b) fold(T);                                           // every 64 particles
+                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
+                if (((t + 1) & (2 * k - 1)) == 0) fold(T);
                 if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
             }
             fold(T);
         }
     }
-    // ---- a11: results to the caller's order ----
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        if (T.id[s] < 0) continue;
-        A.out[A.order[T.id[s]]] = make_float4((float)T.dax[s], (float)T.day[s], (float)T.daz[s], (float)T.dph[s]);
+    // ---- the parts of a target are adjacent lanes: sum them (fixed order) ----
+    for (int o = 1; o < k; o <<= 1) {
+        T.dax += shfl_xor_double(T.dax, o); T.day += shfl_xor_double(T.day, o);
+        T.daz += shfl_xor_double(T.daz, o); T.dph += shfl_xor_double(T.dph, o);
     }
+    // ---- a11: results to the caller's order ----
+    if (v && part == 0) A.out[orig] = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
 }
 
-__global__ void __launch_bounds__(FORCE_THREADS, 4) k_force(force_args A)
+// work item 2g + s: slot s (32 targets) of group g; dynamic scheduling, persistent grid
+__global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(force_args A)
 {
     __shared__ tile_smem smem[FORCE_WARPS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     tile_smem& S = smem[w];
-    const int ng = A.info->n_groups;
+    const int nitems = 2 * A.info->n_groups;
     for (;;) {
-        int g = 0;
-        if (lane == 0) g = (int)atomicAdd(&A.info->group_cursor3, 1u);
-        g = __shfl_sync(0xffffffffu, g, 0);
-        if (g >= ng) break;
+        int it = 0;
+        if (lane == 0) it = (int)atomicAdd(&A.info->group_cursor3, 1u);
+        it = __shfl_sync(0xffffffffu, it, 0);
+        if (it >= nitems) break;
+        const int g = it >> 1, s = it & 1;
         const int gb = A.gbegin[g], ge = A.gbegin[g + 1];
-        if (ge - gb > 32) force_group<2>(A, S, g, gb, ge);
-        else              force_group<1>(A, S, g, gb, ge);
+        const int tb = gb + 32 * s;
+        if (tb >= ge) continue;
+        force_item(A, S, g, tb, min(ge, tb + 32));
         __syncwarp();
     }
 }
