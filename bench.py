@@ -35,6 +35,8 @@ if str(ROOT) not in sys.path:
 # FP32-pipe instructions the method needs per interaction
 INSTR_PP, INSTR_PC = 15, 37
 FLOP_PP, FLOP_PC = 20, 60
+# DRAM traffic of the dominant kernel from the committed ncu capture (profiles/), per launch, by workload
+TRAFFIC_NCU = {"plummer1m_kroupa": 752.8e6}
 
 
 def peaks():
@@ -185,7 +187,7 @@ def run_ours(args, w, rank, world, local_rank, dist):
     sampler = ClockSampler(local_rank)
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    walk_ms, build_ms, force_ms, sort_ms = [], [], [], []
+    walk_ms, build_ms, force_ms, sort_ms, eval_ms, count_ms = [], [], [], [], [], []
     for k in range(args.steps):
         flush.zero_()                                     # L2 flush between timed iterations (outside the event pair)
         ev[k][0].record()
@@ -193,6 +195,7 @@ def run_ours(args, w, rank, world, local_rank, dist):
         ev[k][1].record()
         st = ctx.stats()                                  # synchronises; after the closing event
         walk_ms.append(st["ms_walk"]); build_ms.append(st["ms_build"]); force_ms.append(st["ms_force"]); sort_ms.append(st["ms_sort"])
+        eval_ms.append(st["ms_eval"]); count_ms.append(st["ms_count"])
     barrier()
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in ev]
@@ -229,15 +232,16 @@ def run_ours(args, w, rank, world, local_rank, dist):
     value = units / (total_ms_max * 1e-3)
     e2e_value = units / (e2e_ms_max * 1e-3)
     n_int = st["n_pp"] + st["n_pc"]
-    wms = float(np.mean(walk_ms))
+    wms = float(np.mean(eval_ms))                        # the dominant kernel: k_force
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     alg_instr = INSTR_PP * st["n_pp"] + INSTR_PC * st["n_pc"]
     peak_instr = sms * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # Tinstr/s, FP32 lanes x clock
     achieved = alg_instr / (wms * 1e-3) / 1e12
     roofline = {
-        "bound": "alu", "kernel": "k_walk<1> (walk + p-c/p-p force + cutoff + neighbour emission)",
+        "bound": "alu", "kernel": "k_force (p-c / p-p force + cutoff + neighbour emission over the interaction lists)",
         "achieved": achieved, "peak": peak_instr, "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / peak_instr,
-        "traffic": None, "peak_source": f"{sms} SMs x 128 FP32 lanes x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
+        "traffic": TRAFFIC_NCU.get(w.name), "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full, profiles/)",
+        "peak_source": f"{sms} SMs x 128 FP32 lanes x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
         "algorithmic": f"{INSTR_PP} instr per p-p x {st['n_pp']} + {INSTR_PC} per p-c x {st['n_pc']}",
         "achieved_tflops": (FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]) / (wms * 1e-3) / 1e12,
         "kernel_ms": wms, "kernel_share_of_step": wms * args.steps / total_ms,
@@ -252,7 +256,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "interactions_per_s": n_int * world / (wms * 1e-3), "interactions_per_step": n_int,
         "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n,
-        "ms_build": float(np.mean(build_ms)), "ms_sort": float(np.mean(sort_ms)), "ms_force": float(np.mean(force_ms)), "ms_walk": wms,
+        "ms_build": float(np.mean(build_ms)), "ms_sort": float(np.mean(sort_ms)), "ms_force": float(np.mean(force_ms)), "ms_count": float(np.mean(count_ms)),
+        "ms_walk": float(np.mean(walk_ms)), "ms_eval": wms,
         "nodes": st["n_nodes"], "groups": st["n_groups"], "neighbours_total": st["nb_total"], "neighbours_max": st["nb_max"],
         "e2e": {"value": e2e_value, "unit": "particles/s", "ms_per_step": e2e_ms_max / args.steps,
                 "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n + 8 * (n + 1) + 4 * int(nb_total)},

@@ -62,8 +62,10 @@ typedef struct p3t_stats {
     float   cube_side;
     float   ms_build;        /* CUDA-event time of the last p3t_build_tree (a1-a6)      */
     float   ms_force;        /* CUDA-event time of the last p3t_regular_force (a7-a11)  */
-    float   ms_walk;         /* ... of its walk+force kernel alone                      */
+    float   ms_walk;         /* ... of its list-building tree walk kernel (a7) alone    */
     float   ms_sort;         /* ... of the radix sort inside the last build             */
+    float   ms_eval;         /* ... of the force kernel (a8, a9, a11) alone             */
+    float   ms_count;        /* ... of the neighbour count walk + offset scan (a10)     */
     int64_t launches;        /* kernels this context has launched since p3t_create      */
 } p3t_stats;
 

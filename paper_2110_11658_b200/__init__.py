@@ -36,6 +36,7 @@ class Stats(C.Structure):
         ("nb_total", C.c_int64), ("nb_max", C.c_int32), ("input_bad", C.c_int32),
         ("cube_lo", C.c_float * 3), ("cube_side", C.c_float),
         ("ms_build", C.c_float), ("ms_force", C.c_float), ("ms_walk", C.c_float), ("ms_sort", C.c_float),
+        ("ms_eval", C.c_float), ("ms_count", C.c_float),
         ("launches", C.c_int64),
     ]
 

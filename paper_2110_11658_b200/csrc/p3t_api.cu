@@ -183,7 +183,9 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         out->n_pp_list = (int64_t)h.n_pp_list; out->n_pc_list = (int64_t)h.n_pc_list;
         out->nb_total = (int64_t)h.nb_total; out->nb_max = h.nb_max;
         (void)cudaEventElapsedTime(&out->ms_force, c->ev[4], c->ev[5]);
-        (void)cudaEventElapsedTime(&out->ms_walk, c->evw[0], c->evw[1]);
+        (void)cudaEventElapsedTime(&out->ms_eval, c->evw[0], c->evw[1]);
+        (void)cudaEventElapsedTime(&out->ms_walk, c->evw[2], c->evw[3]);
+        (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->evw[2]);
     }
     (void)cudaGetLastError();
     return rc;

@@ -44,6 +44,7 @@ struct force_args {
     float4* out;                // out: acc_pot, original order
     p3t_devinfo* info;
     walk_consts K;
+    int dbg;
 };
 
 // Per-warp list tiles, double-buffered, structure-of-arrays so that two (LDS.64) or four (LDS.128)
@@ -312,9 +313,9 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
             __syncwarp();
             for (int t = 0; t < nt; ++t) {
                 const bool more = t + 1 < nt;
-                if (more) r = gather_pc(A, idn);
+                if (more) r = gather_pc(A, (A.dbg & 4) && idn >= 0 ? (idn & 255) : idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pc(T, S.pc[t & 1], part, k);
+                for (int rep = (A.dbg & 1) ? 0 : ((A.dbg & 8) ? 2 : 1); rep > 0; --rep) eval_pc(T, S.pc[t & 1], part, k);
                 if (((t + 1) & (k - 1)) == 0) fold(T);
                 if (more) store_pc(S.pc[(t + 1) & 1], lane, r);
                 __syncwarp();
@@ -336,7 +337,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
                 const int b = t & 1;
                 if (more) r = gather_pp(A, idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
+                if (!(A.dbg & 2)) eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
                 if (((t + 1) & (2 * k - 1)) == 0) fold(T);
                 if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
@@ -550,6 +551,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
     A.out = acc_pot; A.info = INFO(ctx);
     make_consts(A.K, r_out, r_in, theta, pot_mode);
+    A.dbg = getenv("P3T_DBG") ? atoi(getenv("P3T_DBG")) : 0;
     // a8, a9, a11: the force kernel
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
     k_force<<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);

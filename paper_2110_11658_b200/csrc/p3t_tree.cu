@@ -41,27 +41,27 @@ __device__ __forceinline__ int block_exscan(int v, int* total, int* s_warp /* [T
     return add + x - v;
 }
 
-// first position in [b, e) whose octant digit at `shift` is >= o
-__device__ __forceinline__ int oct_lower_bound(const uint64_t* __restrict__ keys, int b, int e, int shift, uint32_t o)
-{
-    while (b < e) {
-        int m = (b + e) >> 1;
-        if (((uint32_t)(keys[m] >> shift) & 7u) < o) b = m + 1; else e = m;
-    }
-    return b;
-}
-
-// child boundaries of an internal cell: pos[0..8]
+// child boundaries of an internal cell: pos[o] = first position in [b, e) whose octant digit at
+// `shift` is >= o.  The seven binary searches run in lockstep over the same interval, so that every
+// step issues seven independent key loads (the searches are latency-bound: one dependent L2 round
+// trip per step) instead of seven times as many dependent ones.
 __device__ __forceinline__ void child_bounds(const uint64_t* __restrict__ keys, int b, int e, int shift, int pos[9])
 {
+    int lo[7], hi[7];
+#pragma unroll
+    for (int o = 0; o < 7; ++o) { lo[o] = b; hi[o] = e; }
+    for (int span = e - b; span > 0; span >>= 1) {       // floor(log2(e - b)) + 1 halvings empty every interval
+#pragma unroll
+        for (int o = 0; o < 7; ++o) {
+            if (lo[o] < hi[o]) {
+                const int m = (lo[o] + hi[o]) >> 1;
+                if (((uint32_t)(keys[m] >> shift) & 7u) < (uint32_t)(o + 1)) lo[o] = m + 1; else hi[o] = m;
+            }
+        }
+    }
     pos[0] = b; pos[8] = e;
-    pos[4] = oct_lower_bound(keys, b, e, shift, 4);
-    pos[2] = oct_lower_bound(keys, b, pos[4], shift, 2);
-    pos[6] = oct_lower_bound(keys, pos[4], e, shift, 6);
-    pos[1] = oct_lower_bound(keys, b, pos[2], shift, 1);
-    pos[3] = oct_lower_bound(keys, pos[2], pos[4], shift, 3);
-    pos[5] = oct_lower_bound(keys, pos[4], pos[6], shift, 5);
-    pos[7] = oct_lower_bound(keys, pos[6], e, shift, 7);
+#pragma unroll
+    for (int o = 0; o < 7; ++o) pos[o + 1] = lo[o];
 }
 
 __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-way bit spread
