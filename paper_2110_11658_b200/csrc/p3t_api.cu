@@ -74,7 +74,7 @@ int p3t_destroy(p3t_ctx* c)
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
-                        &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp,
+                        &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill, &c->pcpool, &c->pppool, &c->glist,
                         &c->info, &c->stage_in, &c->stage_out };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
@@ -114,7 +114,8 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     RES(nlevel, C * 4); RES(nbegin, C * 4); RES(nend, C * 4); RES(nfirst, C * 4); RES(nnchild, C * 4);
     RES(m64, C * 80);
     RES(ncom, C * 16); RES(nlo, C * 16); RES(nhi, C * 16); RES(nq0, C * 16); RES(nq1, C * 8); RES(nlink, C * 8);
-    RES(scan_tmp, (size_t)c->coop_blocks_tree * 4 + 64);
+    RES(scan_tmp, (size_t)22 * ((N + 255) / 256) * 4 + 64); RES(pcl, N + 64); RES(plam, N + 64);
+    RES(nparent, C * 4); RES(nfc, C * 4); RES(ncount, C * 4); RES(gsum, ((N + 4095) / 4096 + 1) * 4);
     RES(gflag, N + 64); RES(gbegin, (N + 2) * 4); RES(gnpp, (N + 1) * 4); RES(gnpc, (N + 1) * 4);
 #undef RES
     const float4* pm = (const float4*)pos_mass;

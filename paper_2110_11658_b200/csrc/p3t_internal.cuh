@@ -56,7 +56,10 @@ struct p3t_ctx {
     p3t_buf nlevel, nbegin, nend, nfirst, nnchild;        // int32 per node
     p3t_buf m64;                     // double[10] per node: M, com[3], Q[6]
     p3t_buf ncom, nlo, nhi, nq0, nq1, nlink;              // walk SoA (see p3t_tree.cu)
-    p3t_buf scan_tmp;                // block sums of the cooperative kernels
+    p3t_buf scan_tmp;                // tree build: starters per level and block [22][blocks]
+    p3t_buf pcl, plam;               // int8 per particle: cl(i), lam(i) (p3t_tree.cu)
+    p3t_buf nparent, nfc, ncount;    // int32 per node: parent, first-child rank, arrival counter
+    p3t_buf gsum;                    // block sums of the group compaction
     p3t_buf gflag, gbegin;           // group start flags [n+1] / compacted starts [n_groups+1]
     p3t_buf gnpp, gnpc;              // per-group list lengths
     p3t_buf nbcount, nboff, nbidx;   // neighbour CSR: counts (sorted order) -> offsets (original order), indices
@@ -72,7 +75,6 @@ struct p3t_ctx {
     int nb_valid;
     cudaEvent_t ev[6];               // build begin/end, sort begin/end ... force begin/end, walk begin/end
     cudaEvent_t evw[4];
-    int coop_blocks_tree;            // co-resident grid of the tree kernel
     p3t_stats last;
     float r_out, r_in, theta;
     int64_t launches;                // kernels launched so far

@@ -1,67 +1,208 @@
 // p3t_tree.cu -- steps a4-a6: canonical octree topology, bottom-up monopole +
-// traceless quadrupole moments, target groups.  ONE cooperative kernel (grid = co-resident CTAs,
-// grid-wide barriers between levels) so that the whole stage is a single launch.
+// traceless quadrupole moments, target groups.
 // Rules: DESIGN.md R-S4 (topology), R-S5 (sibling-run groups), R-S6 (moments).
 // The paper gives no detail of this stage ("the BONSAI library").
+//
+// Topology without a level loop.  The canonical rule "a cell with more than NLEAF particles (and
+// level < B) is split" makes the existence of a cell a LOCAL property of the sorted key array:
+//   cl(i)  = number of leading octant digits that key[i-1] and key[i] share (cl(0) = -1):
+//            particle i begins a new cell at every level l > cl(i);
+//   a(i)   = number of leading digits that key[i] and key[i+NLEAF] share: the NLEAF+1 particles
+//            i .. i+NLEAF lie in one cell down to level a(i);
+//   P(i)   = max a(j), j in [i-NLEAF, i]  = the deepest level at which the cell of particle i
+//            holds more than NLEAF particles (-1: not even the root);
+//   lam(i) = min(P(i) + 1, B)             = the level of the leaf that holds particle i.
+// The cell (l, i) -- level l, first particle i -- exists iff cl(i) < l <= lam(i) (and (0, 0), the
+// root).  Numbering the cells by level, then by first particle, needs one multi-level prefix sum
+// over the particles: three streaming kernels instead of two grid-wide barriers per level.
+// Moments then climb the tree with one arrival counter per cell (the last child to arrive
+// computes its parent, combining the children in their fixed order), again without barriers.
 #include "p3t_internal.cuh"
-#include <cooperative_groups.h>
-namespace cg = cooperative_groups;
 
-#define TREE_THREADS 256
+#define TOPO_THREADS 256
+#define TOPO_WARPS   (TOPO_THREADS / 32)
+#define MAXLEV       22                  // levels 0 .. 21
+#define NODE_THREADS 128
 
 struct tree_args {
     const uint64_t* keys;      // sorted
     const float4* spm;         // sorted bodies
-    int n, B, nleaf, ncrit, node_cap;
-    int32_t *nlevel, *nbegin, *nend, *nfirst, *nnchild;
+    int n, B, nleaf, ncrit, node_cap, nblk;
+    int8_t *pcl, *plam;        // per particle: cl(i), lam(i)
+    int32_t* blksum;           // [MAXLEV][nblk] starters per level and block -> exclusive prefix
+    int32_t *nlevel, *nbegin, *nend, *nfirst, *nnchild, *nparent, *nfc, *ncount;
     double* m64;               // [node][10] = M, sum m x (3), Q about COM (6: xx yy zz xy xz yz)
     float4 *ncom, *nlo, *nhi, *nq0;
     float2* nq1;
     int2* nlink;
-    int32_t* scan_tmp;         // [gridDim]
     uint8_t* gflag;            // [n + 16] zeroed by the host side
     int32_t* gbegin;           // [n + 1]
+    int32_t* gsum;             // block sums of the group-flag compaction
     p3t_devinfo* info;
 };
 
-// exclusive scan of one int per thread over the block; returns the exclusive prefix, *total = block sum
-__device__ __forceinline__ int block_exscan(int v, int* total, int* s_warp /* [TREE_THREADS/32 + 1] */)
+// number of leading octant digits two keys of 3B bits share
+__device__ __forceinline__ int common_digits(uint64_t a, uint64_t b, int B)
 {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    int x = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-    __syncthreads();                       // protect s_warp from the previous use
-    if (lane == 31) s_warp[w] = x;
-    __syncthreads();
-    int add = 0, tot = 0;
-#pragma unroll
-    for (int k = 0; k < TREE_THREADS / 32; ++k) { int t = s_warp[k]; if (k < w) add += t; tot += t; }
-    *total = tot;
-    return add + x - v;
+    const uint64_t x = a ^ b;
+    if (x == 0) return B;
+    return (__clzll((long long)x) - (64 - 3 * B)) / 3;
 }
 
-// child boundaries of an internal cell: pos[o] = first position in [b, e) whose octant digit at
-// `shift` is >= o.  The seven binary searches run in lockstep over the same interval, so that every
-// step issues seven independent key loads (the searches are latency-bound: one dependent L2 round
-// trip per step) instead of seven times as many dependent ones.
-__device__ __forceinline__ void child_bounds(const uint64_t* __restrict__ keys, int b, int e, int shift, int pos[9])
+// ---------------- a4, pass 1: cl, lam, starters per level and block ----------------
+__global__ void __launch_bounds__(TOPO_THREADS) k_topo_count(tree_args A)
 {
-    int lo[7], hi[7];
-#pragma unroll
-    for (int o = 0; o < 7; ++o) { lo[o] = b; hi[o] = e; }
-    for (int span = e - b; span > 0; span >>= 1) {       // floor(log2(e - b)) + 1 halvings empty every interval
-#pragma unroll
-        for (int o = 0; o < 7; ++o) {
-            if (lo[o] < hi[o]) {
-                const int m = (lo[o] + hi[o]) >> 1;
-                if (((uint32_t)(keys[m] >> shift) & 7u) < (uint32_t)(o + 1)) lo[o] = m + 1; else hi[o] = m;
-            }
-        }
+    __shared__ uint64_t s_key[TOPO_THREADS + 2 * P3T_MAX_NCRIT + 1];
+    __shared__ int8_t   s_a[TOPO_THREADS + P3T_MAX_NCRIT];
+    __shared__ int      s_cnt[TOPO_WARPS][MAXLEV];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int t0 = blockIdx.x * TOPO_THREADS, L = A.nleaf;
+    // keys t0 - L - 1 .. t0 + 255 + L
+    for (int q = tid; q < TOPO_THREADS + 2 * L + 1; q += TOPO_THREADS) {
+        const int j = t0 - L - 1 + q;
+        s_key[q] = (j >= 0 && j < A.n) ? A.keys[j] : 0ull;
     }
-    pos[0] = b; pos[8] = e;
+    __syncthreads();
+    // a(j) for j = t0 - L .. t0 + 255
+    for (int q = tid; q < TOPO_THREADS + L; q += TOPO_THREADS) {
+        const int j = t0 - L + q;
+        int a = -1;
+        if (j >= 0 && j + L < A.n) a = common_digits(s_key[q + 1], s_key[q + 1 + L], A.B);
+        s_a[q] = (int8_t)a;
+    }
+    __syncthreads();
+    const int i = t0 + tid;
+    int cl = MAXLEV, lam = -1;                  // idle threads start nothing
+    if (i < A.n) {
+        cl = i == 0 ? -1 : common_digits(s_key[tid + L], s_key[tid + L + 1], A.B);
+        int P = -1;
+        for (int q = tid; q <= tid + L; ++q) P = max(P, (int)s_a[q]);
+        lam = min(P + 1, A.B);
+        A.pcl[i] = (int8_t)cl; A.plam[i] = (int8_t)lam;
+    }
+    for (int l = 1; l <= A.B; ++l) {
+        const uint32_t m = __ballot_sync(0xffffffffu, cl < l && l <= lam);
+        if (lane == 0) s_cnt[w][l] = __popc(m);
+    }
+    __syncthreads();
+    if (tid >= 1 && tid <= A.B) {
+        int t = 0;
 #pragma unroll
-    for (int o = 0; o < 7; ++o) pos[o + 1] = lo[o];
+        for (int k = 0; k < TOPO_WARPS; ++k) t += s_cnt[k][tid];
+        A.blksum[(size_t)tid * A.nblk + blockIdx.x] = t;
+    }
+}
+
+// ---------------- a4, pass 2: exclusive prefix over the blocks, one warp per level ----------------
+__global__ void __launch_bounds__(32 * MAXLEV) k_topo_scan(tree_args A)
+{
+    __shared__ int s_tot[MAXLEV];
+    const int lane = threadIdx.x & 31, l = threadIdx.x >> 5;
+    if (l >= 1 && l <= A.B) {
+        int32_t* row = A.blksum + (size_t)l * A.nblk;
+        int run = 0;
+        for (int b0 = 0; b0 < A.nblk; b0 += 32) {
+            const int b = b0 + lane;
+            const int v = b < A.nblk ? row[b] : 0;
+            int x = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+            if (b < A.nblk) row[b] = run + x - v;
+            run += __shfl_sync(0xffffffffu, x, 31);
+        }
+        if (lane == 0) s_tot[l] = run;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int off = 1, maxl = 0;                    // the root is cell 0
+        A.info->level_begin[0] = 0; A.info->level_begin[1] = 1;
+        for (int k = 1; k <= A.B; ++k) {
+            if (s_tot[k] > 0) maxl = k;
+            off += s_tot[k];
+            A.info->level_begin[k + 1 < 24 ? k + 1 : 23] = off;
+        }
+        for (int k = A.B + 2; k < 24; ++k) A.info->level_begin[k] = off;
+        A.info->n_nodes = off; A.info->max_level = maxl;
+        A.info->node_overflow = off > A.node_cap ? 1 : 0;
+    }
+}
+
+// ---------------- a4, pass 3: the cells ----------------
+__global__ void __launch_bounds__(TOPO_THREADS) k_topo_nodes(tree_args A)
+{
+    __shared__ int s_cnt[TOPO_WARPS][MAXLEV + 1];   // starters per warp and level, then exclusive over the warps
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const int i = blockIdx.x * TOPO_THREADS + tid;
+    int cl = MAXLEV, lam = -1;
+    if (i < A.n) { cl = A.pcl[i]; lam = A.plam[i]; }
+    const int* __restrict__ lb = A.info->level_begin;
+    if (A.info->node_overflow) return;
+    for (int l = 1; l <= A.B; ++l) {
+        const uint32_t m = __ballot_sync(0xffffffffu, cl < l && l <= lam);
+        if (lane == 0) s_cnt[w][l] = __popc(m);
+    }
+    if (lane == 0) s_cnt[w][0] = 0;
+    __syncthreads();
+    if (tid <= A.B) {
+        int run = tid == 0 ? 0 : A.blksum[(size_t)tid * A.nblk + blockIdx.x];
+#pragma unroll
+        for (int k = 0; k < TOPO_WARPS; ++k) { const int t = s_cnt[k][tid]; s_cnt[k][tid] = run; run += t; }
+    }
+    __syncthreads();
+    // rank of particle i among the starters of level l = s_cnt[w][l] + popc(ballot_l & lanes below);
+    // level 0 has the single starter (0, 0)
+    uint32_t m_prev = 0, m_cur = __ballot_sync(0xffffffffu, cl < 1 && 1 <= lam);
+    int r_prev = i > 0 ? 1 : 0;                  // starters of level 0 before i
+    if (i == 0) {                                // the root
+        A.nlevel[0] = 0; A.nbegin[0] = 0; A.nparent[0] = -1;
+        A.nfc[0] = 1;                            // rank 0 among the level-1 starters
+    }
+    for (int l = 1; l <= A.B; ++l) {
+        const uint32_t m_next = l < A.B ? __ballot_sync(0xffffffffu, cl < l + 1 && l + 1 <= lam) : 0u;
+        const int r_cur = s_cnt[w][l] + __popc(m_cur & lt_mask);
+        if (cl < l && l <= lam) {
+            const int id = lb[l] + r_cur;
+            const int r_next = l < A.B ? s_cnt[w][l + 1] + __popc(m_next & lt_mask) : 0;
+            A.nlevel[id] = l; A.nbegin[id] = i;
+            A.nfc[id] = lb[l + 1 < 24 ? l + 1 : 23] + r_next;
+            A.nparent[id] = lb[l - 1] + r_prev - (cl < l - 1 ? 0 : 1);
+        }
+        r_prev = r_cur; m_prev = m_cur; m_cur = m_next;
+    }
+    (void)m_prev;
+}
+
+// ---------------- a4, pass 4: ranges and child links ----------------
+// Children tile their parent: the range of a cell ends where its next sibling begins, and the last
+// child ends where its parent ends (climb until a cell has a next sibling).  The children of a cell
+// are numbered consecutively; their number is the distance to the first child of the next cell of
+// the same level.
+__global__ void __launch_bounds__(NODE_THREADS) k_topo_link(tree_args A)
+{
+    const int nn = A.info->n_nodes;
+    const int k = blockIdx.x * NODE_THREADS + threadIdx.x;
+    const int* __restrict__ lb = A.info->level_begin;
+    int leaf = 0;
+    if (k < nn && !A.info->node_overflow) {
+        const int lev = A.nlevel[k];
+        int end = A.n;
+        for (int w = k, l = lev; l > 0; --l) {
+            const int v = w + 1;
+            const int p = A.nparent[w];
+            if (v < lb[l + 1] && A.nparent[v] == p) { end = A.nbegin[v]; break; }
+            w = p;
+        }
+        A.nend[k] = end;
+        const int fc = A.nfc[k];
+        const int fc_next = k + 1 < lb[lev + 1] ? A.nfc[k + 1] : lb[lev + 2 < 24 ? lev + 2 : 23];
+        const int nc = lev < A.B ? fc_next - fc : 0;
+        A.nnchild[k] = nc; A.nfirst[k] = nc > 0 ? fc : -1;
+        A.ncount[k] = 0;
+        leaf = nc == 0;
+    }
+    const int tot = __syncthreads_count(leaf);
+    if (threadIdx.x == 0 && tot) atomicAdd(&A.info->n_leaves, tot);
 }
 
 __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-way bit spread
@@ -103,89 +244,16 @@ __device__ void store_node(const tree_args& A, int k, int level, int b, int e, i
     A.nlink[k] = nchild > 0 ? make_int2(first, nchild) : make_int2(b, -(e - b));
 }
 
-__global__ void __launch_bounds__(TREE_THREADS) k_tree(tree_args A)
+// ---------------- a5 moments (R-S6), fp64 ----------------
+// One thread per cell.  A leaf sums its particles, then climbs: every cell counts the children that
+// have finished; the thread that brings the count to n_child combines the children (in child order,
+// whatever the order of arrival: the result is bit-reproducible) and goes on to the parent.
+__global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
 {
-    cg::grid_group grid = cg::this_grid();
-    __shared__ int s_warp[TREE_THREADS / 32 + 1];
-    __shared__ int s_run;
-    const int nb = gridDim.x, bid = blockIdx.x, tid = threadIdx.x;
-    const uint64_t* __restrict__ keys = A.keys;
-
-    // ---------------- a4 topology, level by level (R-S4) ----------------
-    if (bid == 0 && tid == 0) {
-        A.nlevel[0] = 0; A.nbegin[0] = 0; A.nend[0] = A.n;
-        A.info->level_begin[0] = 0; A.info->level_begin[1] = 1;
-    }
-    grid.sync();
-    int lb = 0, le = 1, n_leaves = 0, max_level = 0, overflow = 0;
-    for (int lev = 0; lev <= A.B; ++lev) {
-        const int cnt = le - lb;
-        const int per = (cnt + nb - 1) / nb;
-        const int cb = min(le, lb + bid * per), ce = min(le, cb + per);
-        const int shift = 3 * (A.B - lev - 1);
-        // phase 1: child counts
-        int bsum = 0;
-        for (int k0 = cb; k0 < ce; k0 += TREE_THREADS) {
-            int k = k0 + tid, c = 0;
-            if (k < ce) {
-                int b = A.nbegin[k], e = A.nend[k];
-                if (e - b > A.nleaf && lev < A.B) {
-                    int pos[9];
-                    child_bounds(keys, b, e, shift, pos);
-#pragma unroll
-                    for (int o = 0; o < 8; ++o) c += pos[o + 1] > pos[o];
-                }
-                A.nnchild[k] = c;
-            }
-            bsum += c;
-        }
-        {
-            int tot; (void)block_exscan(bsum, &tot, s_warp);
-            if (tid == 0) A.scan_tmp[bid] = tot;
-        }
-        grid.sync();
-        // phase 2: numbering and child records
-        int before = 0, total = 0;
-        for (int k = tid; k < nb; k += TREE_THREADS) { int t = A.scan_tmp[k]; total += t; if (k < bid) before += t; }
-        { int t2; (void)block_exscan(before, &t2, s_warp); before = t2; }
-        { int t2; (void)block_exscan(total, &t2, s_warp); total = t2; }
-        if (le + total > A.node_cap) { overflow = 1; total = 0; }
-        int run = le + before;
-        for (int k0 = cb; k0 < ce && total > 0; k0 += TREE_THREADS) {
-            int k = k0 + tid;
-            int c = k < ce ? A.nnchild[k] : 0, tot;
-            int first = run + block_exscan(c, &tot, s_warp);
-            run += tot;
-            if (k < ce) {
-                if (c > 0) {
-                    int b = A.nbegin[k], e = A.nend[k], pos[9];
-                    child_bounds(keys, b, e, shift, pos);
-                    int w = first;
-#pragma unroll
-                    for (int o = 0; o < 8; ++o)
-                        if (pos[o + 1] > pos[o]) { A.nlevel[w] = lev + 1; A.nbegin[w] = pos[o]; A.nend[w] = pos[o + 1]; ++w; }
-                    A.nfirst[k] = first;
-                } else A.nfirst[k] = -1;
-            }
-        }
-        if (total == 0) {     // every cell of this level is a leaf (or capacity hit)
-            for (int k = cb + tid; k < ce; k += TREE_THREADS) A.nfirst[k] = -1;
-        }
-        if (bid == 0 && tid == 0) A.info->level_begin[lev + 2 < 24 ? lev + 2 : 23] = le + total;
-        max_level = lev;
-        grid.sync();
-        lb = le; le = le + total;
-        if (total == 0) break;
-    }
-    const int nn = le;
-    if (bid == 0 && tid == 0) {
-        A.info->n_nodes = nn; A.info->max_level = max_level; A.info->node_overflow = overflow;
-    }
-
-    // ---------------- a5 moments (R-S6): leaves from their particles, fp64 ----------------
-    for (int k = bid * TREE_THREADS + tid; k < nn; k += nb * TREE_THREADS) {
-        if (A.nnchild[k] != 0) continue;
-        ++n_leaves;
+    const int nn = A.info->n_nodes;
+    int k = blockIdx.x * NODE_THREADS + threadIdx.x;
+    if (k >= nn || A.info->node_overflow || A.nnchild[k] != 0) return;
+    {
         const int b = A.nbegin[k], e = A.nend[k];
         double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
         float4 p0 = A.spm[b];
@@ -208,129 +276,170 @@ __global__ void __launch_bounds__(TREE_THREADS) k_tree(tree_args A)
         }
         store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, Q, clo, chi);
     }
-    {   // leaf count
-        int tot; (void)block_exscan(n_leaves, &tot, s_warp);
-        if (tid == 0 && tot) atomicAdd(&A.info->n_leaves, tot);
-    }
-    grid.sync();
-    // internal cells bottom-up: parallel-axis combination of the children, fp64
-    for (int lev = max_level - 1; lev >= 0; --lev) {
-        const int l0 = A.info->level_begin[lev], l1 = A.info->level_begin[lev + 1];
-        for (int k = l0 + bid * TREE_THREADS + tid; k < l1; k += nb * TREE_THREADS) {
-            const int nc = A.nnchild[k];
-            if (nc == 0) continue;
-            const int fc = A.nfirst[k];
-            double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
-            float clo[3] = { INFINITY, INFINITY, INFINITY }, chi[3] = { -INFINITY, -INFINITY, -INFINITY };
-            for (int c = fc; c < fc + nc; ++c) {
-                const double* m = A.m64 + (size_t)c * 10;
-                M += m[0]; s[0] += m[1]; s[1] += m[2]; s[2] += m[3];
-                float4 lo = A.nlo[c], hi = A.nhi[c];
-                clo[0] = fminf(clo[0], lo.x); clo[1] = fminf(clo[1], lo.y); clo[2] = fminf(clo[2], lo.z);
-                chi[0] = fmaxf(chi[0], hi.x); chi[1] = fmaxf(chi[1], hi.y); chi[2] = fmaxf(chi[2], hi.z);
-            }
-            const double cm[3] = { s[0] / M, s[1] / M, s[2] / M };
-            double Q[6] = { 0, 0, 0, 0, 0, 0 };
-            for (int c = fc; c < fc + nc; ++c) {
-                const double* m = A.m64 + (size_t)c * 10;
-                const double Mc = m[0];
-                const double dx = m[1] / Mc - cm[0], dy = m[2] / Mc - cm[1], dz = m[3] / Mc - cm[2];
-                const double d2 = dx * dx + dy * dy + dz * dz;
-                Q[0] += m[4] + Mc * (3 * dx * dx - d2); Q[1] += m[5] + Mc * (3 * dy * dy - d2); Q[2] += m[6] + Mc * (3 * dz * dz - d2);
-                Q[3] += m[7] + Mc * 3 * dx * dy; Q[4] += m[8] + Mc * 3 * dx * dz; Q[5] += m[9] + Mc * 3 * dy * dz;
-            }
-            store_node(A, k, lev, A.nbegin[k], A.nend[k], fc, nc, M, s, Q, clo, chi);
-        }
-        grid.sync();
-    }
-
-    // ---------------- a6 groups (R-S5 sibling runs): flag every group start ----------------
-    if (bid == 0 && tid == 0 && A.n <= A.ncrit) A.gflag[0] = 1;
-    for (int k = bid * TREE_THREADS + tid; k < nn; k += nb * TREE_THREADS) {
-        const int b = A.nbegin[k], e = A.nend[k];
-        if (e - b <= A.ncrit) continue;
-        const int nc = A.nnchild[k];
-        if (nc == 0) {                                 // over-full leaf at the deepest level
-            for (int s = b; s < e; s += A.ncrit) A.gflag[s] = 1;
-            continue;
-        }
-        const int fc = A.nfirst[k];
-        int run = -1;                                  // size of the open run, -1 = none
+    for (;;) {
+        const int p = A.nparent[k];
+        if (p < 0) break;
+        __threadfence();                                           // this cell's data before the count
+        if (atomicAdd(&A.ncount[p], 1) + 1 < A.nnchild[p]) break;  // a later sibling will do the parent
+        __threadfence();
+        // internal cell: parallel-axis combination of the children (read past L1: other SMs wrote them)
+        k = p;
+        const int nc = A.nnchild[k], fc = A.nfirst[k];
+        double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
+        float clo[3] = { INFINITY, INFINITY, INFINITY }, chi[3] = { -INFINITY, -INFINITY, -INFINITY };
         for (int c = fc; c < fc + nc; ++c) {
-            const int cb2 = A.nbegin[c], cnt = A.nend[c] - cb2;
-            if (cnt > A.ncrit) run = -1;               // that child makes its own groups
-            else if (run >= 0 && run + cnt <= A.ncrit) run += cnt;
-            else { A.gflag[cb2] = 1; run = cnt; }
+            const double* m = A.m64 + (size_t)c * 10;
+            M += __ldcg(m); s[0] += __ldcg(m + 1); s[1] += __ldcg(m + 2); s[2] += __ldcg(m + 3);
+            float4 lo = __ldcg(&A.nlo[c]), hi = __ldcg(&A.nhi[c]);
+            clo[0] = fminf(clo[0], lo.x); clo[1] = fminf(clo[1], lo.y); clo[2] = fminf(clo[2], lo.z);
+            chi[0] = fmaxf(chi[0], hi.x); chi[1] = fmaxf(chi[1], hi.y); chi[2] = fmaxf(chi[2], hi.z);
         }
+        const double cm[3] = { s[0] / M, s[1] / M, s[2] / M };
+        double Q[6] = { 0, 0, 0, 0, 0, 0 };
+        for (int c = fc; c < fc + nc; ++c) {
+            const double* m = A.m64 + (size_t)c * 10;
+            const double Mc = __ldcg(m);
+            const double dx = __ldcg(m + 1) / Mc - cm[0], dy = __ldcg(m + 2) / Mc - cm[1], dz = __ldcg(m + 3) / Mc - cm[2];
+            const double d2 = dx * dx + dy * dy + dz * dz;
+            Q[0] += __ldcg(m + 4) + Mc * (3 * dx * dx - d2); Q[1] += __ldcg(m + 5) + Mc * (3 * dy * dy - d2); Q[2] += __ldcg(m + 6) + Mc * (3 * dz * dz - d2);
+            Q[3] += __ldcg(m + 7) + Mc * 3 * dx * dy; Q[4] += __ldcg(m + 8) + Mc * 3 * dx * dz; Q[5] += __ldcg(m + 9) + Mc * 3 * dy * dz;
+        }
+        store_node(A, k, A.nlevel[k], A.nbegin[k], A.nend[k], fc, nc, M, s, Q, clo, chi);
     }
-    grid.sync();
-    // compaction of the flags into ascending group starts
-    {
-        const int n16 = (A.n + 15) / 16;               // 16 flags per thread step
-        const int per = (n16 + nb - 1) / nb;
-        const int cb = min(n16, bid * per), ce = min(n16, cb + per);
-        const uint4* f4 = (const uint4*)A.gflag;
-        int bsum = 0;
-        for (int q = cb + tid; q < ce; q += TREE_THREADS) {
-            uint4 v = f4[q];
-            bsum += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
-        }
-        int tot; (void)block_exscan(bsum, &tot, s_warp);
-        if (tid == 0) A.scan_tmp[bid] = tot;
-        grid.sync();
-        int before = 0, total = 0;
-        for (int k = tid; k < nb; k += TREE_THREADS) { int t = A.scan_tmp[k]; total += t; if (k < bid) before += t; }
-        { int t2; (void)block_exscan(before, &t2, s_warp); before = t2; }
-        { int t2; (void)block_exscan(total, &t2, s_warp); total = t2; }
-        if (tid == 0) s_run = before;
-        __syncthreads();
-        for (int q0 = cb; q0 < ce; q0 += TREE_THREADS) {
-            int q = q0 + tid, c = 0;
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (q < ce) { v = f4[q]; c = __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
-            int t3, ex = block_exscan(c, &t3, s_warp);
-            int w = s_run + ex;
-            if (c) {
-                const uint32_t words[4] = { v.x, v.y, v.z, v.w };
+}
+
+// ---------------- a6 groups (R-S5 sibling runs): flag every group start, then compact ----------------
+__global__ void __launch_bounds__(NODE_THREADS) k_group_flags(tree_args A)
+{
+    const int nn = A.info->n_nodes;
+    const int k = blockIdx.x * NODE_THREADS + threadIdx.x;
+    if (k == 0 && A.n <= A.ncrit) A.gflag[0] = 1;
+    if (k >= nn || A.info->node_overflow) return;
+    const int b = A.nbegin[k], e = A.nend[k];
+    if (e - b <= A.ncrit) return;
+    const int nc = A.nnchild[k];
+    if (nc == 0) {                                 // over-full leaf at the deepest level
+        for (int s = b; s < e; s += A.ncrit) A.gflag[s] = 1;
+        return;
+    }
+    const int fc = A.nfirst[k];
+    int run = -1;                                  // size of the open run, -1 = none
+    for (int c = fc; c < fc + nc; ++c) {
+        const int cb2 = A.nbegin[c], cnt = A.nend[c] - cb2;
+        if (cnt > A.ncrit) run = -1;               // that child makes its own groups
+        else if (run >= 0 && run + cnt <= A.ncrit) run += cnt;
+        else { A.gflag[cb2] = 1; run = cnt; }
+    }
+}
+
+#define GC_THREADS 256
+__device__ __forceinline__ int flags16(const uint4 v) { return __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
+
+__global__ void __launch_bounds__(GC_THREADS) k_group_count(tree_args A)
+{
+    const int n16 = (A.n + 15) / 16;
+    const int q = blockIdx.x * GC_THREADS + threadIdx.x;
+    const int c = q < n16 ? flags16(((const uint4*)A.gflag)[q]) : 0;
+    const int tot = c;
+    // block sum by warp shuffles
+    __shared__ int s_w[GC_THREADS / 32];
+    int x = tot;
 #pragma unroll
-                for (int j = 0; j < 16; ++j)
-                    if ((words[j >> 2] >> (8 * (j & 3))) & 0xffu) A.gbegin[w++] = q * 16 + j;
-            }
-            __syncthreads();
-            if (tid == 0) s_run += t3;
-            __syncthreads();
-        }
-        if (bid == 0 && tid == 0) { A.gbegin[total] = A.n; A.info->n_groups = total; }
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+#pragma unroll
+        for (int k = 0; k < GC_THREADS / 32; ++k) t += s_w[k];
+        A.gsum[blockIdx.x] = t;
+    }
+}
+
+__global__ void __launch_bounds__(1024) k_group_scan(tree_args A, int nb)
+{
+    __shared__ int s_w[32];
+    __shared__ int s_run;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_run = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nb; b0 += 1024) {
+        const int b = b0 + threadIdx.x;
+        const int v = b < nb ? A.gsum[b] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) s_w[w] = x;
+        __syncthreads();
+        int add = s_run, tot = 0;
+        for (int k = 0; k < 32; ++k) { const int t = s_w[k]; if (k < w) add += t; tot += t; }
+        if (b < nb) A.gsum[b] = add + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) s_run += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { A.gbegin[s_run] = A.n; A.info->n_groups = s_run; }
+}
+
+__global__ void __launch_bounds__(GC_THREADS) k_group_compact(tree_args A)
+{
+    __shared__ int s_w[GC_THREADS / 32];
+    const int n16 = (A.n + 15) / 16;
+    const int q = blockIdx.x * GC_THREADS + threadIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint4 v = make_uint4(0, 0, 0, 0);
+    if (q < n16) v = ((const uint4*)A.gflag)[q];
+    const int c = flags16(v);
+    int x = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) s_w[w] = x;
+    __syncthreads();
+    int out = A.gsum[blockIdx.x] + x - c;
+    for (int k = 0; k < w; ++k) out += s_w[k];
+    if (c) {
+        const uint32_t words[4] = { v.x, v.y, v.z, v.w };
+#pragma unroll
+        for (int j = 0; j < 16; ++j)
+            if ((words[j >> 2] >> (8 * (j & 3))) & 0xffu) A.gbegin[out++] = q * 16 + j;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-int p3t_tree_init(p3t_ctx* ctx)
-{
-    int per_sm = 0;
-    P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tree, TREE_THREADS, 0));
-    if (per_sm < 1) per_sm = 1;
-    if (per_sm > 4) per_sm = 4;
-    ctx->coop_blocks_tree = per_sm * ctx->num_sms;
-    return P3T_OK;
-}
+int p3t_tree_init(p3t_ctx* ctx) { (void)ctx; return P3T_OK; }
 
 int p3t_launch_tree(p3t_ctx* ctx)
 {
     tree_args A;
+    const int n = (int)ctx->n;
     A.keys = P<uint64_t>(ctx->keys[0]); A.spm = P<float4>(ctx->spm);
-    A.n = (int)ctx->n; A.B = ctx->bits; A.nleaf = ctx->nleaf; A.ncrit = ctx->ncrit; A.node_cap = (int)ctx->node_cap;
+    A.n = n; A.B = ctx->bits; A.nleaf = ctx->nleaf; A.ncrit = ctx->ncrit; A.node_cap = (int)ctx->node_cap;
+    A.nblk = (n + TOPO_THREADS - 1) / TOPO_THREADS;
+    A.pcl = P<int8_t>(ctx->pcl); A.plam = P<int8_t>(ctx->plam); A.blksum = P<int32_t>(ctx->scan_tmp);
     A.nlevel = P<int32_t>(ctx->nlevel); A.nbegin = P<int32_t>(ctx->nbegin); A.nend = P<int32_t>(ctx->nend);
     A.nfirst = P<int32_t>(ctx->nfirst); A.nnchild = P<int32_t>(ctx->nnchild);
+    A.nparent = P<int32_t>(ctx->nparent); A.nfc = P<int32_t>(ctx->nfc); A.ncount = P<int32_t>(ctx->ncount);
     A.m64 = P<double>(ctx->m64);
     A.ncom = P<float4>(ctx->ncom); A.nlo = P<float4>(ctx->nlo); A.nhi = P<float4>(ctx->nhi);
     A.nq0 = P<float4>(ctx->nq0); A.nq1 = P<float2>(ctx->nq1); A.nlink = P<int2>(ctx->nlink);
-    A.scan_tmp = P<int32_t>(ctx->scan_tmp);
     A.gflag = P<uint8_t>(ctx->gflag); A.gbegin = P<int32_t>(ctx->gbegin);
+    A.gsum = P<int32_t>(ctx->gsum);
     A.info = INFO(ctx);
-    P3T_CUDA(ctx, cudaMemsetAsync(ctx->gflag.p, 0, (size_t)ctx->n + 32, ctx->stream));
-    void* args[] = { &A };
-    P3T_CUDA(ctx, cudaLaunchCooperativeKernel((void*)k_tree, dim3(ctx->coop_blocks_tree), dim3(TREE_THREADS), args, 0, ctx->stream));
-    ctx->launches += 1;
+    cudaStream_t st = ctx->stream;
+    P3T_CUDA(ctx, cudaMemsetAsync(ctx->gflag.p, 0, (size_t)n + 32, st));
+    k_topo_count<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
+    k_topo_scan<<<1, 32 * MAXLEV, 0, st>>>(A);
+    k_topo_nodes<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
+    // one thread per cell: the cell count is only known on the device; the bound of p3t_build_tree
+    // (node_cap) sizes the grids, threads beyond n_nodes return at once
+    const int nodes_grid = (int)(((long long)ctx->node_cap + NODE_THREADS - 1) / NODE_THREADS);
+    k_topo_link<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
+    k_moments<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
+    k_group_flags<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
+    const int n16 = (n + 15) / 16, gcb = (n16 + GC_THREADS - 1) / GC_THREADS;
+    k_group_count<<<gcb, GC_THREADS, 0, st>>>(A);
+    k_group_scan<<<1, 1024, 0, st>>>(A, gcb);
+    k_group_compact<<<gcb, GC_THREADS, 0, st>>>(A);
+    P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 9;
     return P3T_OK;
 }
