@@ -5,8 +5,8 @@
 //   F_R,i = sum_j m_j W(x_ij) (x_j - x_i) / r_ij^3,  W = 1 - K,  x = (r - r_in)/(r_out - r_in)
 //   (eq. 1, 3, 4, 6, 8-10; attractive sign: DESIGN.md R1)
 //
-// One warp evaluates one target group (<= 64 particles, one or two target slots per lane) against
-// the interaction lists that k_walk<WALK_LISTS> left in HBM.  32 list entries at a time are gathered
+// One warp evaluates one work item (up to 32 targets of one group, see `target` below) against the
+// group's interaction lists that k_walk<WALK_LISTS> left in HBM.  32 list entries at a time are gathered
 // (node / particle data, L2-resident) into a double-buffered structure-of-arrays tile in shared
 // memory while the previous tile is being evaluated, so the FP32 pipe never waits for the walk.
 // Rules: DESIGN.md R-S8 (evaluation), R-S9 (accumulation), R10 (neighbour predicate, bit-specified).
@@ -44,7 +44,6 @@ struct force_args {
     float4* out;                // out: acc_pot, original order
     p3t_devinfo* info;
     walk_consts K;
-    int dbg;
 };
 
 // Per-warp list tiles, double-buffered, structure-of-arrays so that two (LDS.64) or four (LDS.128)
@@ -313,9 +312,9 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
             __syncwarp();
             for (int t = 0; t < nt; ++t) {
                 const bool more = t + 1 < nt;
-                if (more) r = gather_pc(A, (A.dbg & 4) && idn >= 0 ? (idn & 255) : idn);
+                if (more) r = gather_pc(A, idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                for (int rep = (A.dbg & 1) ? 0 : ((A.dbg & 8) ? 2 : 1); rep > 0; --rep) eval_pc(T, S.pc[t & 1], part, k);
+                eval_pc(T, S.pc[t & 1], part, k);
                 if (((t + 1) & (k - 1)) == 0) fold(T);
                 if (more) store_pc(S.pc[(t + 1) & 1], lane, r);
                 __syncwarp();
@@ -337,7 +336,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
                 const int b = t & 1;
                 if (more) r = gather_pp(A, idn);
                 idn = load_id(ids, (t + 2) * TILE + lane, n);
-                if (!(A.dbg & 2)) eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
+                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
                 if (((t + 1) & (2 * k - 1)) == 0) fold(T);
                 if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
@@ -551,7 +550,6 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
     A.out = acc_pot; A.info = INFO(ctx);
     make_consts(A.K, r_out, r_in, theta, pot_mode);
-    A.dbg = getenv("P3T_DBG") ? atoi(getenv("P3T_DBG")) : 0;
     // a8, a9, a11: the force kernel
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
     k_force<<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
