@@ -93,8 +93,8 @@ __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float
     return -W * rinv - K.k140 * integral;
 }
 
-// One work item = up to 32 targets of one group (a group of 33..64 particles makes two items that
-// stream the same lists).  An item with c <= 16 targets gives every target k = 2, 4 or 8 lanes
+// One work item = up to 32 targets of one group (see k_force; the items of a group stream the same
+// lists).  An item with c <= 16 targets gives every target k = 2, 4 or 8 lanes
 // ("parts"): lane = target * k + part, and part p evaluates the 4-entry blocks p, p + k, ... of every
 // tile, so that a half-empty item costs half the time instead of idling half the lanes.  The parts
 // of a target are summed by shuffles at the end.
@@ -186,15 +186,16 @@ __device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 
 }
 
 // R10 + eq. 6, near zone (d2 < r_out^2): neighbour emission and the cutoff-weighted pair term.
-// Scalar pass over this lane's blocks of a tile, run only by warps whose tile came within r_out of
-// one of their targets (about one tile in eight).  nbrow[slot] counts the entries already written
+// Scalar pass over the 4-entry blocks in which the far pass saw this lane's target within r_out
+// (bit mask), run only by warps that have such a block in the tile (about one tile in eight).  nbrow[slot] counts the entries already written
 // to the target's CSR row (shared by the parts of a target).
-__device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
+__device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE], const int* ppj, uint32_t nearblocks,
                                              long long rowbase, int* nbrow, const force_args& A)
 {
     const walk_consts& K = A.K;
-#pragma unroll 1
-    for (int e0 = 4 * part; e0 < TILE; e0 += 4 * k) {
+    while (nearblocks) {
+        const int e0 = (__ffs(nearblocks) - 1) << 2;
+        nearblocks &= nearblocks - 1;
 #pragma unroll 1
         for (int e = e0; e < e0 + 4; ++e) {
             const float dx = __fsub_rn(pp[0][e], T.x), dy = __fsub_rn(pp[1][e], T.y), dz = __fsub_rn(pp[2][e], T.z);
@@ -225,17 +226,18 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
 __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
                                         long long rowbase, int* nbrow, const force_args& A)
 {
-    float dmin = INFINITY;
+    uint32_t nearblocks = 0;                     // bit b: this lane's target came within r_out of block b
 #pragma unroll 1
     for (int e = 4 * part; e < TILE; e += 4 * k) {
         ulonglong2 v[4];
 #pragma unroll
         for (int r = 0; r < 4; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pp[r][e]);
-        dmin = pp_far_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, dmin);
+        float dmin = pp_far_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, INFINITY);
         dmin = pp_far_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
+        if (dmin < A.K.rout2) nearblocks |= 1u << (e >> 2);
     }
-    if (!__any_sync(0xffffffffu, dmin < A.K.rout2)) return;
-    pp_near_pass(T, pp, ppj, part, k, rowbase, nbrow, A);
+    if (!__any_sync(0xffffffffu, nearblocks != 0)) return;
+    pp_near_pass(T, pp, ppj, nearblocks, rowbase, nbrow, A);
 }
 
 // Software pipeline of the list stream: the ids of tile t+2 and the node / particle data of tile
@@ -353,23 +355,35 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     if (v && part == 0) A.out[orig] = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
 }
 
-// work item 2g + s: slot s (32 targets) of group g; dynamic scheduling, persistent grid
+// Work items: the c <= 64 targets of a group are cut into chunks of 32, 32, 16 and c mod 16 targets,
+// which run with k = 1, 1, 2 and 2 / 4 / 8 lanes per target: every chunk but the last fills its
+// warp, and a chunk costs list length / k.  Persistent grid, dynamic
+// scheduling; the chunks are handed out in four passes, k = 1 first and k = 8 last, so that the
+// kernel ends on its cheapest items and the warps finish together.
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(force_args A)
 {
     __shared__ tile_smem smem[FORCE_WARPS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     tile_smem& S = smem[w];
-    const int nitems = 2 * A.info->n_groups;
+    const int ng = A.info->n_groups;
+    // cursor ranges of the passes: [0, 2 ng) chunks 0-1 (k = 1), [2 ng, 3 ng) chunk 2 (k = 2), [3 ng, 4 ng) chunk 3 (the rest)
     for (;;) {
-        int it = 0;
-        if (lane == 0) it = (int)atomicAdd(&A.info->group_cursor3, 1u);
-        it = __shfl_sync(0xffffffffu, it, 0);
-        if (it >= nitems) break;
-        const int g = it >> 1, s = it & 1;
-        const int gb = A.gbegin[g], ge = A.gbegin[g + 1];
-        const int tb = gb + 32 * s;
-        if (tb >= ge) continue;
-        force_item(A, S, g, tb, min(ge, tb + 32));
+        int c = 0;
+        if (lane == 0) c = (int)atomicAdd(&A.info->group_cursor3, 1u);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= 4 * ng) break;
+        int g, j;
+        if (c < 2 * ng)      { g = c >> 1; j = c & 1; }
+        else if (c < 3 * ng) { g = c - 2 * ng; j = 2; }
+        else                 { g = c - 3 * ng; j = 3; }
+        const int gb = A.gbegin[g], n = A.gbegin[g + 1] - gb;
+        const int full = n >> 5, r = n & 31;
+        int tb, len;
+        if (j < 2)       { tb = 32 * j;                len = j < full ? 32 : 0; }
+        else if (j == 2) { tb = 32 * full;             len = r & 16; }
+        else             { tb = 32 * full + (r & 16);  len = r & 15; }
+        if (len == 0) continue;
+        force_item(A, S, g, gb + tb, gb + tb + len);
         __syncwarp();
     }
 }
