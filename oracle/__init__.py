@@ -51,6 +51,8 @@ def lib() -> C.CDLL:
         _lib.p3t_o_psi.restype = d; _lib.p3t_o_psi.argtypes = [d, d, d]
         _lib.p3t_o_direct.restype = i64
         _lib.p3t_o_direct.argtypes = [i64, vp, d, d, i64, vp, vp, vp, vp, vp]
+        _lib.p3t_o_irregular.restype = i64
+        _lib.p3t_o_irregular.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_neighbours.restype = i64
         _lib.p3t_o_neighbours.argtypes = [i64, vp, f32, C.c_int, i64, vp, vp, vp]
         _lib.p3t_o_tree_build.restype = vp
@@ -117,6 +119,16 @@ def direct(pos_mass, r_out: float, r_in: float, targets=None):
     ar = np.zeros((nt, 3)); ai = np.zeros((nt, 3)); pr = np.zeros(nt); pn = np.zeros(nt)
     co = lib().p3t_o_direct(n, _p(pm), float(r_out), float(r_in), nt, _p(tg), _p(ar), _p(pr), _p(ai), _p(pn))
     return dict(acc_reg=ar, phi_reg=pr, acc_irr=ai, phi_newt=pn, coincident=int(co))
+
+
+def irregular(pos_mass, vel, r_out: float, r_in: float, targets=None):
+    """Irregular acceleration, jerk, potential over the neighbour sphere (eq. 1, 2, 5, 7); fp64 arrays."""
+    pm = _pm(pos_mass); v = _pm(vel)
+    t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
+    nt = pm.shape[0] if t is None else t.shape[0]
+    acc = np.zeros((nt, 3)); jerk = np.zeros((nt, 3)); phi = np.zeros(nt); ab = np.zeros(nt)
+    coinc = lib().p3t_o_irregular(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(acc), _p(jerk), _p(phi), _p(ab))
+    return dict(acc_irr=acc, jerk_irr=jerk, phi_irr=phi, abs_jerk=ab, coincident=int(coinc))
 
 
 def neighbours(pos_mass, r_out: float, targets=None, fp32_predicate: bool = True):

@@ -158,3 +158,60 @@ int64_t p3t_o_neighbours(int64_t n, const float* pm, float r_out, int fp32_predi
     free(off);
     return total;
 }
+
+/* eq. 1, 2, 5, 7: irregular acceleration and its time derivative (jerk) of
+ * nt targets, summed over j != i with r_ij < r_out (the neighbour sphere; K = 0 beyond it).
+ * With d = x_j - x_i, v = xdot_j - xdot_i (readings R1: attraction; eq. 5 with the same sign
+ * convention), r = |d|, x = (r - r_in)/(r_out - r_in), K = 1 - W:
+ *     F_I    = sum m_j K d / r^3                                                   (eq. 1)
+ *     Fdot_I = sum m_j [ K ( v / r^3 - 3 (d.v) d / r^5 ) + Kdot d / r^3 ]          (eq. 2)
+ *     Kdot   = dK/dt = -W'(x) xdot,   xdot = (d.v) / (r (r_out - r_in)),
+ *     W'(x)  = 140 x^3 (1-x)^3 = the polynomial of eq. 7.
+ * Reading R2: eq. 2 as printed has K multiplying only the first term and eq. 7 gives
+ * K' the opposite sign; Fdot_I here is the exact time derivative of eq. 1 (pinned by finite
+ * differences in tests/test_oracle_irregular.py).  Coincident pairs (r = 0, reading R8) are skipped
+ * (a KS pair in the host code) and counted in the return value.
+ * vel: n x 4 fp32 (vx, vy, vz, unused).  Outputs (any may be NULL): acc_irr[3 nt], jerk_irr[3 nt],
+ * phi_irr[nt] = sum m_j (-1/r - psi(r)), abs_jerk[nt] = sum of |term| of the jerk (conditioning). */
+int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_out, double r_in,
+                        int64_t nt, const int64_t* targets,
+                        double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk)
+{
+    int64_t coincident = 0;
+    const double D = r_out - r_in;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : coincident)
+    for (int64_t t = 0; t < nt; ++t) {
+        const int64_t i = targets ? targets[t] : t;
+        const double xi[3] = { pm[4 * i], pm[4 * i + 1], pm[4 * i + 2] };
+        const double vi[3] = { vel[4 * i], vel[4 * i + 1], vel[4 * i + 2] };
+        double a[3] = { 0, 0, 0 }, jk[3] = { 0, 0, 0 }, phi = 0.0, ab = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            const double d[3] = { pm[4 * j] - xi[0], pm[4 * j + 1] - xi[1], pm[4 * j + 2] - xi[2] };
+            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            if (r2 >= r_out * r_out) continue;
+            if (r2 == 0.0) { ++coincident; continue; }
+            const double v[3] = { vel[4 * j] - vi[0], vel[4 * j + 1] - vi[1], vel[4 * j + 2] - vi[2] };
+            const double m = pm[4 * j + 3], r = sqrt(r2), r3 = r2 * r, r5 = r3 * r2;
+            const double dv = d[0] * v[0] + d[1] * v[1] + d[2] * v[2];
+            const double x = (r - r_in) / D;
+            const double K = 1.0 - p3t_o_W(x);
+            const double Kdot = -p3t_o_dW(x) * dv / (r * D);
+            double tn = 0.0;
+            for (int c = 0; c < 3; ++c) {
+                a[c] += m * K * d[c] / r3;
+                const double term = m * (K * (v[c] / r3 - 3.0 * dv * d[c] / r5) + Kdot * d[c] / r3);
+                jk[c] += term; tn += term * term;
+            }
+            ab += sqrt(tn);
+            phi += m * (-1.0 / r - p3t_o_psi(r, r_out, r_in));
+        }
+        for (int c = 0; c < 3; ++c) {
+            if (acc_irr) acc_irr[3 * t + c] = a[c];
+            if (jerk_irr) jerk_irr[3 * t + c] = jk[c];
+        }
+        if (phi_irr) phi_irr[t] = phi;
+        if (abs_jerk) abs_jerk[t] = ab;
+    }
+    return coincident;
+}

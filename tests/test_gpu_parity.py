@@ -369,3 +369,22 @@ def test_theta_and_radii_change_without_rebuild(p3t, cfg1):
             v.r_out = float(np.float32(ro)); v.r_in = float(np.float32(0.1 * ro))
             check_force(ctx, T, v, 0)
             check_neighbours(ctx, v, targets=workloads.sample_targets(w.n, 2000))
+
+
+def test_list_pools_grow_between_calls(p3t):
+    """The interaction-list pools of a context are sized by its first call; a later, much larger problem
+    must repeat the walk with larger pools and still match the oracle exactly."""
+    small = workloads.make_config(1, n_override=3000)
+    big = workloads.make_config(2, n_override=60000, theta=0.3)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(small.pos_mass), 63)
+        ctx.regular_force(small.r_out, small.r_in, small.theta, 0)
+        T = oracle.Tree(big.pos_mass, 63, NLEAF, NCRIT)
+        ctx.build_tree(_cuda(big.pos_mass), 63)
+        check_force(ctx, T, big, 0)
+        check_neighbours(ctx, big)
+        # and back to the small one with the large pools
+        Ts = oracle.Tree(small.pos_mass, 63, NLEAF, NCRIT)
+        ctx.build_tree(_cuda(small.pos_mass), 63)
+        check_force(ctx, Ts, small, 0)
+        check_neighbours(ctx, small)

@@ -64,6 +64,42 @@ def plummer_positions(seed: int, n: int) -> np.ndarray:
     return _isotropic(seed, n, r)
 
 
+def plummer_velocities(seed: int, pos: np.ndarray) -> np.ndarray:
+    """Isotropic velocities of the Plummer model at the given positions (Aarseth, Henon & Wielen 1974):
+    speed q v_esc with q drawn from q^2 (1 - q^2)^(7/2) by rejection, v_esc^2 = 2 / sqrt(r^2 + a^2)
+    (Henon units).  Input of the irregular-force path; for the King
+    configuration the same recipe stands in (only the magnitude and isotropy of v matter there).
+    Returns float64 [n, 3]."""
+    n = pos.shape[0]
+    q = np.zeros(n)
+    todo = np.arange(n)
+    rnd = 0
+    while todo.size:
+        u1 = uniform(seed, 8 + 2 * rnd, n)[todo]
+        u2 = uniform(seed, 9 + 2 * rnd, n)[todo]
+        ok = 0.1 * u2 < u1 * u1 * (1.0 - u1 * u1) ** 3.5
+        q[todo[ok]] = u1[ok]
+        todo = todo[~ok]
+        rnd += 1
+        if rnd > 200:
+            q[todo] = 0.5
+            break
+    r2 = (pos * pos).sum(axis=1)
+    speed = q * np.sqrt(2.0) * (r2 + PLUMMER_A * PLUMMER_A) ** (-0.25)
+    cz = 2.0 * uniform(seed, 6, n) - 1.0
+    ph = 2.0 * np.pi * uniform(seed, 7, n)
+    sz = np.sqrt(np.maximum(0.0, 1.0 - cz * cz))
+    return np.stack([speed * sz * np.cos(ph), speed * sz * np.sin(ph), speed * cz], axis=1)
+
+
+def velocities_for(w) -> np.ndarray:
+    """float32 [n, 4] = vx, vy, vz, 0 for a Workload (C-contiguous), seeded by the workload's seed."""
+    v = plummer_velocities(w.seed, w.pos_mass[:, :3].astype(np.float64))
+    out = np.zeros((v.shape[0], 4), dtype=np.float32)
+    out[:, :3] = v.astype(np.float32)
+    return np.ascontiguousarray(out)
+
+
 def _king_rho(w: float) -> float:
     if w <= 0.0:
         return 0.0
