@@ -202,6 +202,14 @@ def run_ours(args, w, rank, world, local_rank, dist):
     total_ms = float(sum(step_ms))
     launches = int(st["launches"] - st0["launches"])
 
+    # ---- SURVEY 8f NEXT-1 (outside the step): irregular force + jerk over the emitted lists ----
+    vel_dev = torch.from_numpy(workloads.velocities_for(w)).to(dev)
+    irr_ms = []
+    for k in range(5):
+        ctx.irregular_force(vel_dev)
+        irr_ms.append(ctx.stats()["ms_irregular"])
+    irr_ms = float(np.median(irr_ms[1:]))
+
     # ---- end-to-end arm: HOST buffers through p3t_step_host ----
     pm_host = torch.from_numpy(w.pos_mass).pin_memory()
     acc_host = torch.empty((n, 4), dtype=torch.float32).pin_memory()
@@ -261,6 +269,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
         "nodes": st["n_nodes"], "groups": st["n_groups"], "neighbours_total": st["nb_total"], "neighbours_max": st["nb_max"],
         "e2e": {"value": e2e_value, "unit": "particles/s", "ms_per_step": e2e_ms_max / args.steps,
                 "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n + 8 * (n + 1) + 4 * int(nb_total)},
+        "next1_irregular": {"ms": irr_ms, "list_entries_per_s": st["nb_total"] / (irr_ms * 1e-3) if irr_ms > 0 else None,
+                            "note": "p3t_irregular_force (F_I, jerk, phi_I over the neighbour lists); not part of the timed step"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -66,6 +66,7 @@ typedef struct p3t_stats {
     float   ms_sort;         /* ... of the radix sort inside the last build             */
     float   ms_eval;         /* ... of the force kernel (a8, a9, a11) alone             */
     float   ms_count;        /* ... of the neighbour count walk + offset scan (a10)     */
+    float   ms_irregular;    /* ... of the last p3t_irregular_force kernel (0 if none)  */
     int64_t launches;        /* kernels this context has launched since p3t_create      */
 } p3t_stats;
 
@@ -93,6 +94,16 @@ int p3t_build_tree(p3t_ctx* ctx, int64_t n, const float* pos_mass, int key_bits)
  * potential -sum m_j / r_ij.  Requires a prior build; theta, r_out, r_in may change between
  * calls without a rebuild.  Also produces the neighbour lists returned by p3t_neighbours. */
 int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float* acc_pot);
+
+/* irregular force, jerk and potential over the neighbour lists of the last
+ * p3t_regular_force (same r_out, r_in), eq. 1, 2, 5, 7 (the paper's CUTOFF / cutoff0
+ * routines, :396-398):  F_I = sum_{j in L(i)} m_j K d / r^3,  Fdot_I = its exact time derivative
+ * (R2: eq. 2 / 7 are garbled in the text),  phi_I = sum m_j (-1/r - psi(r)), so that
+ * F_I + F_R and phi_I + phi_R (pot_mode 0) are the unsplit Newtonian sums.
+ * vel: DEVICE pointer, n x {vx, vy, vz, unused} fp32, ORIGINAL order, caller-owned, read-only.
+ * acc_irr: DEVICE, n x {ax, ay, az, phi_I}; jerk_irr: DEVICE, n x {jx, jy, jz, 0}; ORIGINAL order.
+ * All three 16-byte aligned.  P3T_ESTATE without a prior p3t_regular_force.  Does not synchronise. */
+int p3t_irregular_force(p3t_ctx* ctx, const float* vel, float* acc_irr, float* jerk_irr);
 
 /* Neighbour lists L(i) = { j != i : r_ij < r_out } of the last
  * p3t_regular_force, as CSR in ORIGINAL particle ids: offsets[n+1] (int64), indices[total]

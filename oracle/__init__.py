@@ -52,7 +52,7 @@ def lib() -> C.CDLL:
         _lib.p3t_o_direct.restype = i64
         _lib.p3t_o_direct.argtypes = [i64, vp, d, d, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_irregular.restype = i64
-        _lib.p3t_o_irregular.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp]
+        _lib.p3t_o_irregular.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp, vp]
         _lib.p3t_o_neighbours.restype = i64
         _lib.p3t_o_neighbours.argtypes = [i64, vp, f32, C.c_int, i64, vp, vp, vp]
         _lib.p3t_o_tree_build.restype = vp
@@ -126,9 +126,9 @@ def irregular(pos_mass, vel, r_out: float, r_in: float, targets=None):
     pm = _pm(pos_mass); v = _pm(vel)
     t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
     nt = pm.shape[0] if t is None else t.shape[0]
-    acc = np.zeros((nt, 3)); jerk = np.zeros((nt, 3)); phi = np.zeros(nt); ab = np.zeros(nt)
-    coinc = lib().p3t_o_irregular(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(acc), _p(jerk), _p(phi), _p(ab))
-    return dict(acc_irr=acc, jerk_irr=jerk, phi_irr=phi, abs_jerk=ab, coincident=int(coinc))
+    acc = np.zeros((nt, 3)); jerk = np.zeros((nt, 3)); phi = np.zeros(nt); ab = np.zeros(nt); an = np.zeros(nt)
+    coinc = lib().p3t_o_irregular(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(acc), _p(jerk), _p(phi), _p(ab), _p(an))
+    return dict(acc_irr=acc, jerk_irr=jerk, phi_irr=phi, abs_jerk=ab, abs_newt=an, coincident=int(coinc))
 
 
 def neighbours(pos_mass, r_out: float, targets=None, fp32_predicate: bool = True):

@@ -38,10 +38,11 @@ int64_t p3t_o_direct(int64_t n, const float* pos_mass, double r_out, double r_in
 
 /* eq. 1, 2, 5, 7: irregular acceleration, jerk and potential over the neighbour sphere r_ij < r_out
  * (SURVEY 8f NEXT-1).  vel: n x 4 fp32.  Outputs (any may be NULL): acc_irr[3nt], jerk_irr[3nt],
- * phi_irr[nt], abs_jerk[nt] (sum of |jerk term|).  Returns the number of coincident pairs skipped. */
+ * phi_irr[nt], abs_jerk[nt] (sum of |jerk term|), abs_newt[nt] (sum of the K = 1 term sizes).
+ * Returns the number of coincident pairs skipped. */
 int64_t p3t_o_irregular(int64_t n, const float* pos_mass, const float* vel, double r_out, double r_in,
                         int64_t nt, const int64_t* targets,
-                        double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk);
+                        double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt);
 
 /* Brute-force neighbour rows for nt targets.  fp32_predicate = 1: the bit-spec predicate
  * (R10); 0: the fp64 "physics" predicate r_ij < r_out.  counts[nt] is always written;

@@ -172,10 +172,11 @@ int64_t p3t_o_neighbours(int64_t n, const float* pm, float r_out, int fp32_predi
  * differences in tests/test_oracle_irregular.py).  Coincident pairs (r = 0, reading R8) are skipped
  * (a KS pair in the host code) and counted in the return value.
  * vel: n x 4 fp32 (vx, vy, vz, unused).  Outputs (any may be NULL): acc_irr[3 nt], jerk_irr[3 nt],
- * phi_irr[nt] = sum m_j (-1/r - psi(r)), abs_jerk[nt] = sum of |term| of the jerk (conditioning). */
+ * phi_irr[nt] = sum m_j (-1/r - psi(r)); conditioning of the sums: abs_jerk[nt] = sum of |jerk term|,
+ * abs_newt[nt] = sum m_j (|v|/r^3 + 3 |d.v|/r^4), the size of the unweighted (K = 1) jerk terms. */
 int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_out, double r_in,
                         int64_t nt, const int64_t* targets,
-                        double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk)
+                        double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt)
 {
     int64_t coincident = 0;
     const double D = r_out - r_in;
@@ -184,7 +185,7 @@ int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_o
         const int64_t i = targets ? targets[t] : t;
         const double xi[3] = { pm[4 * i], pm[4 * i + 1], pm[4 * i + 2] };
         const double vi[3] = { vel[4 * i], vel[4 * i + 1], vel[4 * i + 2] };
-        double a[3] = { 0, 0, 0 }, jk[3] = { 0, 0, 0 }, phi = 0.0, ab = 0.0;
+        double a[3] = { 0, 0, 0 }, jk[3] = { 0, 0, 0 }, phi = 0.0, ab = 0.0, an = 0.0;
         for (int64_t j = 0; j < n; ++j) {
             if (j == i) continue;
             const double d[3] = { pm[4 * j] - xi[0], pm[4 * j + 1] - xi[1], pm[4 * j + 2] - xi[2] };
@@ -204,6 +205,7 @@ int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_o
                 jk[c] += term; tn += term * term;
             }
             ab += sqrt(tn);
+            an += m * (sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) / r3 + 3.0 * fabs(dv) / (r2 * r2));
             phi += m * (-1.0 / r - p3t_o_psi(r, r_out, r_in));
         }
         for (int c = 0; c < 3; ++c) {
@@ -212,6 +214,7 @@ int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_o
         }
         if (phi_irr) phi_irr[t] = phi;
         if (abs_jerk) abs_jerk[t] = ab;
+        if (abs_newt) abs_newt[t] = an;
     }
     return coincident;
 }

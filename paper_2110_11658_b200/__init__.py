@@ -22,7 +22,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4, -5
 # every symbol include/p3t.h declares
 SYMBOLS = [
     "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_build_tree", "p3t_regular_force",
-    "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
+    "p3t_irregular_force", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
 ]
@@ -36,7 +36,7 @@ class Stats(C.Structure):
         ("nb_total", C.c_int64), ("nb_max", C.c_int32), ("input_bad", C.c_int32),
         ("cube_lo", C.c_float * 3), ("cube_side", C.c_float),
         ("ms_build", C.c_float), ("ms_force", C.c_float), ("ms_walk", C.c_float), ("ms_sort", C.c_float),
-        ("ms_eval", C.c_float), ("ms_count", C.c_float),
+        ("ms_eval", C.c_float), ("ms_count", C.c_float), ("ms_irregular", C.c_float),
         ("launches", C.c_int64),
     ]
 
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
     L.p3t_set_tree_params.argtypes = [vp, C.c_int, C.c_int]
     L.p3t_build_tree.argtypes = [vp, i64, vp, C.c_int]
     L.p3t_regular_force.argtypes = [vp, f32, f32, f32, C.c_int, vp]
+    L.p3t_irregular_force.argtypes = [vp, vp, vp, vp]
     L.p3t_neighbours.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
     L.p3t_neighbours_copy.argtypes = [vp, vp, vp]
     L.p3t_neighbours_nbody6.argtypes = [vp, i32, vp]
@@ -172,6 +173,19 @@ class Context:
             out = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
         self._check(lib().p3t_regular_force(self._h, r_out, r_in, theta, pot_mode, self._dev_f32(out, 4)), "p3t_regular_force")
         return out
+
+    def irregular_force(self, vel, acc_out=None, jerk_out=None):
+        """Irregular force over the neighbour lists of the last regular_force.
+        vel: CUDA float32 [n, 4] (vx, vy, vz, unused), original order.  Returns (acc_irr [n, 4] = ax, ay,
+        az, phi_I; jerk_irr [n, 4] = jx, jy, jz, 0) as CUDA tensors in original order."""
+        torch = self._torch
+        if acc_out is None:
+            acc_out = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
+        if jerk_out is None:
+            jerk_out = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
+        self._check(lib().p3t_irregular_force(self._h, self._dev_f32(vel, 4), self._dev_f32(acc_out, 4), self._dev_f32(jerk_out, 4)),
+                    "p3t_irregular_force")
+        return acc_out, jerk_out
 
     def neighbours(self):
         """(offsets int64 [n+1], indices int32 [total]) as CUDA tensors (copied from the library's buffers)."""

@@ -59,6 +59,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
     for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evw[k]);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evi[k]);
     if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
     int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
     if (rc == P3T_OK) rc = p3t_tree_init(c);
@@ -73,13 +74,14 @@ int p3t_destroy(p3t_ctx* c)
     if (!c) return P3T_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
+    p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill, &c->pcpool, &c->pppool, &c->glist,
                         &c->info, &c->stage_in, &c->stage_out };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
+    for (int k = 0; k < 2; ++k) if (c->evi[k]) cudaEventDestroy(c->evi[k]);
     (void)cudaGetLastError();
     delete c;
     return P3T_OK;
@@ -98,7 +100,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     if (((uintptr_t)pos_mass & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
     P3T_CUDA(c, cudaSetDevice(c->device));
-    c->state = 0; c->nb_valid = 0;
+    c->state = 0; c->nb_valid = 0; c->irr_done = 0;
     c->n = n; c->key_bits = key_bits; c->bits = key_bits / 3;
     // hard bound on the cell count (data layout): leaves <= n, branching cells < n,
     // one-child chain cells <= levels * n / (nleaf + 1)
@@ -109,7 +111,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     const size_t ntiles = (N + P3T_SORT_TILE - 1) / P3T_SORT_TILE;
     int rc;
 #define RES(buf, bytes) if ((rc = p3t_reserve(c, &c->buf, (bytes))) != P3T_OK) return rc
-    RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16);
+    RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16); RES(rank, N * 4);
     RES(hist, (ntiles + 1) * P3T_RADIX * 4);
     RES(nlevel, C * 4); RES(nbegin, C * 4); RES(nend, C * 4); RES(nfirst, C * 4); RES(nnchild, C * 4);
     RES(m64, C * 80);
@@ -141,11 +143,24 @@ int p3t_regular_force(p3t_ctx* c, float r_out, float r_in, float theta, int pot_
     if (c->sticky) return P3T_ECUDA;
     if (c->state < 1) return P3T_ESTATE;
     P3T_CUDA(c, cudaSetDevice(c->device));
-    c->nb_valid = 0;
+    c->nb_valid = 0; c->irr_done = 0;
     c->r_out = r_out; c->r_in = r_in; c->theta = theta;
     int rc = p3t_launch_force(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot);
     if (rc != P3T_OK) return rc;
     c->state = 2; c->nb_valid = 1;
+    return P3T_OK;
+}
+
+int p3t_irregular_force(p3t_ctx* c, const float* vel, float* acc_irr, float* jerk_irr)
+{
+    if (!c || !vel || !acc_irr || !jerk_irr) return P3T_EINVAL;
+    if ((((uintptr_t)vel | (uintptr_t)acc_irr | (uintptr_t)jerk_irr) & 15u) != 0) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 2 || !c->nb_valid) return P3T_ESTATE;
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    int rc = p3t_launch_irregular(c, (const float4*)vel, (float4*)acc_irr, (float4*)jerk_irr);
+    if (rc != P3T_OK) return rc;
+    c->irr_done = 1;
     return P3T_OK;
 }
 
@@ -187,6 +202,7 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         (void)cudaEventElapsedTime(&out->ms_eval, c->evw[0], c->evw[1]);
         (void)cudaEventElapsedTime(&out->ms_walk, c->evw[2], c->evw[3]);
         (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->evw[2]);
+        if (c->irr_done) (void)cudaEventElapsedTime(&out->ms_irregular, c->evi[0], c->evi[1]);
     }
     (void)cudaGetLastError();
     return rc;

@@ -11,6 +11,7 @@
 // memory while the previous tile is being evaluated, so the FP32 pipe never waits for the walk.
 // Rules: DESIGN.md R-S8 (evaluation), R-S9 (accumulation), R10 (neighbour predicate, bit-specified).
 #include "p3t_internal.cuh"
+#include "p3t_cutoff.cuh"
 #include <stdio.h>
 #include <stdlib.h>
 #include <math.h>
@@ -20,18 +21,6 @@
 #define FORCE_CTAS_PER_SM 5
 #define TILE          32                  // list entries per tile
 #define FAR_AWAY      1.0e18f             // position of the zero-mass padding entries of a tile
-
-struct walk_consts {
-    float rout2, rin2, r_in, inv_delta;   // inv_delta = 1 / (r_out - r_in)
-    float psi_in;                          // psi(r_in), the constant regular pair potential inside r_in
-    float k140;                            // 140 / (r_out - r_in)
-    float s1;                              // S(1)
-    float sc[6];                           // S(t) = t (sc0 + t (sc1 + ... t sc5))
-    float rem;                             // c^3 (1+c)^3  (> 0)
-    float c;                               // r_in / (r_out - r_in)
-    float theta;
-    int   pot_mode;
-};
 
 struct force_args {
     const float4* spm; const uint32_t* order;
@@ -74,24 +63,6 @@ __device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1,
 __device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-
-// eq. 6, 0 < x < 1: W = x^4 (35 - 84 x + 70 x^2 - 20 x^3); evaluated through the
-// symmetry W(x) = 1 - W(1 - x) above x = 1/2 so that fp32 Horner never cancels.
-__device__ __forceinline__ float cutoff_W(float x)
-{
-    float t = x > 0.5f ? 1.0f - x : x;
-    float t2 = t * t;
-    float w = t2 * t2 * (35.0f + t * (-84.0f + t * (70.0f - 20.0f * t)));
-    return x > 0.5f ? 1.0f - w : w;
-}
-
-// regular pair potential for r_in < r < r_out (R6): -W/r - (140/D) int_x^1 t^3(1-t)^3/(t+c) dt
-__device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float W, float rinv)
-{
-    float sx = x * (K.sc[0] + x * (K.sc[1] + x * (K.sc[2] + x * (K.sc[3] + x * (K.sc[4] + x * K.sc[5])))));
-    float integral = (K.s1 - sx) - K.rem * __logf((1.0f + K.c) / (x + K.c));
-    return -W * rinv - K.k140 * integral;
-}
 
 // One work item = up to 32 targets of one group (see k_force; the items of a group stream the same
 // lists).  An item with c <= 16 targets gives every target k = 2, 4 or 8 lanes
@@ -484,28 +455,6 @@ __global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict
             idx[rb + r] = v;
         }
     }
-}
-
-
-static void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode)
-{
-    // fp32 thresholds exactly as DESIGN.md R10 states them: one fp32 product each
-    volatile float ro2 = r_out * r_out, ri2 = r_in * r_in;
-    K.rout2 = ro2; K.rin2 = ri2; K.r_in = r_in;
-    const double D = (double)r_out - (double)r_in, c = (double)r_in / D, c1 = 1.0 + c;
-    K.inv_delta = (float)(1.0 / D);
-    K.k140 = (float)(140.0 / D);
-    // t^3 (1-t)^3 = (t + c) (b5 t^5 + ... + b0) - c^3 (1+c)^3   (synthetic division at t = -c)
-    const double b[6] = { c * c * c1 * c1 * c1, -c * c1 * c1 * c1, c1 * c1 * c1, -(3.0 + 3.0 * c + c * c), 3.0 + c, -1.0 };
-    double s1 = 0.0;
-    for (int k = 0; k < 6; ++k) { K.sc[k] = (float)(b[k] / (k + 1)); s1 += b[k] / (k + 1); }
-    K.s1 = (float)s1;
-    K.rem = (float)(c * c * c * c1 * c1 * c1);
-    K.c = (float)c;
-    // psi(r_in) = -(140/D) [ S(1) + rem ln((1+c)/c) ... ] with W(0) = 0; here the remainder enters with a minus sign
-    K.psi_in = (float)(-(140.0 / D) * (s1 - c * c * c * c1 * c1 * c1 * log(c1 / c)));
-    K.theta = theta;
-    K.pot_mode = pot_mode;
 }
 
 

@@ -52,6 +52,7 @@ struct p3t_ctx {
     // device buffers (grow-only)
     p3t_buf keys[2], idx[2];         // uint64 / uint32 ping-pong; after the sort [0] holds the result
     p3t_buf spm;                     // float4 sorted bodies
+    p3t_buf rank;                    // int32: original id -> sorted position
     p3t_buf hist;                    // sort: per-block digit counts
     p3t_buf nlevel, nbegin, nend, nfirst, nnchild;        // int32 per node
     p3t_buf m64;                     // double[10] per node: M, com[3], Q[6]
@@ -75,6 +76,8 @@ struct p3t_ctx {
     int nb_valid;
     cudaEvent_t ev[6];               // build begin/end, sort begin/end ... force begin/end, walk begin/end
     cudaEvent_t evw[4];
+    cudaEvent_t evi[2];              // irregular-force kernel begin/end
+    int irr_done;
     p3t_stats last;
     float r_out, r_in, theta;
     int64_t launches;                // kernels launched so far
@@ -103,5 +106,7 @@ int p3t_launch_tree(p3t_ctx* ctx);
 int p3t_walk_init(p3t_ctx* ctx);
 int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta);
 int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta);
+// p3t_irregular.cu : SURVEY 8f NEXT-1
+int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk);
 // p3t_force.cu : a8-a11
 int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot);

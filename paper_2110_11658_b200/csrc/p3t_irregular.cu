@@ -1,0 +1,112 @@
+// p3t_irregular.cu -- SURVEY.md 8f NEXT-1: the irregular force, its time derivative (jerk) and the
+// irregular potential of every particle over the neighbour list that p3t_regular_force emitted
+// (eq. 1, 2, 5, 7; the paper's CUTOFF / cutoff0 routines, Table B2 :396-398).
+//
+// With d = x_j - x_i, v = xdot_j - xdot_i (attractive sign: DESIGN.md R1), r = |d|,
+// x = (r - r_in)/(r_out - r_in), K = 1 - W (eq. 6):
+//     F_I    = sum_{j in L(i)} m_j K d / r^3                                               (eq. 1)
+//     Fdot_I = sum_{j in L(i)} m_j [ K ( v / r^3 - 3 (d.v) d / r^5 ) + Kdot d / r^3 ]      (eq. 2)
+//     Kdot   = -W'(x) (d.v) / (r (r_out - r_in)),  W'(x) = 140 x^3 (1-x)^3                 (eq. 7)
+//     phi_I  = sum_{j in L(i)} m_j ( -1/r - psi(r) )            (so that phi_I + phi_R = phi_Newton)
+// Reading R2: eq. 2 / 7 are garbled in the text; Fdot_I is the exact time derivative of
+// eq. 1.  Coincident pairs (r = 0, R8) are skipped.
+//
+// The lists are short (mean 2 entries at the paper's radii, up to ~500 in a King core): one thread
+// per row up to 32 entries, one warp per longer row; terms in fp32 (IEEE sqrt and division, so that
+// the r^-5 factor keeps 1e-7), sums in fp64.  HBM/L2-bound gather: 36 B per list entry.
+#include "p3t_internal.cuh"
+#include "p3t_cutoff.cuh"
+
+struct irr_args {
+    const float4* spm; const int32_t* rank;     // sorted bodies, original id -> sorted position
+    const float4* vel;                          // original order
+    const int64_t* nboff; const int32_t* nbidx; // CSR, original ids
+    float4 *acc, *jerk;                         // original order
+    int n;
+    walk_consts K;
+};
+
+struct irr_sum { double ax, ay, az, jx, jy, jz, ph; };
+
+__device__ __forceinline__ void irr_term(const irr_args& A, const float4 pi, const float4 vi, int j, irr_sum& S)
+{
+    const walk_consts& K = A.K;
+    const float4 pj = A.spm[A.rank[j]], vj = A.vel[j];
+    const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (!(r2 > 0.0f)) return;                                    // coincident pair (R8)
+    const float vx = vj.x - vi.x, vy = vj.y - vi.y, vz = vj.z - vi.z;
+    const float r = sqrtf(r2), ri = 1.0f / r, ri2 = ri * ri, ri3 = ri2 * ri;
+    const float dv = fmaf(dz, vz, fmaf(dy, vy, dx * vx));
+    const float m = pj.w;
+    float Kc = 1.0f, Kdot = 0.0f, ph;
+    if (r2 > K.rin2) {
+        const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f), y = 1.0f - x;
+        Kc = cutoff_W(y);                                        // K(x) = 1 - W(x) = W(1 - x), no cancellation
+        const float xy = x * y;
+        Kdot = -140.0f * xy * xy * xy * dv * ri * K.inv_delta;   // -W'(x) xdot
+        // -1/r - psi = -K/r + (140/D) int_x^1 t^3 (1-t)^3 / (t+c) dt = -cutoff_psi with W replaced by -K
+        ph = -cutoff_psi64(K, x, -Kc, ri);
+    } else {
+        ph = -ri - K.psi_in;
+    }
+    const float a = m * Kc * ri3;                                // m K / r^3
+    const float b = m * (Kdot * ri3 - 3.0f * Kc * dv * ri3 * ri2);   // m ( Kdot / r^3 - 3 K (d.v) / r^5 )
+    S.ax += (double)(a * dx); S.ay += (double)(a * dy); S.az += (double)(a * dz);
+    S.jx += (double)fmaf(a, vx, b * dx); S.jy += (double)fmaf(a, vy, b * dy); S.jz += (double)fmaf(a, vz, b * dz);
+    S.ph += (double)(m * ph);
+}
+
+__global__ void __launch_bounds__(256) k_irregular(irr_args A)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    long long b = 0; int len = 0;
+    float4 pi = make_float4(0, 0, 0, 0), vi = pi;
+    if (i < A.n) { b = A.nboff[i]; len = (int)(A.nboff[i + 1] - b); pi = A.spm[A.rank[i]]; vi = A.vel[i]; }
+    irr_sum S = { 0, 0, 0, 0, 0, 0, 0 };
+    if (len <= 32)
+        for (int k = 0; k < len; ++k) irr_term(A, pi, vi, A.nbidx[b + k], S);
+    // rows longer than a warp: all 32 lanes share the row, partial sums reduced by shuffle (fixed order)
+    uint32_t m = __ballot_sync(0xffffffffu, len > 32);
+    while (m) {
+        const int src = __ffs(m) - 1; m &= m - 1;
+        const long long rb = __shfl_sync(0xffffffffu, b, src);
+        const int rl = __shfl_sync(0xffffffffu, len, src);
+        float4 p, v;
+        p.x = __shfl_sync(0xffffffffu, pi.x, src); p.y = __shfl_sync(0xffffffffu, pi.y, src);
+        p.z = __shfl_sync(0xffffffffu, pi.z, src); p.w = 0.0f;
+        v.x = __shfl_sync(0xffffffffu, vi.x, src); v.y = __shfl_sync(0xffffffffu, vi.y, src);
+        v.z = __shfl_sync(0xffffffffu, vi.z, src); v.w = 0.0f;
+        irr_sum R = { 0, 0, 0, 0, 0, 0, 0 };
+        for (int k = lane; k < rl; k += 32) irr_term(A, p, v, A.nbidx[rb + k], R);
+        double* r = &R.ax;
+#pragma unroll
+        for (int c = 0; c < 7; ++c)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                int lo = __double2loint(r[c]), hi = __double2hiint(r[c]);
+                lo = __shfl_xor_sync(0xffffffffu, lo, o); hi = __shfl_xor_sync(0xffffffffu, hi, o);
+                r[c] += __hiloint2double(hi, lo);
+            }
+        if (lane == src) S = R;
+    }
+    if (i < A.n) {
+        A.acc[i]  = make_float4((float)S.ax, (float)S.ay, (float)S.az, (float)S.ph);
+        A.jerk[i] = make_float4((float)S.jx, (float)S.jy, (float)S.jz, 0.0f);
+    }
+}
+
+int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk)
+{
+    irr_args A;
+    A.spm = P<float4>(ctx->spm); A.rank = P<int32_t>(ctx->rank);
+    A.vel = vel; A.nboff = P<int64_t>(ctx->nboff); A.nbidx = P<int32_t>(ctx->nbidx);
+    A.acc = acc; A.jerk = jerk; A.n = (int)ctx->n;
+    make_consts(A.K, ctx->r_out, ctx->r_in, ctx->theta, 0);
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evi[0], ctx->stream));
+    k_irregular<<<(A.n + 255) / 256, 256, 0, ctx->stream>>>(A);
+    P3T_CUDA(ctx, cudaGetLastError());
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evi[1], ctx->stream));
+    ctx->launches += 1;
+    return P3T_OK;
+}

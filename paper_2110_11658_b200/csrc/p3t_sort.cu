@@ -204,10 +204,10 @@ __global__ void __launch_bounds__(P3T_SORT_THREADS) k_scatter(const uint64_t* __
 }
 
 __global__ void __launch_bounds__(256) k_permute(const float4* __restrict__ pm, const uint32_t* __restrict__ order,
-                                                 int n, float4* __restrict__ spm)
+                                                 int n, float4* __restrict__ spm, int32_t* __restrict__ rank)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) spm[i] = __ldg(pm + order[i]);
+    if (i < n) { const uint32_t o = order[i]; spm[i] = __ldg(pm + o); rank[o] = i; }    // rank: original id -> sorted position
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -255,7 +255,7 @@ int p3t_launch_sort(p3t_ctx* ctx)
 int p3t_launch_permute(p3t_ctx* ctx, const float4* pm)
 {
     const int n = (int)ctx->n;
-    k_permute<<<(n + 255) / 256, 256, 0, ctx->stream>>>(pm, P<uint32_t>(ctx->idx[0]), n, P<float4>(ctx->spm));
+    k_permute<<<(n + 255) / 256, 256, 0, ctx->stream>>>(pm, P<uint32_t>(ctx->idx[0]), n, P<float4>(ctx->spm), P<int32_t>(ctx->rank));
     P3T_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
     return P3T_OK;

@@ -1,0 +1,115 @@
+"""GPU parity of p3t_irregular_force (eq. 1, 2, 5, 7 over the emitted neighbour
+lists) against the fp64 oracle (oracle.irregular, pinned in test_oracle_irregular.py), through the C-ABI.
+
+Tolerance: every term is evaluated in fp32 with IEEE sqrt and division (a few ulp each, 6e-8) and
+summed in fp64: |error| <= 2e-6 x the sum of |terms| of the row.  On top of that the cutoff argument
+x = (r - r_in)/(r_out - r_in) carries the rounding of r, dx ~ 7e-8, so K and K' = dW/dx move by
+W' dx <= 1.5e-7 and W'' dx <= 5e-7 of the UNWEIGHTED (K = 1) term: + 1e-6 x abs_newt.  (Near x = 1
+the weighted terms vanish like (1-x)^4 and that absolute floor is what is left.)"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def p3t():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2110_11658_b200 as m
+    m.lib()
+    return m
+
+
+def _cuda(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _check(p3t, w, targets=None, r_out=None):
+    r_out = w.r_out if r_out is None else r_out
+    r_in = float(np.float32(0.1) * np.float32(r_out))
+    vel = workloads.velocities_for(w)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        reg = ctx.regular_force(r_out, r_in, w.theta, 0).cpu().numpy().astype(np.float64)
+        acc, jerk = ctx.irregular_force(_cuda(vel))
+        acc = acc.cpu().numpy().astype(np.float64); jerk = jerk.cpu().numpy().astype(np.float64)
+        off, idx = ctx.neighbours()
+        off = off.cpu().numpy(); idx = idx.cpu().numpy()
+        st = ctx.stats()
+    o = oracle.irregular(w.pos_mass, vel, r_out, r_in, targets=targets)
+    sel = slice(None) if targets is None else targets
+    a, j = acc[sel], jerk[sel]
+    ea = np.linalg.norm(a[:, :3] - o["acc_irr"], axis=1)
+    ej = np.linalg.norm(j[:, :3] - o["jerk_irr"], axis=1)
+    na = np.linalg.norm(o["acc_irr"], axis=1)
+    tol = 2e-6 * o["abs_jerk"] + 1e-6 * o["abs_newt"] + 1e-30
+    assert np.all(ej <= tol), (ej / tol).max()
+    assert np.linalg.norm(j[:, :3] - o["jerk_irr"]) <= 1e-6 * np.linalg.norm(o["jerk_irr"])
+    assert np.linalg.norm(a[:, :3] - o["acc_irr"]) <= 1e-6 * np.linalg.norm(o["acc_irr"])
+    has = na > 0
+    if has.sum() > 10:
+        assert np.median(ea[has] / na[has]) <= 1e-6
+    # potential: relative to the row's unweighted sum of m_j / r (the rounding of r moves every pair
+    # term by eps m K / r, which is all that is left of a pair near r_out where phi_I vanishes like (1-x)^5)
+    rows = np.repeat(np.arange(w.n), np.diff(off))
+    pos = w.pos_mass[:, :3].astype(np.float64)
+    rij = np.linalg.norm(pos[idx] - pos[rows], axis=1)
+    newt = np.zeros(w.n)
+    np.add.at(newt, rows[rij > 0], w.pos_mass[idx[rij > 0], 3].astype(np.float64) / rij[rij > 0])
+    assert np.all(np.abs(a[:, 3] - o["phi_irr"]) <= 3e-6 * np.abs(o["phi_irr"]) + 3e-7 * newt[sel] + 1e-30)
+    assert np.all(j[:, 3] == 0)
+    # empty rows give exact zeros (lists are often empty)
+    empty = np.diff(off) == 0
+    assert np.all(acc[empty] == 0) and np.all(jerk[empty] == 0)
+    return reg, acc, jerk, o, st
+
+
+def test_config1_full(p3t):
+    """Config 1 (Plummer 16k): every particle; F_I + F_R is the unsplit Newtonian force (eq. 3)."""
+    w = workloads.make_config(1)
+    reg, acc, jerk, o, st = _check(p3t, w)
+    d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
+    newton = d["acc_reg"] + d["acc_irr"]
+    tot = reg[:, :3] + acc[:, :3]
+    err = np.linalg.norm(tot - newton, axis=1) / np.linalg.norm(newton, axis=1)
+    assert np.median(err) < 2e-3 and np.percentile(err, 99) < 2e-2          # the tree error of F_R, north_star bound
+    assert np.abs((reg[:, 3] + acc[:, 3]) / d["phi_newt"] - 1).max() < 1e-3
+    assert st["ms_irregular"] > 0
+
+
+def test_larger_radius_long_rows(p3t):
+    """Rows longer than a warp (the warp-cooperative branch): 4 x the configured radius."""
+    w = workloads.make_config(1, n_override=6000)
+    reg, acc, jerk, o, st = _check(p3t, w, r_out=4 * w.r_out)
+    assert st["nb_max"] > 32
+
+
+def test_king_core_sampled(p3t):
+    """Config 4 recipe (King W0 = 9, Kroupa masses) at N = 2^17: long rows in the core, sampled targets."""
+    w = workloads.make_config(4, n_override=131072)
+    t = workloads.sample_targets(w.n, 4096)
+    _check(p3t, w, targets=t)
+
+
+def test_state_and_arguments(p3t):
+    import torch
+    w = workloads.make_config(1, n_override=2000)
+    vel = _cuda(workloads.velocities_for(w))
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.irregular_force(vel)                       # no regular force yet: no lists
+        assert e.value.code == -2
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0)
+        a1, j1 = ctx.irregular_force(vel)
+        a2, j2 = ctx.irregular_force(vel)                  # deterministic
+        assert torch.equal(a1, a2) and torch.equal(j1, j2)
+        # zero velocities: zero jerk, same acceleration
+        a0, j0 = ctx.irregular_force(torch.zeros_like(vel))
+        assert torch.equal(a0, a1) and torch.count_nonzero(j0) == 0
