@@ -157,6 +157,7 @@ def reduce_over_ranks(total_ms: float, units: float, dist) -> tuple:
 
 def run_ours(args, w, rank, world, local_rank, dist):
     import torch
+    import workloads
     import paper_2110_11658_b200 as p3t
 
     p3t.lib()                                             # fail loudly when the CUDA library is missing
