@@ -64,6 +64,8 @@ def lib() -> C.CDLL:
             f.restype = None; f.argtypes = [vp] * nargs
         _lib.p3t_o_tree_force.restype = None
         _lib.p3t_o_tree_force.argtypes = [vp, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
+        _lib.p3t_o_tree_force_buffered.restype = None
+        _lib.p3t_o_tree_force_buffered.argtypes = [vp, f32, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_pc_term.restype = None; _lib.p3t_o_pc_term.argtypes = [vp, vp, vp, vp]
         _lib.p3t_o_open_test.restype = C.c_int
         _lib.p3t_o_open_test.argtypes = [vp, vp, vp, vp, vp, f32, f32, f32, f32]
@@ -199,15 +201,17 @@ class Tree:
         lib().p3t_o_tree_groups(self._h, _p(b), _p(e), _p(glo), _p(ghi))
         return dict(begin=b, end=e, glo=glo, ghi=ghi)
 
-    def force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, group_ids=None, want_abs: bool = False):
+    def force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, group_ids=None, want_abs: bool = False,
+              r_list: float | None = None):
         """dict(acc_pot [n,4] fp64 in original order (rows of unwalked groups are NaN), npp, npc, abs_sum)."""
         gi = None if group_ids is None else np.ascontiguousarray(group_ids, dtype=np.int64)
         ng = self.n_groups if gi is None else gi.shape[0]
         out = np.full((self.n, 4), np.nan)
         npp = np.zeros(ng, np.int64); npc = np.zeros(ng, np.int64)
         ab = np.full(self.n, np.nan) if want_abs else None
-        lib().p3t_o_tree_force(self._h, float(np.float32(r_out)), float(np.float32(r_in)), float(np.float32(theta)),
-                               int(pot_mode), ng, _p(gi), _p(out), _p(npp), _p(npc), _p(ab))
+        rl = r_out if r_list is None else r_list          # neighbour search radius in the opening rule (NEXT-2)
+        lib().p3t_o_tree_force_buffered(self._h, float(np.float32(rl)), float(np.float32(r_out)), float(np.float32(r_in)),
+                                        float(np.float32(theta)), int(pot_mode), ng, _p(gi), _p(out), _p(npp), _p(npc), _p(ab))
         return dict(acc_pot=out, npp=npp, npc=npc, abs_sum=ab)
 
 

@@ -81,6 +81,16 @@ void p3t_o_tree_force(const p3t_o_tree* t, float r_out_f, float r_in_f, float th
                       int64_t ng, const int64_t* group_ids, double* acc_pot,
                       int64_t* npp, int64_t* npc, double* abs_sum)
 {
+    p3t_o_tree_force_buffered(t, r_out_f, r_out_f, r_in_f, theta, pot_mode, ng, group_ids, acc_pot, npp, npc, abs_sum);
+}
+
+/* SURVEY 8f NEXT-2, PAPER.md:113 (section 2.3, R_cut = R_s + R_buff) and eq. 20 (:156): the neighbour
+ * search reaches r_list = r_out + r_buff >= r_out, so the second clause of the opening rule uses
+ * r_list; the force itself is unchanged (cutoff between r_in and r_out). */
+void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list_f, float r_out_f, float r_in_f, float theta, int pot_mode,
+                               int64_t ng, const int64_t* group_ids, double* acc_pot,
+                               int64_t* npp, int64_t* npc, double* abs_sum)
+{
     const double r_out = r_out_f, r_in = r_in_f, D = r_out - r_in;
     const double psi_in = p3t_o_psi(r_in, r_out, r_in);
 #pragma omp parallel
@@ -90,7 +100,7 @@ void p3t_o_tree_force(const p3t_o_tree* t, float r_out_f, float r_in_f, float th
         for (int64_t q = 0; q < ng; ++q) {
             int64_t g = group_ids ? group_ids[q] : q;
             pc.n = pp.n = 0;
-            walk(t, g, 0, theta, r_out_f, &pc, &pp);
+            walk(t, g, 0, theta, r_list_f, &pc, &pp);
             if (npp) npp[q] = pp.n;
             if (npc) npc[q] = pc.n;
             for (int32_t i = t->gbegin[g]; i < t->gend[g]; ++i) {

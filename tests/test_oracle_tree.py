@@ -273,3 +273,50 @@ def test_tree_vs_direct_error_bound(cfg1):
     filled = ~np.isnan(sub["acc_pot"][:, 0])
     assert filled.sum() == cnt[0] + cnt[5]
     assert np.array_equal(sub["acc_pot"][filled], f["acc_pot"][filled])
+
+
+# ---- buffered neighbour search radius (eq. 20 :156) ----
+def test_buffered_search_radius(cfg1):
+    """r_list = r_out + r_buff only widens the second clause of the opening rule: the force stays the
+    regular force of eq. 3 (same cutoff radii), every particle within r_list of a target is met particle
+    by particle (so the buffered neighbour sets are complete), and theta -> 0 is still the direct sum."""
+    w = cfg1
+    t = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    r_list = float(np.float32(4.0 * w.r_out))     # large enough for the second clause to bite (l / theta ~ 0.08 at the leaves)
+    f0 = t.force(w.r_out, w.r_in, 0.4)
+    f1 = t.force(w.r_out, w.r_in, 0.4, r_list=r_list)
+    assert np.all(f1["npp"] >= f0["npp"]) and f1["npp"].sum() > f0["npp"].sum()      # more leaves opened
+    d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
+    err = np.linalg.norm(f1["acc_pot"][:, :3] - d["acc_reg"], axis=1) / np.linalg.norm(d["acc_reg"], axis=1)
+    assert np.median(err) < 2e-4 and np.percentile(err, 99) < 2e-2
+    # completeness: for a few groups, every brute-force neighbour within r_list is on the group's p-p list
+    g = t.groups(); keys, order = t.keys()
+    ooff, oidx = oracle.neighbours(w.pos_mass, r_list)
+    inv = np.empty(w.n, np.int64); inv[order] = np.arange(w.n)
+    import ctypes as C
+    for gid in (0, 7, len(g["begin"]) // 2, len(g["begin"]) - 1):
+        # the oracle does not export the lists; rebuild the p-p list of the group with the exported opening test
+        nodes, mom = t.nodes(), t.moments()
+        lo, side = t.cube()
+        pp = []
+        stack = [0]
+        while stack:
+            k = stack.pop()
+            l = side / 2.0 ** int(nodes["level"][k])
+            if oracle.open_test(g["glo"][gid], g["ghi"][gid], mom["com_m"][k, :3], mom["clo"][k], mom["chi"][k],
+                                l, mom["delta"][k], 0.4, r_list):
+                if nodes["n_child"][k] == 0:
+                    pp.extend(range(nodes["begin"][k], nodes["end"][k]))
+                else:
+                    stack.extend(range(nodes["first_child"][k], nodes["first_child"][k] + nodes["n_child"][k]))
+        pp = set(pp)
+        assert len(pp) == f1["npp"][gid]
+        for s in range(g["begin"][gid], g["end"][gid]):
+            i = int(order[s])
+            assert all(int(inv[j]) in pp for j in oidx[ooff[i]:ooff[i + 1]])
+    # theta -> 0
+    pm = _small(1024, scale=0.3)
+    ts = oracle.Tree(pm, 63, NLEAF, NCRIT)
+    fs = ts.force(0.05, 0.005, 1e-3, r_list=0.08)
+    ds = oracle.direct(pm, float(np.float32(0.05)), float(np.float32(0.005)))
+    assert np.abs(fs["acc_pot"][:, :3] - ds["acc_reg"]).max() < 1e-11 * np.abs(ds["acc_reg"]).max()
