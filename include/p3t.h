@@ -95,6 +95,17 @@ int p3t_build_tree(p3t_ctx* ctx, int64_t n, const float* pos_mass, int key_bits)
  * calls without a rebuild.  Also produces the neighbour lists returned by p3t_neighbours. */
 int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float* acc_pot);
 
+/* p3t_regular_force with the neighbour search reaching r_list = r_out + r_buff
+ * (PAPER.md:113, section 2.3: R_cut = R_s + R_buff; eq. 20, :156: r_buff = 3 tau sigma) and the leapfrog
+ * half-kick of eq. 12 fused into the epilogue of the force kernel:
+ *     L(i) = { j != i : r_ij < r_list },  r_list = fl32(r_out + r_buff)   (the cutoff stays at r_in, r_out:
+ *     list members with r >= r_out contribute wholly to F_R and nothing to F_I);
+ *     vel_i += half_dt * F_R,i   (one fma per component on the fp32 acceleration that is returned).
+ * r_buff >= 0.  vel: DEVICE pointer, n x {vx, vy, vz, unused} fp32, ORIGINAL order, 16-byte aligned,
+ * updated in place; NULL = no kick.  Everything else as p3t_regular_force (= r_buff 0, vel NULL). */
+int p3t_regular_force_ex(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                         float half_dt, float* vel, float* acc_pot);
+
 /* irregular force, jerk and potential over the neighbour lists of the last
  * p3t_regular_force (same r_out, r_in), eq. 1, 2, 5, 7 (the paper's CUTOFF / cutoff0
  * routines, :396-398):  F_I = sum_{j in L(i)} m_j K d / r^3,  Fdot_I = its exact time derivative

@@ -22,7 +22,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4, -5
 # every symbol include/p3t.h declares
 SYMBOLS = [
     "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_build_tree", "p3t_regular_force",
-    "p3t_irregular_force", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
+    "p3t_regular_force_ex", "p3t_irregular_force", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
 ]
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
     L.p3t_set_tree_params.argtypes = [vp, C.c_int, C.c_int]
     L.p3t_build_tree.argtypes = [vp, i64, vp, C.c_int]
     L.p3t_regular_force.argtypes = [vp, f32, f32, f32, C.c_int, vp]
+    L.p3t_regular_force_ex.argtypes = [vp, f32, f32, f32, C.c_int, f32, f32, vp, vp]
     L.p3t_irregular_force.argtypes = [vp, vp, vp, vp]
     L.p3t_neighbours.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
     L.p3t_neighbours_copy.argtypes = [vp, vp, vp]
@@ -166,12 +167,20 @@ class Context:
         self.n = int(pos_mass.shape[0])
         self._check(lib().p3t_build_tree(self._h, self.n, self._dev_f32(pos_mass, 4), key_bits), "p3t_build_tree")
 
-    def regular_force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, out=None):
-        """Returns acc_pot: CUDA float32 [n, 4] = ax, ay, az, phi in original particle order."""
+    def regular_force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, out=None,
+                      r_buff: float = 0.0, half_dt: float = 0.0, vel=None):
+        """Returns acc_pot: CUDA float32 [n, 4] = ax, ay, az, phi in original particle order.
+        r_buff > 0: neighbour lists reach r_out + r_buff; vel (CUDA float32 [n, 4]) is kicked in place by
+        half_dt * F_R."""
         torch = self._torch
         if out is None:
             out = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
-        self._check(lib().p3t_regular_force(self._h, r_out, r_in, theta, pot_mode, self._dev_f32(out, 4)), "p3t_regular_force")
+        if r_buff == 0.0 and vel is None:
+            self._check(lib().p3t_regular_force(self._h, r_out, r_in, theta, pot_mode, self._dev_f32(out, 4)), "p3t_regular_force")
+        else:
+            pv = None if vel is None else self._dev_f32(vel, 4)
+            self._check(lib().p3t_regular_force_ex(self._h, r_out, r_in, theta, pot_mode, r_buff, half_dt, pv, self._dev_f32(out, 4)),
+                        "p3t_regular_force_ex")
         return out
 
     def irregular_force(self, vel, acc_out=None, jerk_out=None):

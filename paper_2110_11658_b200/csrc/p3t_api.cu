@@ -134,21 +134,29 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     return P3T_OK;
 }
 
-int p3t_regular_force(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float* acc_pot)
+int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                         float half_dt, float* vel, float* acc_pot)
 {
     if (!c || !acc_pot) return P3T_EINVAL;
     if (!(r_in >= 0.0f) || !(r_in < r_out) || !(theta > 0.0f) || !isfinite(r_out) || !isfinite(theta)) return P3T_EINVAL;
+    if (!(r_buff >= 0.0f) || !isfinite(r_buff) || !isfinite(half_dt)) return P3T_EINVAL;
     if (pot_mode != 0 && pot_mode != 1) return P3T_EINVAL;
-    if (((uintptr_t)acc_pot & 15u) != 0) return P3T_EINVAL;
+    if (((uintptr_t)acc_pot & 15u) != 0 || ((uintptr_t)vel & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
     if (c->state < 1) return P3T_ESTATE;
     P3T_CUDA(c, cudaSetDevice(c->device));
     c->nb_valid = 0; c->irr_done = 0;
-    c->r_out = r_out; c->r_in = r_in; c->theta = theta;
-    int rc = p3t_launch_force(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot);
+    volatile float rl = r_out + r_buff;                        // one fp32 sum: the list radius of DESIGN.md section 10
+    c->r_out = r_out; c->r_in = r_in; c->theta = theta; c->r_list = rl;
+    int rc = p3t_launch_force(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot, rl, half_dt, (float4*)vel);
     if (rc != P3T_OK) return rc;
     c->state = 2; c->nb_valid = 1;
     return P3T_OK;
+}
+
+int p3t_regular_force(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float* acc_pot)
+{
+    return p3t_regular_force_ex(c, r_out, r_in, theta, pot_mode, 0.0f, 0.0f, nullptr, acc_pot);
 }
 
 int p3t_irregular_force(p3t_ctx* c, const float* vel, float* acc_irr, float* jerk_irr)

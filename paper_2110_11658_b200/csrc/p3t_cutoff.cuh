@@ -6,6 +6,7 @@
 
 struct walk_consts {
     float rout2, rin2, r_in, inv_delta;   // inv_delta = 1 / (r_out - r_in)
+    float rlist2;                          // neighbour search radius squared, r_list = r_out + r_buff >= r_out (NEXT-2)
     float psi_in;                          // psi(r_in), the constant regular pair potential inside r_in
     float k140;                            // 140 / (r_out - r_in)
     float s1;                              // S(1)
@@ -47,8 +48,11 @@ __device__ __forceinline__ float cutoff_psi64(const walk_consts& K, float xf, fl
     return (float)(-(double)W * (double)rinv - K.dk140 * integral);
 }
 
-static inline void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode)
+static inline void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode, float r_list = -1.0f)
 {
+    if (!(r_list >= r_out)) r_list = r_out;
+    volatile float rl2 = r_list * r_list;
+    K.rlist2 = rl2;
     // fp32 thresholds exactly as DESIGN.md R10 states them: one fp32 product each
     volatile float ro2 = r_out * r_out, ri2 = r_in * r_in;
     K.rout2 = ro2; K.rin2 = ri2; K.r_in = r_in;

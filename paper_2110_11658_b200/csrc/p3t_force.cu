@@ -31,6 +31,8 @@ struct force_args {
     const int64_t* nboff;       // per ORIGINAL id
     int32_t* nbraw;             // out: unsorted rows
     float4* out;                // out: acc_pot, original order
+    float4* vel;                // in/out (may be NULL): velocities, original order, kicked by half_dt * F_R (eq. 12)
+    float half_dt;
     p3t_devinfo* info;
     walk_consts K;
 };
@@ -137,15 +139,15 @@ __device__ __forceinline__ void eval_pc(target& T, const float (*pc)[TILE], int 
 
 // Two sources per packed operation: the far zone (d2 >= r_out^2, W = 1, pure Newtonian) of the
 // p-p list, branch-free.  d2 follows R10 bit for bit (sub, mul, fma, fma; all rn).  A near pair is
-// masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
+// (d2 < r_list^2, the neighbour search radius) masked out by replacing its d2 with +inf (rsqrt -> 0, every term exactly 0); the smallest d2 seen
 // by the lane is returned so that the caller knows whether the tile needs the near pass.
-__device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 pm, float rout2, float dmin)
+__device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 pm, float rlist2, float dmin)
 {
     const f2 dx = sub2(px, pk(T.x, T.x)), dy = sub2(py, pk(T.y, T.y)), dz = sub2(pz, pk(T.z, T.z));
     const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
     const float d2a = f2lo(d2), d2b = f2hi(d2);
     dmin = fminf(dmin, fminf(d2a, d2b));
-    const f2 ri = pk(rsqrt_approx(d2a < rout2 ? INFINITY : d2a), rsqrt_approx(d2b < rout2 ? INFINITY : d2b));
+    const f2 ri = pk(rsqrt_approx(d2a < rlist2 ? INFINITY : d2a), rsqrt_approx(d2b < rlist2 ? INFINITY : d2b));
     const f2 mri = mul2(pm, ri);
     const f2 f = mul2(mri, mul2(ri, ri));
     T.ph = add2(T.ph, mri);
@@ -171,12 +173,16 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
         for (int e = e0; e < e0 + 4; ++e) {
             const float dx = __fsub_rn(pp[0][e], T.x), dy = __fsub_rn(pp[1][e], T.y), dz = __fsub_rn(pp[2][e], T.z);
             const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
-            if (d2 < K.rout2) {
+            if (d2 < K.rlist2) {
                 const int j = ppj[e];
                 if (T.id >= 0 && j != T.id) {                        // self excluded by index; idle lanes
                     A.nbraw[rowbase + atomicAdd(&nbrow[T.slot], 1)] = (int32_t)A.order[j];
                     const float m = pp[3][e];
-                    if (d2 > K.rin2) {
+                    if (d2 >= K.rout2) {                               // buffer shell r_out <= r < r_list: on the list, wholly regular
+                        const float ri = rsqrt_approx(d2), mr = m * ri, f = mr * ri * ri;
+                        T.nax = fmaf(f, dx, T.nax); T.nay = fmaf(f, dy, T.nay); T.naz = fmaf(f, dz, T.naz);
+                        T.nph -= mr;
+                    } else if (d2 > K.rin2) {
                         const float ri = rsqrt_approx(d2), r = d2 * ri;
                         const float x = fminf(fmaxf((r - K.r_in) * K.inv_delta, 0.0f), 1.0f);
                         const float W = cutoff_W(x);
@@ -203,9 +209,9 @@ __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], cons
         ulonglong2 v[4];
 #pragma unroll
         for (int r = 0; r < 4; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pp[r][e]);
-        float dmin = pp_far_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rout2, INFINITY);
-        dmin = pp_far_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rout2, dmin);
-        if (dmin < A.K.rout2) nearblocks |= 1u << (e >> 2);
+        float dmin = pp_far_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, A.K.rlist2, INFINITY);
+        dmin = pp_far_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, A.K.rlist2, dmin);
+        if (dmin < A.K.rlist2) nearblocks |= 1u << (e >> 2);
     }
     if (!__any_sync(0xffffffffu, nearblocks != 0)) return;
     pp_near_pass(T, pp, ppj, nearblocks, rowbase, nbrow, A);
@@ -323,7 +329,15 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
         T.daz += shfl_xor_double(T.daz, o); T.dph += shfl_xor_double(T.dph, o);
     }
     // ---- a11: results to the caller's order ----
-    if (v && part == 0) A.out[orig] = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
+    if (v && part == 0) {
+        const float4 a = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
+        A.out[orig] = a;
+        if (A.vel) {                            // eq. 12: xdot += (dt_reg / 2) F_R, one fma per component
+            float4 u = A.vel[orig];
+            u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
+            A.vel[orig] = u;
+        }
+    }
 }
 
 // Work items: the c <= 64 targets of a group are cut into chunks of 32, 32, 16 and c mod 16 targets,
@@ -458,7 +472,8 @@ __global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict
 }
 
 
-int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot)
+int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
+                     float r_list, float half_dt, float4* vel)
 {
     const int n = (int)ctx->n;
     static int per_sm = 0;
@@ -474,7 +489,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
 
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
     // a10, sizes: neighbour counts (range search only) -> CSR offsets, so that the lists can be written in place
-    if ((rc = p3t_launch_walk_count(ctx, r_out, theta))) return rc;
+    if ((rc = p3t_launch_walk_count(ctx, r_list, theta))) return rc;
     k_nb_blocksum<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), INFO(ctx));
     k_nb_scansums<<<1, 1024, 0, ctx->stream>>>(P<long long>(ctx->nbcur), nsb, P<long long>(ctx->nboff) + n, INFO(ctx));
     k_nb_offsets<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), P<long long>(ctx->nboff));
@@ -482,7 +497,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     ctx->launches += 3;
     // a7: interaction lists
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
-    if ((rc = p3t_launch_walk_lists(ctx, r_out, theta))) return rc;
+    if ((rc = p3t_launch_walk_lists(ctx, r_list, theta))) return rc;
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
     // the one host synchronisation of this call: the neighbour total sizes the list buffers, and the
     // walk reports whether its list pools were large enough (if not it is repeated, normally only on
@@ -496,7 +511,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
         ctx->pool_cap_pc = (((long long)h.need_pc + h.need_pc / 4 + 16384) + 31) & ~31ll;
         ctx->pool_cap_pp = (((long long)h.need_pp + h.need_pp / 4 + 16384) + 31) & ~31ll;
         P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
-        if ((rc = p3t_launch_walk_lists(ctx, r_out, theta))) return rc;
+        if ((rc = p3t_launch_walk_lists(ctx, r_list, theta))) return rc;
         P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
     }
     const long long total = (long long)h.nb_total;
@@ -512,7 +527,8 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.pcpool = P<int32_t>(ctx->pcpool); A.pppool = P<int32_t>(ctx->pppool);
     A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
     A.out = acc_pot; A.info = INFO(ctx);
-    make_consts(A.K, r_out, r_in, theta, pot_mode);
+    make_consts(A.K, r_out, r_in, theta, pot_mode, r_list);
+    A.vel = vel; A.half_dt = half_dt;
     // a8, a9, a11: the force kernel
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
     k_force<<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);

@@ -79,7 +79,7 @@ struct p3t_ctx {
     cudaEvent_t evi[2];              // irregular-force kernel begin/end
     int irr_done;
     p3t_stats last;
-    float r_out, r_in, theta;
+    float r_out, r_in, theta, r_list;
     int64_t launches;                // kernels launched so far
 };
 
@@ -104,9 +104,10 @@ int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
 // p3t_walk.cu : a7 (interaction lists), a10 (neighbour counts)
 int p3t_walk_init(p3t_ctx* ctx);
-int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta);
-int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta);
+int p3t_launch_walk_count(p3t_ctx* ctx, float r_list, float theta);   // r_list: neighbour search radius (>= r_out)
+int p3t_launch_walk_lists(p3t_ctx* ctx, float r_list, float theta);
 // p3t_irregular.cu : SURVEY 8f NEXT-1
 int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk);
 // p3t_force.cu : a8-a11
-int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot);
+int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
+                     float r_list, float half_dt, float4* vel);

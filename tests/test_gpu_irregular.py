@@ -113,3 +113,54 @@ def test_state_and_arguments(p3t):
         # zero velocities: zero jerk, same acceleration
         a0, j0 = ctx.irregular_force(torch.zeros_like(vel))
         assert torch.equal(a0, a1) and torch.count_nonzero(j0) == 0
+
+
+# ---- buffered search radius and the fused leapfrog half-kick ----
+def test_buffered_lists_and_kick(p3t):
+    """r_list = r_out + r_buff: neighbour CSR bit-exact against brute force at r_list, interaction lists and
+    force against the oracle tree with the widened opening clause; eq. 12 kick = one fma on the returned a."""
+    import torch
+    w = workloads.make_config(1)
+    r_buff = float(np.float32(3.0 * w.r_out))                       # large enough for the clause to bite
+    r_list = float(np.float32(w.r_out) + np.float32(r_buff))
+    vel = workloads.velocities_for(w)
+    half_dt = float(np.float32(1.0 / 256.0))
+    T = oracle.Tree(w.pos_mass, 63, 16, 64)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        v_dev = _cuda(vel)
+        out = ctx.regular_force(w.r_out, w.r_in, w.theta, 0, r_buff=r_buff, half_dt=half_dt, vel=v_dev)
+        a32 = out.cpu().numpy()
+        a = a32.astype(np.float64)
+        npp, npc = ctx.list_lengths()
+        off, idx = ctx.neighbours()
+        off = off.cpu().numpy(); idx = idx.cpu().numpy()
+        f = T.force(w.r_out, w.r_in, w.theta, 0, want_abs=True, r_list=r_list)
+        assert np.array_equal(npp, f["npp"]) and np.array_equal(npc, f["npc"]), "interaction lists differ"
+        ref = f["acc_pot"]
+        assert np.linalg.norm(a[:, :3] - ref[:, :3]) <= 1e-6 * np.linalg.norm(ref[:, :3])
+        assert np.all(np.linalg.norm(a[:, :3] - ref[:, :3], axis=1) <= 1e-6 * f["abs_sum"] + 1e-30)
+        assert np.all(np.abs(a[:, 3] - ref[:, 3]) <= 2e-6 * np.abs(ref[:, 3]))
+        ooff, oidx = oracle.neighbours(w.pos_mass, r_list)
+        assert np.array_equal(ooff, off) and np.array_equal(oidx, idx), "buffered neighbour CSR differs"
+        o0, _ = oracle.neighbours(w.pos_mass, w.r_out)
+        assert off[-1] > 5 * o0[-1]                                  # the buffer shell is populated
+        # kick: v' = fma(half_dt, a, v) in fp32; exact product + one rounding, emulated in fp64 (the product
+        # of two fp32 is exact in fp64; the sum may round twice: allow 1 ulp)
+        v1 = v_dev.cpu().numpy()
+        want = (np.float64(half_dt) * a32[:, :3].astype(np.float64) + vel[:, :3].astype(np.float64)).astype(np.float32)
+        ulp = np.spacing(np.abs(want))
+        assert np.all(np.abs(v1[:, :3] - want) <= ulp) and np.mean(v1[:, :3] == want) > 0.999
+        assert np.array_equal(v1[:, 3], vel[:, 3])
+        # the irregular force over the buffered lists: shell members (r >= r_out) contribute nothing
+        acc, jerk = ctx.irregular_force(_cuda(vel))
+        o = oracle.irregular(w.pos_mass, vel, w.r_out, w.r_in)
+        acc = acc.cpu().numpy().astype(np.float64); jerk = jerk.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(acc[:, :3] - o["acc_irr"]) <= 1e-6 * np.linalg.norm(o["acc_irr"])
+        assert np.all(np.linalg.norm(jerk[:, :3] - o["jerk_irr"], axis=1) <= 2e-6 * o["abs_jerk"] + 1e-6 * o["abs_newt"] + 1e-30)
+        # r_buff = 0 through the _ex entry point is p3t_regular_force
+        b0 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0)
+        b1 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0, r_buff=0.0, vel=torch.zeros_like(v_dev))
+        assert torch.equal(b0, b1)
+        with pytest.raises(p3t.P3TError):
+            ctx.regular_force(w.r_out, w.r_in, w.theta, 0, r_buff=-1.0, vel=v_dev)
