@@ -53,6 +53,10 @@ def lib() -> C.CDLL:
         _lib.p3t_o_direct.argtypes = [i64, vp, d, d, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_irregular.restype = i64
         _lib.p3t_o_irregular.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp, vp]
+        _lib.p3t_o_knn_density.restype = None
+        _lib.p3t_o_knn_density.argtypes = [i64, vp, i64, vp, C.c_int, vp, vp, vp]
+        _lib.p3t_o_core_quantities.restype = None
+        _lib.p3t_o_core_quantities.argtypes = [i64, vp, i64, vp, vp, vp]
         _lib.p3t_o_neighbours.restype = i64
         _lib.p3t_o_neighbours.argtypes = [i64, vp, f32, C.c_int, i64, vp, vp, vp]
         _lib.p3t_o_tree_build.restype = vp
@@ -131,6 +135,24 @@ def irregular(pos_mass, vel, r_out: float, r_in: float, targets=None):
     acc = np.zeros((nt, 3)); jerk = np.zeros((nt, 3)); phi = np.zeros(nt); ab = np.zeros(nt); an = np.zeros(nt)
     coinc = lib().p3t_o_irregular(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(acc), _p(jerk), _p(phi), _p(ab), _p(an))
     return dict(acc_irr=acc, jerk_irr=jerk, phi_irr=phi, abs_jerk=ab, abs_newt=an, coincident=int(coinc))
+
+
+def knn_density(pos_mass, sample, k: int = 6):
+    """K nearest neighbours of the sample particles (brute force, order (fp32 d2, index)) and their
+    Casertano-Hut densities: dict(nbr [ns,k] int32, d2k [ns] float32, rho [ns] float64)."""
+    pm = _pm(pos_mass); sm = np.ascontiguousarray(sample, dtype=np.int32)
+    ns = sm.shape[0]
+    nbr = np.zeros((ns, k), np.int32); d2k = np.zeros(ns, np.float32); rho = np.zeros(ns)
+    lib().p3t_o_knn_density(pm.shape[0], _p(pm), ns, _p(sm), int(k), _p(nbr), _p(d2k), _p(rho))
+    return dict(nbr=nbr, d2k=d2k, rho=rho)
+
+
+def core_quantities(pos_mass, sample, rho):
+    """dict(center [3], r_core, rho_core, n_core) from the sample densities (NBODY6 conventions)."""
+    pm = _pm(pos_mass); sm = np.ascontiguousarray(sample, dtype=np.int32)
+    r = np.ascontiguousarray(rho, dtype=np.float64); out = np.zeros(6)
+    lib().p3t_o_core_quantities(pm.shape[0], _p(pm), sm.shape[0], _p(sm), _p(r), _p(out))
+    return dict(center=out[:3].copy(), r_core=float(out[3]), rho_core=float(out[4]), n_core=float(out[5]))
 
 
 def neighbours(pos_mass, r_out: float, targets=None, fp32_predicate: bool = True):

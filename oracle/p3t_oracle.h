@@ -44,6 +44,13 @@ int64_t p3t_o_irregular(int64_t n, const float* pos_mass, const float* vel, doub
                         int64_t nt, const int64_t* targets,
                         double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt);
 
+/* sampled K-nearest-neighbour densities (Casertano & Hut 1985) and the core
+ * quantities built from them.  sample: ns original ids.  nbr[ns*K] (may be NULL),
+ * d2k[ns] fp32, rho[ns] fp64.  out[6] = density centre (3), R_core, rho_core, N_core. */
+void p3t_o_knn_density(int64_t n, const float* pos_mass, int64_t ns, const int32_t* sample, int K,
+                       int32_t* nbr, float* d2k, double* rho);
+void p3t_o_core_quantities(int64_t n, const float* pos_mass, int64_t ns, const int32_t* sample, const double* rho, double out[6]);
+
 /* Brute-force neighbour rows for nt targets.  fp32_predicate = 1: the bit-spec predicate
  * (R10); 0: the fp64 "physics" predicate r_ij < r_out.  counts[nt] is always written;
  * if indices != NULL rows are written back to back (ascending j) and must hold sum(counts). */

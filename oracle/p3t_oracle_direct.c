@@ -218,3 +218,71 @@ int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_o
     }
     return coincident;
 }
+
+/* core quantities by a sampled 6-nearest-neighbour search (section 2.5,
+ * :245 section 3.2.1: "takes a random sample of min(N, sqrt(5000 N)) particles, then performs a
+ * brute-force search for those particles' 6 nearest neighbours"; the estimator is Casertano & Hut 1985,
+ * which the paper cites and does not restate: readings R17-R19 of DESIGN.md).
+ *
+ * Step 1, per sample particle i (brute force over all j != i, by index):
+ *   the K nearest neighbours under the order (d2, j), d2 the fp32 squared distance of R10
+ *   (dx = fl(x_j - x_i) ..., d2 = fma(dz,dz,fma(dy,dy,fl(dx dx)))): an integer decision, so it is taken
+ *   in the kernel's precision on both sides; ties by the smaller original index;
+ *   rho_i = (sum of the masses of the K-1 nearest) / (4 pi / 3 r_K^3),  r_K = sqrt(d2_K) in fp64
+ *   (Casertano & Hut's unbiased estimator: the K-th neighbour and the particle itself are left out).
+ * Outputs: nbr[ns*K] original ids in ascending (d2, j), d2k[ns] fp32 d2 of the K-th, rho[ns] fp64. */
+void p3t_o_knn_density(int64_t n, const float* pm, int64_t ns, const int32_t* sample, int K,
+                       int32_t* nbr, float* d2k, double* rho)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t s = 0; s < ns; ++s) {
+        const int64_t i = sample[s];
+        const float xi = pm[4 * i], yi = pm[4 * i + 1], zi = pm[4 * i + 2];
+        float bd[64]; int32_t bj[64];
+        int cnt = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            const float dx = pm[4 * j] - xi, dy = pm[4 * j + 1] - yi, dz = pm[4 * j + 2] - zi;
+            const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (cnt == K && !(d2 < bd[K - 1])) continue;          /* j ascending: an equal d2 never displaces */
+            int p = cnt < K ? cnt++ : K - 1;
+            while (p > 0 && d2 < bd[p - 1]) { bd[p] = bd[p - 1]; bj[p] = bj[p - 1]; --p; }
+            bd[p] = d2; bj[p] = (int32_t)j;
+        }
+        double m = 0.0;
+        for (int q = 0; q < K; ++q) { if (nbr) nbr[s * K + q] = q < cnt ? bj[q] : -1; if (q < K - 1 && q < cnt) m += (double)pm[4 * (int64_t)bj[q] + 3]; }
+        const double rk = cnt == K ? sqrt((double)bd[K - 1]) : 0.0;
+        if (d2k) d2k[s] = cnt == K ? bd[K - 1] : INFINITY;
+        if (rho) rho[s] = rk > 0.0 ? m / (4.0 * M_PI / 3.0 * rk * rk * rk) : 0.0;
+    }
+}
+
+/* Step 2, over the sample (fp64, index order): density centre, core radius, core density, core number
+ * (NBODY6's conventions, reading R18):
+ *   x_d = sum rho_i x_i / sum rho_i;  R_core^2 = sum rho_i^2 |x_i - x_d|^2 / sum rho_i^2;
+ *   rho_core = sum rho_i^2 / sum rho_i;  N_core = (N / ns) * #{ sample i : |x_i - x_d| < R_core }  (R19).
+ * out[6] = x_d (3), R_core, rho_core, N_core. */
+void p3t_o_core_quantities(int64_t n, const float* pm, int64_t ns, const int32_t* sample, const double* rho, double out[6])
+{
+    double sr = 0, sr2 = 0, c[3] = { 0, 0, 0 };
+    for (int64_t s = 0; s < ns; ++s) {
+        const float* p = pm + 4 * (int64_t)sample[s];
+        sr += rho[s]; sr2 += rho[s] * rho[s];
+        for (int a = 0; a < 3; ++a) c[a] += rho[s] * (double)p[a];
+    }
+    for (int a = 0; a < 3; ++a) c[a] /= sr;
+    double q = 0;
+    for (int64_t s = 0; s < ns; ++s) {
+        const float* p = pm + 4 * (int64_t)sample[s];
+        double d2 = 0; for (int a = 0; a < 3; ++a) d2 += ((double)p[a] - c[a]) * ((double)p[a] - c[a]);
+        q += rho[s] * rho[s] * d2;
+    }
+    const double rc = sqrt(q / sr2);
+    int64_t inside = 0;
+    for (int64_t s = 0; s < ns; ++s) {
+        const float* p = pm + 4 * (int64_t)sample[s];
+        double d2 = 0; for (int a = 0; a < 3; ++a) d2 += ((double)p[a] - c[a]) * ((double)p[a] - c[a]);
+        inside += d2 < rc * rc;
+    }
+    out[0] = c[0]; out[1] = c[1]; out[2] = c[2]; out[3] = rc; out[4] = sr2 / sr; out[5] = (double)inside * (double)n / (double)ns;
+}
