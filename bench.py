@@ -211,6 +211,15 @@ def run_ours(args, w, rank, world, local_rank, dist):
         irr_ms.append(ctx.stats()["ms_irregular"])
     irr_ms = float(np.median(irr_ms[1:]))
 
+    # ---- SURVEY 8f NEXT-3 (outside the step): sampled 6-NN core quantities, the paper's sample size ----
+    ns = int(min(n, np.sqrt(5000.0 * n)))
+    sample_dev = torch.from_numpy(workloads.sample_targets(n, ns).astype(np.int32)).to(dev)
+    core_ms = []
+    for k in range(5):
+        core = ctx.core_quantities(sample_dev, 6)
+        core_ms.append(ctx.stats()["ms_core"])
+    core_ms = float(np.median(core_ms[1:]))
+
     # ---- end-to-end arm: HOST buffers through p3t_step_host ----
     pm_host = torch.from_numpy(w.pos_mass).pin_memory()
     acc_host = torch.empty((n, 4), dtype=torch.float32).pin_memory()
@@ -272,6 +281,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
                 "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n + 8 * (n + 1) + 4 * int(nb_total)},
         "next1_irregular": {"ms": irr_ms, "list_entries_per_s": st["nb_total"] / (irr_ms * 1e-3) if irr_ms > 0 else None,
                             "note": "p3t_irregular_force (F_I, jerk, phi_I over the neighbour lists); not part of the timed step"},
+        "next3_core": {"ms": core_ms, "sample": ns, "k": 6, "r_core": core["r_core"], "rho_core": core["rho_core"], "n_core": core["n_core"],
+                       "note": "p3t_core_quantities (k-NN on the octree + Casertano-Hut reductions); not part of the timed step"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
     }
     if world == 1 and not args.no_cpu_baseline:

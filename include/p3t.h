@@ -67,6 +67,7 @@ typedef struct p3t_stats {
     float   ms_eval;         /* ... of the force kernel (a8, a9, a11) alone             */
     float   ms_count;        /* ... of the neighbour count walk + offset scan (a10)     */
     float   ms_irregular;    /* ... of the last p3t_irregular_force kernel (0 if none)  */
+    float   ms_core;         /* ... of the last p3t_core_quantities kernels (0 if none)  */
     int64_t launches;        /* kernels this context has launched since p3t_create      */
 } p3t_stats;
 
@@ -105,6 +106,20 @@ int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int po
  * updated in place; NULL = no kick.  Everything else as p3t_regular_force (= r_buff 0, vel NULL). */
 int p3t_regular_force_ex(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float r_buff,
                          float half_dt, float* vel, float* acc_pot);
+
+/* core quantities by a sampled k-nearest-neighbour search (PAPER.md:134, :245:
+ * "a random sample of min(N, sqrt(5000 N)) particles, then ... those particles' 6 nearest neighbours";
+ * estimator of Casertano & Hut 1985 as cited there; R17-R19).  The search runs on the octree
+ * of the last p3t_build_tree and returns exactly the brute-force neighbours under the order
+ * (fp32 squared distance of R10, original index).
+ * sample: DEVICE pointer, ns original ids (the caller draws the random sample); 2 <= k <= 16 (paper: 6).
+ * nbr: DEVICE, ns x k int32 original ids, ascending in that order (may be NULL); d2k: DEVICE, ns fp32,
+ * squared distance of the k-th neighbour; rho: DEVICE, ns fp64, (sum of the masses of the k-1 nearest) /
+ * (4 pi / 3 r_k^3).  core_out: HOST double[6] = density centre sum rho x / sum rho (3), R_core =
+ * sqrt(sum rho^2 |x - x_d|^2 / sum rho^2), rho_core = sum rho^2 / sum rho, N_core = (n / ns) x the
+ * number of sample particles within R_core of the centre.  Requires a prior build.  Synchronises. */
+int p3t_core_quantities(p3t_ctx* ctx, int64_t ns, const int32_t* sample, int k, int32_t* nbr, float* d2k, double* rho,
+                        double* core_out);
 
 /* irregular force, jerk and potential over the neighbour lists of the last
  * p3t_regular_force (same r_out, r_in), eq. 1, 2, 5, 7 (the paper's CUTOFF / cutoff0

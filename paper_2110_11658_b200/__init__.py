@@ -22,7 +22,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4, -5
 # every symbol include/p3t.h declares
 SYMBOLS = [
     "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_build_tree", "p3t_regular_force",
-    "p3t_regular_force_ex", "p3t_irregular_force", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
+    "p3t_regular_force_ex", "p3t_irregular_force", "p3t_core_quantities", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
 ]
@@ -36,7 +36,7 @@ class Stats(C.Structure):
         ("nb_total", C.c_int64), ("nb_max", C.c_int32), ("input_bad", C.c_int32),
         ("cube_lo", C.c_float * 3), ("cube_side", C.c_float),
         ("ms_build", C.c_float), ("ms_force", C.c_float), ("ms_walk", C.c_float), ("ms_sort", C.c_float),
-        ("ms_eval", C.c_float), ("ms_count", C.c_float), ("ms_irregular", C.c_float),
+        ("ms_eval", C.c_float), ("ms_count", C.c_float), ("ms_irregular", C.c_float), ("ms_core", C.c_float),
         ("launches", C.c_int64),
     ]
 
@@ -74,6 +74,7 @@ def lib() -> C.CDLL:
     L.p3t_regular_force.argtypes = [vp, f32, f32, f32, C.c_int, vp]
     L.p3t_regular_force_ex.argtypes = [vp, f32, f32, f32, C.c_int, f32, f32, vp, vp]
     L.p3t_irregular_force.argtypes = [vp, vp, vp, vp]
+    L.p3t_core_quantities.argtypes = [vp, i64, vp, C.c_int, vp, vp, vp, vp]
     L.p3t_neighbours.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
     L.p3t_neighbours_copy.argtypes = [vp, vp, vp]
     L.p3t_neighbours_nbody6.argtypes = [vp, i32, vp]
@@ -195,6 +196,21 @@ class Context:
         self._check(lib().p3t_irregular_force(self._h, self._dev_f32(vel, 4), self._dev_f32(acc_out, 4), self._dev_f32(jerk_out, 4)),
                     "p3t_irregular_force")
         return acc_out, jerk_out
+
+    def core_quantities(self, sample, k: int = 6):
+        """Sampled k-NN densities and core quantities.  sample: CUDA int32 [ns] original ids.
+        Returns dict(nbr int32 [ns, k], d2k float32 [ns], rho float64 [ns] (CUDA tensors), center [3], r_core,
+        rho_core, n_core)."""
+        torch = self._torch
+        assert sample.is_cuda and sample.dtype == torch.int32 and sample.is_contiguous()
+        ns = int(sample.shape[0])
+        nbr = torch.empty((ns, k), dtype=torch.int32, device=self.device)
+        d2k = torch.empty(ns, dtype=torch.float32, device=self.device)
+        rho = torch.empty(ns, dtype=torch.float64, device=self.device)
+        out = (C.c_double * 6)()
+        self._check(lib().p3t_core_quantities(self._h, ns, sample.data_ptr(), k, nbr.data_ptr(), d2k.data_ptr(), rho.data_ptr(), out),
+                    "p3t_core_quantities")
+        return dict(nbr=nbr, d2k=d2k, rho=rho, center=[out[0], out[1], out[2]], r_core=out[3], rho_core=out[4], n_core=out[5])
 
     def neighbours(self):
         """(offsets int64 [n+1], indices int32 [total]) as CUDA tensors (copied from the library's buffers)."""

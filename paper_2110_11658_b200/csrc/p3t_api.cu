@@ -60,6 +60,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evw[k]);
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evi[k]);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evc[k]);
     if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
     int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
     if (rc == P3T_OK) rc = p3t_tree_init(c);
@@ -77,11 +78,12 @@ int p3t_destroy(p3t_ctx* c)
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->spill, &c->pcpool, &c->pppool, &c->glist,
-                        &c->info, &c->stage_in, &c->stage_out };
+                        &c->info, &c->stage_in, &c->stage_out, &c->core };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
     for (int k = 0; k < 2; ++k) if (c->evi[k]) cudaEventDestroy(c->evi[k]);
+    for (int k = 0; k < 2; ++k) if (c->evc[k]) cudaEventDestroy(c->evc[k]);
     (void)cudaGetLastError();
     delete c;
     return P3T_OK;
@@ -100,7 +102,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     if (((uintptr_t)pos_mass & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
     P3T_CUDA(c, cudaSetDevice(c->device));
-    c->state = 0; c->nb_valid = 0; c->irr_done = 0;
+    c->state = 0; c->nb_valid = 0; c->irr_done = 0; c->core_done = 0;
     c->n = n; c->key_bits = key_bits; c->bits = key_bits / 3;
     // hard bound on the cell count (data layout): leaves <= n, branching cells < n,
     // one-child chain cells <= levels * n / (nleaf + 1)
@@ -172,6 +174,23 @@ int p3t_irregular_force(p3t_ctx* c, const float* vel, float* acc_irr, float* jer
     return P3T_OK;
 }
 
+int p3t_core_quantities(p3t_ctx* c, int64_t ns, const int32_t* sample, int k, int32_t* nbr, float* d2k, double* rho,
+                        double* core_out)
+{
+    if (!c || !sample || !d2k || !rho || !core_out || ns < 1 || ns > 0x7fffffff || k < 2 || k > 16) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    if (c->state < 1) return P3T_ESTATE;
+    if (c->n <= k) return P3T_EINVAL;                      // fewer than k other particles
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    int rc = p3t_reserve(c, &c->core, 64);
+    if (rc != P3T_OK) return rc;
+    if ((rc = p3t_launch_core(c, ns, sample, k, nbr, d2k, rho, (double*)c->core.p)) != P3T_OK) return rc;
+    c->core_done = 1;
+    P3T_CUDA(c, cudaMemcpyAsync(core_out, c->core.p, 6 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    P3T_CUDA(c, cudaStreamSynchronize(c->stream));
+    return P3T_OK;
+}
+
 static int sync_and_check(p3t_ctx* c, p3t_devinfo* h)
 {
     P3T_CUDA(c, cudaSetDevice(c->device));
@@ -211,6 +230,9 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         (void)cudaEventElapsedTime(&out->ms_walk, c->evw[2], c->evw[3]);
         (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->evw[2]);
         if (c->irr_done) (void)cudaEventElapsedTime(&out->ms_irregular, c->evi[0], c->evi[1]);
+    }
+    if (c->core_done) {
+        (void)cudaEventElapsedTime(&out->ms_core, c->evc[0], c->evc[1]);
     }
     (void)cudaGetLastError();
     return rc;

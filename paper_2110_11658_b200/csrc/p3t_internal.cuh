@@ -77,6 +77,9 @@ struct p3t_ctx {
     cudaEvent_t ev[6];               // build begin/end, sort begin/end ... force begin/end, walk begin/end
     cudaEvent_t evw[4];
     cudaEvent_t evi[2];              // irregular-force kernel begin/end
+    cudaEvent_t evc[2];              // core-quantity kernels begin/end
+    p3t_buf core;                    // double[6]: result of k_core_reduce
+    int core_done;
     int irr_done;
     p3t_stats last;
     float r_out, r_in, theta, r_list;
@@ -106,6 +109,8 @@ int p3t_launch_tree(p3t_ctx* ctx);
 int p3t_walk_init(p3t_ctx* ctx);
 int p3t_launch_walk_count(p3t_ctx* ctx, float r_list, float theta);   // r_list: neighbour search radius (>= r_out)
 int p3t_launch_walk_lists(p3t_ctx* ctx, float r_list, float theta);
+// p3t_core.cu : SURVEY 8f NEXT-3
+int p3t_launch_core(p3t_ctx* ctx, int64_t ns, const int32_t* sample, int K, int32_t* nbr, float* d2k, double* rho, double* core_dev);
 // p3t_irregular.cu : SURVEY 8f NEXT-1
 int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk);
 // p3t_force.cu : a8-a11
