@@ -260,7 +260,7 @@ __global__ void k_walk_reset(p3t_devinfo* info, int mode)
     }
 }
 
-static int walk_blocks(p3t_ctx* ctx, int mode, int* out)
+static int walk_blocks(p3t_ctx* ctx, int mode, int* out, bool limit_by_n = true)
 {
     static int per_sm[2] = { 0, 0 };
     if (!per_sm[mode]) {
@@ -268,7 +268,11 @@ static int walk_blocks(p3t_ctx* ctx, int mode, int* out)
         else                    P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], k_walk<WALK_LISTS>, WALK_THREADS, 0));
         if (per_sm[mode] < 1) per_sm[mode] = 1;
     }
-    *out = per_sm[mode] * ctx->num_sms;
+    // a persistent grid, but no more warps than there can be groups of >= 32 particles: every walker
+    // warp owns a private region of the list pools, and idle warps would only inflate them
+    const long long by_n = limit_by_n ? (ctx->n / 32 + WALK_WARPS - 1) / WALK_WARPS : (1ll << 40);
+    const long long full = (long long)per_sm[mode] * ctx->num_sms;
+    *out = (int)(by_n < 1 ? 1 : by_n < full ? by_n : full);
     return P3T_OK;
 }
 
@@ -328,8 +332,8 @@ int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta)
 int p3t_walk_init(p3t_ctx* ctx)
 {
     int b0, b1, rc;
-    if ((rc = walk_blocks(ctx, WALK_COUNT, &b0))) return rc;
-    if ((rc = walk_blocks(ctx, WALK_LISTS, &b1))) return rc;
+    if ((rc = walk_blocks(ctx, WALK_COUNT, &b0, false))) return rc;
+    if ((rc = walk_blocks(ctx, WALK_LISTS, &b1, false))) return rc;
     ctx->walk_warps_max = (long long)(b0 > b1 ? b0 : b1) * WALK_WARPS;
     return P3T_OK;
 }
