@@ -19,6 +19,7 @@
 
 struct irr_args {
     const float4* spm; const int32_t* rank;     // sorted bodies, original id -> sorted position
+    const uint32_t* order;                      // sorted position -> original id
     const float4* vel;                          // original order
     const int64_t* nboff; const int32_t* nbidx; // CSR, original ids
     float4 *acc, *jerk;                         // original order
@@ -59,10 +60,12 @@ __device__ __forceinline__ void irr_term(const irr_args& A, const float4 pi, con
 
 __global__ void __launch_bounds__(256) k_irregular(irr_args A)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
-    long long b = 0; int len = 0;
+    // threads take the particles in Morton order: the rows of a warp are neighbours in space, so they
+    // have similar lengths and share most of their entries (L1 hits on spm / vel / rank)
+    const int sp = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    long long b = 0; int len = 0, i = 0;
     float4 pi = make_float4(0, 0, 0, 0), vi = pi;
-    if (i < A.n) { b = A.nboff[i]; len = (int)(A.nboff[i + 1] - b); pi = A.spm[A.rank[i]]; vi = A.vel[i]; }
+    if (sp < A.n) { i = (int)A.order[sp]; b = A.nboff[i]; len = (int)(A.nboff[i + 1] - b); pi = A.spm[sp]; vi = A.vel[i]; }
     irr_sum S = { 0, 0, 0, 0, 0, 0, 0 };
     if (len <= 32)
         for (int k = 0; k < len; ++k) irr_term(A, pi, vi, A.nbidx[b + k], S);
@@ -90,7 +93,7 @@ __global__ void __launch_bounds__(256) k_irregular(irr_args A)
             }
         if (lane == src) S = R;
     }
-    if (i < A.n) {
+    if (sp < A.n) {
         A.acc[i]  = make_float4((float)S.ax, (float)S.ay, (float)S.az, (float)S.ph);
         A.jerk[i] = make_float4((float)S.jx, (float)S.jy, (float)S.jz, 0.0f);
     }
@@ -99,7 +102,7 @@ __global__ void __launch_bounds__(256) k_irregular(irr_args A)
 int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk)
 {
     irr_args A;
-    A.spm = P<float4>(ctx->spm); A.rank = P<int32_t>(ctx->rank);
+    A.spm = P<float4>(ctx->spm); A.rank = P<int32_t>(ctx->rank); A.order = P<uint32_t>(ctx->idx[0]);
     A.vel = vel; A.nboff = P<int64_t>(ctx->nboff); A.nbidx = P<int32_t>(ctx->nbidx);
     A.acc = acc; A.jerk = jerk; A.n = (int)ctx->n;
     make_consts(A.K, ctx->r_out, ctx->r_in, ctx->theta, 0);
