@@ -31,6 +31,10 @@ struct force_args {
     const int64_t* nboff;       // per ORIGINAL id
     int32_t* nbraw;             // out: unsorted rows
     float4* out;                // out: acc_pot, original order
+    int32_t* nbcnt;             // SPLIT: per sorted position, neighbours already written to the row (zeroed)
+    double* part;               // SPLIT: partial sums [nseg][n][4], original order
+    int nseg;                   // SPLIT: list segments per item
+    int n;
     float4* vel;                // in/out (may be NULL): velocities, original order, kicked by half_dt * F_R (eq. 12)
     float half_dt;
     p3t_devinfo* info;
@@ -163,7 +167,7 @@ __device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 
 // (bit mask), run only by warps that have such a block in the tile (about one tile in eight).  nbrow[slot] counts the entries already written
 // to the target's CSR row (shared by the parts of a target).
 __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE], const int* ppj, uint32_t nearblocks,
-                                             long long rowbase, int* nbrow, const force_args& A)
+                                             long long rowbase, int* rowcnt, const force_args& A)
 {
     const walk_consts& K = A.K;
     while (nearblocks) {
@@ -176,7 +180,7 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
             if (d2 < K.rlist2) {
                 const int j = ppj[e];
                 if (T.id >= 0 && j != T.id) {                        // self excluded by index; idle lanes
-                    A.nbraw[rowbase + atomicAdd(&nbrow[T.slot], 1)] = (int32_t)A.order[j];
+                    A.nbraw[rowbase + atomicAdd(rowcnt, 1)] = (int32_t)A.order[j];
                     const float m = pp[3][e];
                     if (d2 >= K.rout2) {                               // buffer shell r_out <= r < r_list: on the list, wholly regular
                         const float ri = rsqrt_approx(d2), mr = m * ri, f = mr * ri * ri;
@@ -201,7 +205,7 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
 }
 
 __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
-                                        long long rowbase, int* nbrow, const force_args& A)
+                                        long long rowbase, int* rowcnt, const force_args& A)
 {
     uint32_t nearblocks = 0;                     // bit b: this lane's target came within r_out of block b
 #pragma unroll 1
@@ -214,7 +218,7 @@ __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], cons
         if (dmin < A.K.rlist2) nearblocks |= 1u << (e >> 2);
     }
     if (!__any_sync(0xffffffffu, nearblocks != 0)) return;
-    pp_near_pass(T, pp, ppj, nearblocks, rowbase, nbrow, A);
+    pp_near_pass(T, pp, ppj, nearblocks, rowbase, rowcnt, A);
 }
 
 // Software pipeline of the list stream: the ids of tile t+2 and the node / particle data of tile
@@ -258,8 +262,12 @@ __device__ __forceinline__ double shfl_xor_double(double v, int o)
     return __hiloint2double(hi, lo);
 }
 
-// targets [tb, te) (sorted positions, te - tb <= 32) of group g against the group's two lists
-__device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te)
+// targets [tb, te) (sorted positions, te - tb <= 32) of group g against the group's two lists.
+// SPLIT (small problems, fewer items than resident warps): the item is shared by nseg warps, warp
+// `seg` takes the tiles seg, seg + nseg, ... of both lists; the partial sums go to A.part and are
+// added in segment order by k_force_final (bit-reproducible), the row cursors are global.
+template <bool SPLIT>
+__device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te, int seg, int nseg)
 {
     const int lane = threadIdx.x & 31;
     const int c = te - tb;
@@ -277,25 +285,26 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     T.nax = T.nay = T.naz = T.nph = 0.0f;
     const uint32_t orig = v ? A.order[T.id] : 0u;
     const long long rowbase = v ? A.nboff[orig] : 0;
-    S.nbrow[lane] = 0;
+    int* rowcnt = SPLIT ? A.nbcnt + (v ? T.id : tb) : &S.nbrow[T.slot];
+    if (!SPLIT) S.nbrow[lane] = 0;
     const uint4 rec = A.glist[g];
     __syncwarp();
     // ---- a8: particle-cell list; a lane sees TILE / k cells per tile: fold every k tiles ----
     {
         const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
         const int n = (int)rec.y, nt = (n + TILE - 1) / TILE;
-        if (nt > 0) {
-            pc_regs r = gather_pc(A, load_id(ids, lane, n));
-            int idn = load_id(ids, TILE + lane, n);
+        if (seg < nt) {
+            pc_regs r = gather_pc(A, load_id(ids, seg * TILE + lane, n));
+            int idn = load_id(ids, (seg + nseg) * TILE + lane, n);
             store_pc(S.pc[0], lane, r);
             __syncwarp();
-            for (int t = 0; t < nt; ++t) {
-                const bool more = t + 1 < nt;
+            for (int t = seg, it = 0; t < nt; t += nseg, ++it) {
+                const bool more = t + nseg < nt;
                 if (more) r = gather_pc(A, idn);
-                idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pc(T, S.pc[t & 1], part, k);
-                if (((t + 1) & (k - 1)) == 0) fold(T);
-                if (more) store_pc(S.pc[(t + 1) & 1], lane, r);
+                idn = load_id(ids, (t + 2 * nseg) * TILE + lane, n);
+                eval_pc(T, S.pc[it & 1], part, k);
+                if (((it + 1) & (k - 1)) == 0) fold(T);
+                if (more) store_pc(S.pc[(it + 1) & 1], lane, r);
                 __syncwarp();
             }
             fold(T);
@@ -305,18 +314,18 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     {
         const int32_t* ids = A.pppool + ((long long)rec.z << 5);
         const int n = (int)rec.w, nt = (n + TILE - 1) / TILE;
-        if (nt > 0) {
-            pp_regs r = gather_pp(A, load_id(ids, lane, n));
-            int idn = load_id(ids, TILE + lane, n);
+        if (seg < nt) {
+            pp_regs r = gather_pp(A, load_id(ids, seg * TILE + lane, n));
+            int idn = load_id(ids, (seg + nseg) * TILE + lane, n);
             store_pp(S.pp[0], S.ppj[0], lane, r);
             __syncwarp();
-            for (int t = 0; t < nt; ++t) {
-                const bool more = t + 1 < nt;
-                const int b = t & 1;
+            for (int t = seg, it = 0; t < nt; t += nseg, ++it) {
+                const bool more = t + nseg < nt;
+                const int b = it & 1;
                 if (more) r = gather_pp(A, idn);
-                idn = load_id(ids, (t + 2) * TILE + lane, n);
-                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, S.nbrow, A);
-                if (((t + 1) & (2 * k - 1)) == 0) fold(T);
+                idn = load_id(ids, (t + 2 * nseg) * TILE + lane, n);
+                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, rowcnt, A);
+                if (((it + 1) & (2 * k - 1)) == 0) fold(T);
                 if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
             }
@@ -328,15 +337,38 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
         T.dax += shfl_xor_double(T.dax, o); T.day += shfl_xor_double(T.day, o);
         T.daz += shfl_xor_double(T.daz, o); T.dph += shfl_xor_double(T.dph, o);
     }
+    if (!(v && part == 0)) return;
+    if (SPLIT) {
+        double* q = A.part + ((size_t)seg * (size_t)A.n + orig) * 4;
+        q[0] = T.dax; q[1] = T.day; q[2] = T.daz; q[3] = T.dph;
+        return;
+    }
     // ---- a11: results to the caller's order ----
-    if (v && part == 0) {
-        const float4 a = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
-        A.out[orig] = a;
-        if (A.vel) {                            // eq. 12: xdot += (dt_reg / 2) F_R, one fma per component
-            float4 u = A.vel[orig];
-            u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
-            A.vel[orig] = u;
-        }
+    const float4 a = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
+    A.out[orig] = a;
+    if (A.vel) {                                // eq. 12: xdot += (dt_reg / 2) F_R, one fma per component
+        float4 u = A.vel[orig];
+        u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
+        A.vel[orig] = u;
+    }
+}
+
+// SPLIT epilogue (a11): the segments of every particle in segment order, then the kick
+__global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double s[4] = { 0, 0, 0, 0 };
+    for (int g = 0; g < A.nseg; ++g) {
+        const double* q = A.part + ((size_t)g * n + i) * 4;
+        s[0] += q[0]; s[1] += q[1]; s[2] += q[2]; s[3] += q[3];
+    }
+    const float4 a = make_float4((float)s[0], (float)s[1], (float)s[2], (float)s[3]);
+    A.out[i] = a;
+    if (A.vel) {
+        float4 u = A.vel[i];
+        u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
+        A.vel[i] = u;
     }
 }
 
@@ -345,6 +377,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
 // warp, and a chunk costs list length / k.  Persistent grid, dynamic
 // scheduling; the chunks are handed out in four passes, k = 1 first and k = 8 last, so that the
 // kernel ends on its cheapest items and the warps finish together.
+template <bool SPLIT>
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(force_args A)
 {
     __shared__ tile_smem smem[FORCE_WARPS];
@@ -356,6 +389,8 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         int c = 0;
         if (lane == 0) c = (int)atomicAdd(&A.info->group_cursor3, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
+        int seg = 0;
+        if (SPLIT) { seg = c % A.nseg; c /= A.nseg; }          // the segments of an item are handed out together
         if (c >= 4 * ng) break;
         int g, j;
         if (c < 2 * ng)      { g = c >> 1; j = c & 1; }
@@ -368,7 +403,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         else if (j == 2) { tb = 32 * full;             len = r & 16; }
         else             { tb = 32 * full + (r & 16);  len = r & 15; }
         if (len == 0) continue;
-        force_item(A, S, g, gb + tb, gb + tb + len);
+        force_item<SPLIT>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1);
         __syncwarp();
     }
 }
@@ -478,7 +513,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     const int n = (int)ctx->n;
     static int per_sm = 0;
     if (!per_sm) {
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force, FORCE_THREADS, 0));
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FORCE_THREADS, 0));
         if (per_sm < 1) per_sm = 1;
     }
     int rc;
@@ -529,9 +564,28 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.out = acc_pot; A.info = INFO(ctx);
     make_consts(A.K, r_out, r_in, theta, pot_mode, r_list);
     A.vel = vel; A.half_dt = half_dt;
-    // a8, a9, a11: the force kernel
+    // a8, a9, a11: the force kernel.  A problem with fewer work items (about 1.4 per 32 particles) than
+    // three per resident warp shares every item among nseg warps (SPLIT), so that small N still fills the GPU.
+    const long long warps = (long long)per_sm * ctx->num_sms * FORCE_WARPS;
+    const long long items = (long long)n * 14 / 320 + 1;
+    int nseg = 1;
+    while (nseg < 8 && items * nseg < 3 * warps) nseg *= 2;
+    A.nseg = nseg; A.n = n; A.nbcnt = nullptr; A.part = nullptr;
+    if (nseg > 1) {
+        if ((rc = p3t_reserve(ctx, &ctx->nbcnt, (size_t)n * 4))) return rc;
+        if ((rc = p3t_reserve(ctx, &ctx->part, (size_t)nseg * n * 32))) return rc;
+        A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcnt.p, 0, (size_t)n * 4, ctx->stream));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->part.p, 0, (size_t)nseg * n * 32, ctx->stream));   // a segment beyond a short list writes nothing
+    }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
-    k_force<<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+    if (nseg > 1) {
+        k_force<true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        k_force_final<<<(n + 255) / 256, 256, 0, ctx->stream>>>(A, n);
+        ctx->launches += 1;
+    } else {
+        k_force<false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+    }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
     k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
     P3T_CUDA(ctx, cudaGetLastError());

@@ -65,6 +65,7 @@ struct p3t_ctx {
     p3t_buf gnpp, gnpc;              // per-group list lengths
     p3t_buf nbcount, nboff, nbidx;   // neighbour CSR: counts (sorted order) -> offsets (original order), indices
     p3t_buf nbcur;                   // int64 per sorted particle: write cursor base
+    p3t_buf nbcnt, part;             // k_force<SPLIT>: row cursors (int32 per particle), partial sums [nseg][n][4] fp64
     p3t_buf spill;                   // walk stack spill
     p3t_buf pcpool, pppool;          // interaction lists: node ids / sorted particle positions, per-warp regions
     p3t_buf glist;                   // uint4 per group: pc offset/32, n_pc, pp offset/32, n_pp
