@@ -18,7 +18,7 @@
 
 #define FORCE_WARPS   4
 #define FORCE_THREADS (FORCE_WARPS * 32)
-#define FORCE_CTAS_PER_SM 5
+#define FORCE_CTAS_PER_SM 3
 #define TILE          32                  // list entries per tile
 #define FAR_AWAY      1.0e18f             // position of the zero-mass padding entries of a tile
 
@@ -131,7 +131,7 @@ __device__ __forceinline__ void pc_pair(target& T, f2 cx, f2 cy, f2 cz, f2 cm, f
 // one tile of TILE cells; this lane takes the 4-entry blocks part, part + k, ...
 __device__ __forceinline__ void eval_pc(target& T, const float (*pc)[TILE], int part, int k)
 {
-#pragma unroll 1
+#pragma unroll 2
     for (int e = 4 * part; e < TILE; e += 4 * k) {
         ulonglong2 v[10];
 #pragma unroll
@@ -208,7 +208,7 @@ __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], cons
                                         long long rowbase, int* rowcnt, const force_args& A)
 {
     uint32_t nearblocks = 0;                     // bit b: this lane's target came within r_out of block b
-#pragma unroll 1
+#pragma unroll 2
     for (int e = 4 * part; e < TILE; e += 4 * k) {
         ulonglong2 v[4];
 #pragma unroll
