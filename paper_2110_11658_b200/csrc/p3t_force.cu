@@ -131,7 +131,7 @@ __device__ __forceinline__ void pc_pair(target& T, f2 cx, f2 cy, f2 cz, f2 cm, f
 // one tile of TILE cells; this lane takes the 4-entry blocks part, part + k, ...
 __device__ __forceinline__ void eval_pc(target& T, const float (*pc)[TILE], int part, int k)
 {
-#pragma unroll 2
+#pragma unroll 4
     for (int e = 4 * part; e < TILE; e += 4 * k) {
         ulonglong2 v[10];
 #pragma unroll
