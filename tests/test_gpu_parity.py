@@ -388,3 +388,14 @@ def test_list_pools_grow_between_calls(p3t):
         ctx.build_tree(_cuda(small.pos_mass), 63)
         check_force(ctx, Ts, small, 0)
         check_neighbours(ctx, small)
+
+
+def test_two_component_cluster_eq26(p3t):
+    """The paper's core-collapse cluster (section 3.2, eq. 26): Plummer 64k, every tenth particle 10x heavier."""
+    w = workloads.make_config(6)
+    T = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        check_build(ctx, T, w.pos_mass, 63)
+        check_force(ctx, T, w, 0)
+        check_neighbours(ctx, w)

@@ -70,3 +70,12 @@ def test_sample_targets():
     s = workloads.sample_targets(1000, 10)
     assert list(s) == list(range(0, 1000, 100)) and s.dtype == np.int64
     assert len(workloads.sample_targets(5, 10)) == 5
+
+
+def test_two_component_spectrum_eq26():
+    """eq. 26: every tenth particle ten times heavier, total mass 1, half the mass in 10 %."""
+    w = workloads.make_config(6)
+    m = w.pos_mass[:, 3].astype(np.float64)
+    assert w.n == 65536 and abs(m.sum() - 1.0) < 1e-4           # exactly 1 only when 10 divides N
+    assert np.allclose(m[::10] / m[1], 10.0, rtol=1e-6) and np.allclose(m[1:10], m[1], rtol=1e-7)
+    assert abs(m[::10].sum() - 10.0 / 19.0) < 1e-3               # 'approximately half of the system's mass'

@@ -183,6 +183,14 @@ def kroupa_masses(seed: int, n: int, m_lo: float = 0.08, m_br: float = 0.5, m_hi
     return m / m.sum()
 
 
+def two_component_masses(n: int) -> np.ndarray:
+    """The mass spectrum of the paper's core-collapse run, eq. 26: m_i = 10 / (1.9 N) if
+    i = 0 (mod 10), else 1 / (1.9 N): about half of the mass in a tenth of the particles; the sum is 1."""
+    m = np.full(n, 1.0 / (1.9 * n))
+    m[::10] = 10.0 / (1.9 * n)
+    return m
+
+
 def equal_masses(n: int) -> np.ndarray:
     return np.full(n, 1.0 / n)
 
@@ -220,6 +228,8 @@ CONFIGS = {
     3: ("plummer1m_kroupa", 1048576, "plummer", "kroupa", (0.4,), 3),
     4: ("king9_1m_kroupa", 1048576, "king9", "kroupa", (0.4,), 4),
     5: ("plummer4m_equal", 4194304, "plummer", "equal", (0.3, 0.5, 0.7), 5),
+    # not a BASELINE.json config: the paper's 64k two-component cluster of section 3.2
+    6: ("plummer64k_two_component", 65536, "plummer", "two_component", (0.4,), 6),
 }
 
 
@@ -229,7 +239,7 @@ def make_config(cfg: int, n_override: int | None = None, theta: float | None = N
         n = int(n_override)
         label = f"{label}@n={n}"
     pos = plummer_positions(seed, n) if model == "plummer" else king_positions(seed, n, 9.0)
-    m = equal_masses(n) if masses == "equal" else kroupa_masses(seed, n)
+    m = equal_masses(n) if masses == "equal" else two_component_masses(n) if masses == "two_component" else kroupa_masses(seed, n)
     r_out = float(np.float32(r_out_for_n(n)))
     r_in = float(np.float32(0.1) * np.float32(r_out))     # gamma = 0.1
     return Workload(label, _pack(pos, m), r_out, float(np.float32(r_in)),
