@@ -55,7 +55,7 @@ struct p3t_ctx {
     p3t_buf rank;                    // int32: original id -> sorted position
     p3t_buf hist;                    // sort: per-block digit counts
     p3t_buf nlevel, nbegin, nend, nfirst, nnchild;        // int32 per node
-    p3t_buf m64;                     // double[10] per node: M, com[3], Q[6]
+    p3t_buf m64;                     // double[13] per node: M, sum m x [3], Q[6], COM[3]
     p3t_buf ncom, nlo, nhi, nq0, nq1, nlink;              // walk SoA (see p3t_tree.cu)
     p3t_buf scan_tmp;                // tree build: starters per level and block [22][blocks]
     p3t_buf pcl, plam;               // int8 per particle: cl(i), lam(i) (p3t_tree.cu)

@@ -31,7 +31,7 @@ struct tree_args {
     int8_t *pcl, *plam;        // per particle: cl(i), lam(i)
     int32_t* blksum;           // [MAXLEV][nblk] starters per level and block -> exclusive prefix
     int32_t *nlevel, *nbegin, *nend, *nfirst, *nnchild, *nparent, *nfc, *ncount;
-    double* m64;               // [node][10] = M, sum m x (3), Q about COM (6: xx yy zz xy xz yz)
+    double* m64;               // [node][13] = M, sum m x (3), Q about COM (6: xx yy zz xy xz yz), COM (3)
     float4 *ncom, *nlo, *nhi, *nq0;
     float2* nq1;
     int2* nlink;
@@ -220,11 +220,12 @@ __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-w
 __device__ void store_node(const tree_args& A, int k, int level, int b, int e, int first, int nchild,
                            double M, const double s[3], const double Q[6], const float clo[3], const float chi[3])
 {
-    double* m = A.m64 + (size_t)k * 10;
+    double* m = A.m64 + (size_t)k * 13;
     m[0] = M; m[1] = s[0]; m[2] = s[1]; m[3] = s[2];
 #pragma unroll
     for (int q = 0; q < 6; ++q) m[4 + q] = Q[q];
     const double c[3] = { s[0] / M, s[1] / M, s[2] / M };
+    m[10] = c[0]; m[11] = c[1]; m[12] = c[2];       // the parent reads the quotient instead of dividing again (same bits)
     // geometric centre from the integer cell coordinates (prefix of the first key)
     const uint64_t prefix = level == 0 ? 0ull : (A.keys[b] >> (3 * (A.B - level)));
     const uint32_t p3[3] = { compact3(prefix >> 2), compact3(prefix >> 1), compact3(prefix) };
@@ -288,7 +289,7 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
         double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
         float clo[3] = { INFINITY, INFINITY, INFINITY }, chi[3] = { -INFINITY, -INFINITY, -INFINITY };
         for (int c = fc; c < fc + nc; ++c) {
-            const double* m = A.m64 + (size_t)c * 10;
+            const double* m = A.m64 + (size_t)c * 13;
             M += __ldcg(m); s[0] += __ldcg(m + 1); s[1] += __ldcg(m + 2); s[2] += __ldcg(m + 3);
             float4 lo = __ldcg(&A.nlo[c]), hi = __ldcg(&A.nhi[c]);
             clo[0] = fminf(clo[0], lo.x); clo[1] = fminf(clo[1], lo.y); clo[2] = fminf(clo[2], lo.z);
@@ -297,9 +298,9 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
         const double cm[3] = { s[0] / M, s[1] / M, s[2] / M };
         double Q[6] = { 0, 0, 0, 0, 0, 0 };
         for (int c = fc; c < fc + nc; ++c) {
-            const double* m = A.m64 + (size_t)c * 10;
+            const double* m = A.m64 + (size_t)c * 13;
             const double Mc = __ldcg(m);
-            const double dx = __ldcg(m + 1) / Mc - cm[0], dy = __ldcg(m + 2) / Mc - cm[1], dz = __ldcg(m + 3) / Mc - cm[2];
+            const double dx = __ldcg(m + 10) - cm[0], dy = __ldcg(m + 11) - cm[1], dz = __ldcg(m + 12) - cm[2];
             const double d2 = dx * dx + dy * dy + dz * dz;
             Q[0] += __ldcg(m + 4) + Mc * (3 * dx * dx - d2); Q[1] += __ldcg(m + 5) + Mc * (3 * dy * dy - d2); Q[2] += __ldcg(m + 6) + Mc * (3 * dz * dz - d2);
             Q[3] += __ldcg(m + 7) + Mc * 3 * dx * dy; Q[4] += __ldcg(m + 8) + Mc * 3 * dx * dz; Q[5] += __ldcg(m + 9) + Mc * 3 * dy * dz;
