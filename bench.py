@@ -265,6 +265,14 @@ def run_ours(args, w, rank, world, local_rank, dist):
         "kernel_ms": wms, "kernel_share_of_step": wms * args.steps / total_ms,
         "frac_at_observed_clock": (achieved / (sms * 128 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
     }
+    # secondary roofline (north_star: "achieved HBM GB/s for build/sort"): a1-a6 against the measured copy bandwidth;
+    # algorithmic bytes per particle from SURVEY.md 8(d): cube 16 + keys 28 + radix sort 200 + gather 36 + topology 16 + moments 54 + groups 4
+    build_ms_mean = float(np.mean(build_ms))
+    build_gbs = 354.0 * n / (build_ms_mean * 1e-3) / 1e9
+    roofline_build = {"bound": "hbm", "kernels": "a1-a6 (cube, keys, radix sort, permute, topology, moments, groups)",
+                      "achieved": build_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": build_gbs / pk["hbm_gbs"],
+                      "algorithmic": "354 B per particle", "ms": build_ms_mean,
+                      "note": "launch/latency-bound below N ~ 2^22: 34 small kernels, working set in L2"}
     line = {
         "metric": "regular_force_particles_per_s", "value": value, "unit": "particles/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms_max / args.steps,
@@ -283,7 +291,7 @@ def run_ours(args, w, rank, world, local_rank, dist):
                             "note": "p3t_irregular_force (F_I, jerk, phi_I over the neighbour lists); not part of the timed step"},
         "next3_core": {"ms": core_ms, "sample": ns, "k": 6, "r_core": core["r_core"], "rho_core": core["rho_core"], "n_core": core["n_core"],
                        "note": "p3t_core_quantities (k-NN on the octree + Casertano-Hut reductions); not part of the timed step"},
-        "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "roofline_build": roofline_build,
     }
     if world == 1 and not args.no_cpu_baseline:
         r = oracle_sample_run(w, 4000 if n >= 500000 else 100000)
