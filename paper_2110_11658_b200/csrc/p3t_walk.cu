@@ -18,6 +18,7 @@
 // measured 6.5 TB/s) and lets either kernel run at its own occupancy.
 // The paper gives no detail of this stage ("the BONSAI library").
 #include "p3t_internal.cuh"
+#include "p3t_f32x2.cuh"
 #include <stdlib.h>
 
 #define WALK_WARPS   8
@@ -185,14 +186,16 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
                 // R10 neighbour predicate, bit-specified fp32, for the 32 particles of this round
                 if (lane < m) { const float4 p = A.spm[j]; C->x[lane] = p.x; C->y[lane] = p.y; C->z[lane] = p.z; C->j[lane] = j; }
                 __syncwarp();
+                // both target slots of the lane in one packed operation; d = x_i - x_j here, the exact negative of
+                // R10's x_j - x_i, so d2 has the same bits.  Self (always met: its own leaf is opened) is counted
+                // and taken off at the end, which spares the index test in the loop.
+                const f2 TX = pk(tx[0], tx[1]), TY = pk(ty[0], ty[1]), TZ = pk(tz[0], tz[1]);
                 for (int e = 0; e < m; ++e) {
-                    const float px = C->x[e], py = C->y[e], pz = C->z[e]; const int pj = C->j[e];
-#pragma unroll
-                    for (int s = 0; s < 2; ++s) {
-                        const float dx = __fsub_rn(px, tx[s]), dy = __fsub_rn(py, ty[s]), dz = __fsub_rn(pz, tz[s]);
-                        const float d2 = fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
-                        cnt[s] += (d2 < A.rout2 && pj != tid[s]) ? 1 : 0;          // self excluded by index
-                    }
+                    const float px = C->x[e], py = C->y[e], pz = C->z[e];
+                    const f2 dx = sub2(TX, pk(px, px)), dy = sub2(TY, pk(py, py)), dz = sub2(TZ, pk(pz, pz));
+                    const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                    cnt[0] += f2lo(d2) < A.rout2 ? 1 : 0;
+                    cnt[1] += f2hi(d2) < A.rout2 ? 1 : 0;
                 }
                 __syncwarp();
             }
@@ -215,7 +218,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
     } else {
 #pragma unroll
         for (int s = 0; s < 2; ++s)
-            if (tid[s] >= 0) A.nbcount[A.order[tid[s]]] = cnt[s];
+            if (tid[s] >= 0) A.nbcount[A.order[tid[s]]] = cnt[s] - (0.0f < A.rout2 ? 1 : 0);   // minus self (d2 = 0)
     }
     if (lane == 0 && overflow) atomicOr(&A.info->stack_overflow, 1);
 }
