@@ -255,6 +255,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
     alg_instr = INSTR_PP * st["n_pp"] + INSTR_PC * st["n_pc"]
     peak_instr = sms * 128 * pk["sm_max_mhz"] * 1e6 / 1e12            # Tinstr/s, FP32 lanes x clock
     achieved = alg_instr / (wms * 1e-3) / 1e12
+    pipes = p3t.pipe_bench(local_rank)                     # FFMA chain etc. on this device
+    peak_meas = pipes["fp32_lane_instr_per_s"] / 1e12
     roofline = {
         "bound": "alu", "kernel": "k_force (p-c / p-p force + cutoff + neighbour emission over the interaction lists)",
         "achieved": achieved, "peak": peak_instr, "unit": "Tinstr/s (FP32 lane-instructions)", "frac": achieved / peak_instr,
@@ -262,6 +264,9 @@ def run_ours(args, w, rank, world, local_rank, dist):
         "peak_source": f"{sms} SMs x 128 FP32 lanes x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
         "algorithmic": f"{INSTR_PP} instr per p-p x {st['n_pp']} + {INSTR_PC} per p-c x {st['n_pc']}",
         "achieved_tflops": (FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]) / (wms * 1e-3) / 1e12,
+        "peak_measured": peak_meas, "frac_of_measured": achieved / peak_meas,
+        "peak_measured_source": "p3t_pipe_bench: FFMA chain, 32 lanes / %.3f cycles per SM sub-partition" % pipes["cycles"]["FFMA (reuse cache)"],
+        "pipe_cycles": pipes["cycles"],
         "kernel_ms": wms, "kernel_share_of_step": wms * args.steps / total_ms,
         "frac_at_observed_clock": (achieved / (sms * 128 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
     }

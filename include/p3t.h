@@ -172,6 +172,13 @@ int p3t_get_groups(p3t_ctx* ctx, int32_t* begin, int32_t* end);
 /* per-group list lengths of the last force call: npp[n_groups], npc[n_groups] (int32) */
 int p3t_get_list_lengths(p3t_ctx* ctx, int32_t* npp, int32_t* npc);
 
+/* Micro-benchmarks of the FP32 pipe (the ALU roofline of the force kernel and the
+ * per-instruction costs behind it).  cycles_out: HOST double[n_out >= 8], SM-clock cycles per SM
+ * sub-partition of: [0] FFMA (best case: operands in the reuse cache), [1] FFMA2 with two distinct register pairs, [2] FFMA2 with three, [3] FMUL2,
+ * [4] one FMUL2 + one FFMA, [5] eight FMUL2 + two MUFU.RSQ, [6] MUFU.RSQ, [7] FFMA with three distinct registers.  sm_clock_mhz / num_sms: HOST,
+ * may be NULL (the device's nominal maximum clock, which the cycle counts assume).  Synchronises; ~20 ms. */
+int p3t_pipe_bench(int device, double* cycles_out, int n_out, double* sm_clock_mhz, int* num_sms);
+
 const char* p3t_strerror(int code);
 const char* p3t_last_error(p3t_ctx* ctx);     /* text of the last CUDA failure ("" if none) */
 
