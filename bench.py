@@ -300,9 +300,17 @@ def run_ours(args, w, rank, world, local_rank, dist):
     }
     if world == 1 and not args.no_cpu_baseline:
         r = oracle_sample_run(w, 4000 if n >= 500000 else 100000)
+        # the plain definition (eq. 3 by direct summation, fp64) on a stride sample of targets
+        import oracle
+        n_t = 2048
+        t0 = time.perf_counter()
+        oracle.direct(w.pos_mass, w.r_out, w.r_in, targets=workloads.sample_targets(n, n_t))
+        t_direct = time.perf_counter() - t0
         line["cpu_baseline"] = {
             "value": r["particles_per_s"], "unit": "particles/s", "cores": r["cores"], "kind": "oracle",
             "interactions_per_s": r["interactions_per_s"],
+            "direct_sum": {"pairs_per_s": n_t * float(n) / t_direct, "targets": n_t, "seconds": t_direct,
+                           "full_n2_seconds_extrapolated": t_direct * n / n_t},
             "sample": (f"full oracle tree build ({r['t_build']:.2f} s) + fp64 tree force of every {r['stride']}th group "
                        f"({r['groups']} groups, {r['n_sample']} particles, {r['t_force']:.2f} s); extrapolated to the full N"),
         }
