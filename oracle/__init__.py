@@ -70,6 +70,8 @@ def lib() -> C.CDLL:
         _lib.p3t_o_tree_force.argtypes = [vp, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_tree_force_buffered.restype = None
         _lib.p3t_o_tree_force_buffered.argtypes = [vp, f32, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
+        _lib.p3t_o_tree_force_order.restype = None
+        _lib.p3t_o_tree_force_order.argtypes = [vp, C.c_int, f32, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_pc_term.restype = None; _lib.p3t_o_pc_term.argtypes = [vp, vp, vp, vp]
         _lib.p3t_o_open_test.restype = C.c_int
         _lib.p3t_o_open_test.argtypes = [vp, vp, vp, vp, vp, f32, f32, f32, f32]
@@ -224,7 +226,7 @@ class Tree:
         return dict(begin=b, end=e, glo=glo, ghi=ghi)
 
     def force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, group_ids=None, want_abs: bool = False,
-              r_list: float | None = None):
+              r_list: float | None = None, order: int = 2):
         """dict(acc_pot [n,4] fp64 in original order (rows of unwalked groups are NaN), npp, npc, abs_sum)."""
         gi = None if group_ids is None else np.ascontiguousarray(group_ids, dtype=np.int64)
         ng = self.n_groups if gi is None else gi.shape[0]
@@ -232,7 +234,7 @@ class Tree:
         npp = np.zeros(ng, np.int64); npc = np.zeros(ng, np.int64)
         ab = np.full(self.n, np.nan) if want_abs else None
         rl = r_out if r_list is None else r_list          # neighbour search radius in the opening rule (NEXT-2)
-        lib().p3t_o_tree_force_buffered(self._h, float(np.float32(rl)), float(np.float32(r_out)), float(np.float32(r_in)),
+        lib().p3t_o_tree_force_order(self._h, int(order), float(np.float32(rl)), float(np.float32(r_out)), float(np.float32(r_in)),
                                         float(np.float32(theta)), int(pot_mode), ng, _p(gi), _p(out), _p(npp), _p(npc), _p(ab))
         return dict(acc_pot=out, npp=npp, npc=npc, abs_sum=ab)
 

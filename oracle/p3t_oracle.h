@@ -90,6 +90,11 @@ void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list, float r_out, f
                                int64_t ng, const int64_t* group_ids, double* acc_pot,
                                int64_t* npp, int64_t* npc, double* abs_sum);
 
+/* the same with the multipole order chosen: 2 = monopole + quadrupole, 1 = monopole only */
+void p3t_o_tree_force_order(const p3t_o_tree* t, int order, float r_list, float r_out, float r_in, float theta, int pot_mode,
+                            int64_t ng, const int64_t* group_ids, double* acc_pot,
+                            int64_t* npp, int64_t* npc, double* abs_sum);
+
 /* single particle-cell term (fp64) from fp32 node data: out = {ax, ay, az, phi} */
 void p3t_o_pc_term(const double xi[3], const float com_m[4], const float quad[6], double out[4]);
 /* the fp32 opening test alone (R7): returns 1 = open */

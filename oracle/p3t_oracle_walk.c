@@ -91,6 +91,17 @@ void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list_f, float r_out_
                                int64_t ng, const int64_t* group_ids, double* acc_pot,
                                int64_t* npp, int64_t* npc, double* abs_sum)
 {
+    p3t_o_tree_force_order(t, 2, r_list_f, r_out_f, r_in_f, theta, pot_mode, ng, group_ids, acc_pot, npp, npc, abs_sum);
+}
+
+/* the monopole-only variant for the accuracy-throughput curve.  order 2 = monopole +
+ * quadrupole (north_star), order 1 = the same walk with the quadrupole of every accepted cell left out
+ * (R-S8 with Q = 0: phi = -M/R, a = -M r/R^3). */
+void p3t_o_tree_force_order(const p3t_o_tree* t, int order, float r_list_f, float r_out_f, float r_in_f, float theta, int pot_mode,
+                            int64_t ng, const int64_t* group_ids, double* acc_pot,
+                            int64_t* npp, int64_t* npc, double* abs_sum)
+{
+    static const float zero_quad[6] = { 0, 0, 0, 0, 0, 0 };
     const double r_out = r_out_f, r_in = r_in_f, D = r_out - r_in;
     const double psi_in = p3t_o_psi(r_in, r_out, r_in);
 #pragma omp parallel
@@ -109,7 +120,7 @@ void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list_f, float r_out_
                 double a[3] = { 0, 0, 0 }, phi = 0, asum = 0;
                 for (int64_t k = 0; k < pc.n; ++k) {
                     double o[4];
-                    p3t_o_pc_term(xi, t->fcom_m + 4 * (int64_t)pc.v[k], t->fquad + 6 * (int64_t)pc.v[k], o);
+                    p3t_o_pc_term(xi, t->fcom_m + 4 * (int64_t)pc.v[k], order >= 2 ? t->fquad + 6 * (int64_t)pc.v[k] : zero_quad, o);
                     a[0] += o[0]; a[1] += o[1]; a[2] += o[2]; phi += o[3];
                     asum += sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]);
                 }

@@ -320,3 +320,28 @@ def test_buffered_search_radius(cfg1):
     fs = ts.force(0.05, 0.005, 1e-3, r_list=0.08)
     ds = oracle.direct(pm, float(np.float32(0.05)), float(np.float32(0.005)))
     assert np.abs(fs["acc_pot"][:, :3] - ds["acc_reg"]).max() < 1e-11 * np.abs(ds["acc_reg"]).max()
+
+
+# ---- monopole-only variant ----
+def test_monopole_only_variant(cfg1):
+    """order = 1 drops the quadrupole of the accepted cells and nothing else: same lists, a larger but still
+    bounded error against eq. 3, theta -> 0 still the direct sum (no cell is accepted), and for a cell made of
+    one particle (Q = 0) both orders agree exactly."""
+    t = oracle.Tree(cfg1.pos_mass, 63, NLEAF, NCRIT)
+    f2 = t.force(cfg1.r_out, cfg1.r_in, 0.4)
+    f1 = t.force(cfg1.r_out, cfg1.r_in, 0.4, order=1)
+    assert np.array_equal(f1["npp"], f2["npp"]) and np.array_equal(f1["npc"], f2["npc"])
+    d = oracle.direct(cfg1.pos_mass, cfg1.r_out, cfg1.r_in)
+    n = np.linalg.norm(d["acc_reg"], axis=1)
+    e1 = np.linalg.norm(f1["acc_pot"][:, :3] - d["acc_reg"], axis=1) / n
+    e2 = np.linalg.norm(f2["acc_pot"][:, :3] - d["acc_reg"], axis=1) / n
+    assert np.median(e1) < 2e-3 and np.percentile(e1, 99) < 2e-2          # still inside north_star's bound
+    assert np.median(e1) > 3 * np.median(e2)                               # and clearly worse than with the quadrupole
+    pm = _small(512, scale=0.3)
+    ts = oracle.Tree(pm, 63, NLEAF, NCRIT)
+    a = ts.force(0.05, 0.005, 1e-3, order=1)["acc_pot"]; b = ts.force(0.05, 0.005, 1e-3, order=2)["acc_pot"]
+    assert np.array_equal(a, b)
+    xi = np.array([1.0, 2.0, 3.0]); cm = np.array([0.25, -0.5, 0.125, 2.0], np.float32)
+    o = oracle.pc_term(xi, cm, np.zeros(6, np.float32))
+    r = xi - cm[:3]; R = np.linalg.norm(r)
+    assert np.allclose(o[:3], -2.0 * r / R ** 3, rtol=1e-14) and np.isclose(o[3], -2.0 / R, rtol=1e-14)
