@@ -81,6 +81,11 @@ int p3t_destroy(p3t_ctx* ctx);
  * Defaults 16 / 64.  Takes effect at the next build. */
 int p3t_set_tree_params(p3t_ctx* ctx, int nleaf, int ncrit);
 
+/* Multipole order of the particle-cell terms: 2 = monopole + quadrupole (default, north_star), 1 = monopole
+ * only (a cheaper point on the accuracy-throughput curve: same walk and lists, the
+ * quadrupole of the accepted cells left out).  Takes effect at the next p3t_regular_force. */
+int p3t_set_multipole_order(p3t_ctx* ctx, int order);
+
 /* Steps a1-a6: bounding cube, Morton keys (key_bits = 30 or 63), stable radix sort,
  * body permutation, canonical octree, monopole + traceless quadrupole moments, target groups.
  * pos_mass: DEVICE pointer, n x {x, y, z, m} fp32 (16-byte aligned), caller-owned, read-only;

@@ -21,7 +21,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/p3t.h declares
 SYMBOLS = [
-    "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_build_tree", "p3t_regular_force",
+    "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_set_multipole_order", "p3t_build_tree", "p3t_regular_force",
     "p3t_regular_force_ex", "p3t_irregular_force", "p3t_core_quantities", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_pipe_bench", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
     L.p3t_create.argtypes = [C.POINTER(vp), C.c_int, vp]
     L.p3t_destroy.argtypes = [vp]
     L.p3t_set_tree_params.argtypes = [vp, C.c_int, C.c_int]
+    L.p3t_set_multipole_order.argtypes = [vp, C.c_int]
     L.p3t_build_tree.argtypes = [vp, i64, vp, C.c_int]
     L.p3t_regular_force.argtypes = [vp, f32, f32, f32, C.c_int, vp]
     L.p3t_regular_force_ex.argtypes = [vp, f32, f32, f32, C.c_int, f32, f32, vp, vp]
@@ -168,6 +169,10 @@ class Context:
         """pos_mass: CUDA float32 tensor [n, 4] = x, y, z, m."""
         self.n = int(pos_mass.shape[0])
         self._check(lib().p3t_build_tree(self._h, self.n, self._dev_f32(pos_mass, 4), key_bits), "p3t_build_tree")
+
+    def set_multipole_order(self, order: int):
+        """2 = monopole + quadrupole (default), 1 = monopole only."""
+        self._check(lib().p3t_set_multipole_order(self._h, order), "p3t_set_multipole_order")
 
     def regular_force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, out=None,
                       r_buff: float = 0.0, half_dt: float = 0.0, vel=None):

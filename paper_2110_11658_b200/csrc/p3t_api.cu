@@ -54,7 +54,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     if (!c) return P3T_ENOMEM;
     memset(c, 0, sizeof(*c));
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
-    c->nleaf = 16; c->ncrit = 64;
+    c->nleaf = 16; c->ncrit = 64; c->order = 2;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
     for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
@@ -93,6 +93,13 @@ int p3t_set_tree_params(p3t_ctx* c, int nleaf, int ncrit)
 {
     if (!c || nleaf < 1 || ncrit < nleaf || ncrit > P3T_MAX_NCRIT) return P3T_EINVAL;
     c->nleaf = nleaf; c->ncrit = ncrit;
+    return P3T_OK;
+}
+
+int p3t_set_multipole_order(p3t_ctx* c, int order)
+{
+    if (!c || (order != 1 && order != 2)) return P3T_EINVAL;
+    c->order = order;
     return P3T_OK;
 }
 

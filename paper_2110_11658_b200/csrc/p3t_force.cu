@@ -36,6 +36,7 @@ struct force_args {
     int32_t* nbcnt;             // SPLIT: per sorted position, neighbours already written to the row (zeroed)
     double* part;               // SPLIT: partial sums [nseg][n][4], original order
     int nseg;                   // SPLIT: list segments per item
+    int mp_order;               // 2: monopole + quadrupole (default); 1: monopole only
     int n;
     float4* vel;                // in/out (may be NULL): velocities, original order, kicked by half_dt * F_R (eq. 12)
     float half_dt;
@@ -128,6 +129,33 @@ __device__ __forceinline__ void eval_pc(target& T, const float (*pc)[TILE], int 
         for (int r = 0; r < 10; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pc[r][e]);
         pc_pair(T, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, v[6].x, v[7].x, v[8].x, v[9].x);
         pc_pair(T, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, v[6].y, v[7].y, v[8].y, v[9].y);
+    }
+}
+
+// Monopole-only variant (SURVEY 8f NEXT-4, p3t_set_multipole_order(ctx, 1)): R-S8 with Q = 0,
+// phi = -M/R, a = M d / R^3; 13 operations per pair instead of 33.
+__device__ __forceinline__ void pc_pair_mono(target& T, f2 cx, f2 cy, f2 cz, f2 cm)
+{
+    const f2 dx = sub2(cx, pk(T.x, T.x)), dy = sub2(cy, pk(T.y, T.y)), dz = sub2(cz, pk(T.z, T.z));
+    const f2 R2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    const f2 ri = pk(rsqrt_approx(f2lo(R2)), rsqrt_approx(f2hi(R2)));
+    const f2 mono = mul2(cm, ri);
+    const f2 f = mul2(mono, mul2(ri, ri));
+    T.ph = add2(T.ph, mono);
+    const float fl = f2lo(f), fh = f2hi(f);
+    T.axe = fmaf(fl, f2lo(dx), T.axe); T.axo = fmaf(fh, f2hi(dx), T.axo);
+    T.aye = fmaf(fl, f2lo(dy), T.aye); T.ayo = fmaf(fh, f2hi(dy), T.ayo);
+    T.aze = fmaf(fl, f2lo(dz), T.aze); T.azo = fmaf(fh, f2hi(dz), T.azo);
+}
+__device__ __forceinline__ void eval_pc_mono(target& T, const float (*pc)[TILE], int part, int k)
+{
+#pragma unroll 2
+    for (int e = 4 * part; e < TILE; e += 4 * k) {
+        ulonglong2 v[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) v[r] = *reinterpret_cast<const ulonglong2*>(&pc[r][e]);
+        pc_pair_mono(T, v[0].x, v[1].x, v[2].x, v[3].x);
+        pc_pair_mono(T, v[0].y, v[1].y, v[2].y, v[3].y);
     }
 }
 
@@ -256,7 +284,7 @@ __device__ __forceinline__ double shfl_xor_double(double v, int o)
 // SPLIT (small problems, fewer items than resident warps): the item is shared by nseg warps, warp
 // `seg` takes the tiles seg, seg + nseg, ... of both lists; the partial sums go to A.part and are
 // added in segment order by k_force_final (bit-reproducible), the row cursors are global.
-template <bool SPLIT>
+template <bool SPLIT, bool MONO>
 __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te, int seg, int nseg)
 {
     const int lane = threadIdx.x & 31;
@@ -292,7 +320,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
                 const bool more = t + nseg < nt;
                 if (more) r = gather_pc(A, idn);
                 idn = load_id(ids, (t + 2 * nseg) * TILE + lane, n);
-                eval_pc(T, S.pc[it & 1], part, k);
+                if (MONO) eval_pc_mono(T, S.pc[it & 1], part, k); else eval_pc(T, S.pc[it & 1], part, k);
                 if (((it + 1) & (k - 1)) == 0) fold(T);
                 if (more) store_pc(S.pc[(it + 1) & 1], lane, r);
                 __syncwarp();
@@ -367,7 +395,7 @@ __global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
 // warp, and a chunk costs list length / k.  Persistent grid, dynamic
 // scheduling; the chunks are handed out in four passes, k = 1 first and k = 8 last, so that the
 // kernel ends on its cheapest items and the warps finish together.
-template <bool SPLIT>
+template <bool SPLIT, bool MONO>
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(force_args A)
 {
     __shared__ tile_smem smem[FORCE_WARPS];
@@ -393,7 +421,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         else if (j == 2) { tb = 32 * full;             len = r & 16; }
         else             { tb = 32 * full + (r & 16);  len = r & 15; }
         if (len == 0) continue;
-        force_item<SPLIT>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1);
+        force_item<SPLIT, MONO>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1);
         __syncwarp();
     }
 }
@@ -503,7 +531,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     const int n = (int)ctx->n;
     static int per_sm = 0;
     if (!per_sm) {
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FORCE_THREADS, 0));
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false, false>, FORCE_THREADS, 0));
         if (per_sm < 1) per_sm = 1;
     }
     int rc;
@@ -553,7 +581,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
     A.out = acc_pot; A.info = INFO(ctx);
     make_consts(A.K, r_out, r_in, theta, pot_mode, r_list);
-    A.vel = vel; A.half_dt = half_dt;
+    A.vel = vel; A.half_dt = half_dt; A.mp_order = ctx->order;
     // a8, a9, a11: the force kernel.  A problem with fewer work items (about 1.4 per 32 particles) than
     // three per resident warp shares every item among nseg warps (SPLIT), so that small N still fills the GPU.
     const long long warps = (long long)per_sm * ctx->num_sms * FORCE_WARPS;
@@ -561,6 +589,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     int nseg = 1;
     while (nseg < 8 && items * nseg < 3 * warps) nseg *= 2;
     A.nseg = nseg; A.n = n; A.nbcnt = nullptr; A.part = nullptr;
+    const bool mono = ctx->order < 2;
     if (nseg > 1) {
         if ((rc = p3t_reserve(ctx, &ctx->nbcnt, (size_t)n * 4))) return rc;
         if ((rc = p3t_reserve(ctx, &ctx->part, (size_t)nseg * n * 32))) return rc;
@@ -570,11 +599,13 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
     if (nseg > 1) {
-        k_force<true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        if (mono) k_force<true, true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        else      k_force<true, false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
         k_force_final<<<(n + 255) / 256, 256, 0, ctx->stream>>>(A, n);
         ctx->launches += 1;
     } else {
-        k_force<false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        if (mono) k_force<false, true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        else      k_force<false, false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
     k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);

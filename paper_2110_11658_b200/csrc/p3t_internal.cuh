@@ -43,6 +43,7 @@ struct p3t_ctx {
     cudaStream_t stream;
     int num_sms;
     int nleaf, ncrit;
+    int order;               // multipole order of the p-c terms: 2 (default) or 1
     int state;               // 0 = created, 1 = built, 2 = force done
     int64_t n;
     int key_bits, bits;      // bits per axis

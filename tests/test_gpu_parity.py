@@ -399,3 +399,31 @@ def test_two_component_cluster_eq26(p3t):
         check_build(ctx, T, w.pos_mass, 63)
         check_force(ctx, T, w, 0)
         check_neighbours(ctx, w)
+
+
+def test_monopole_only_variant(p3t, cfg1):
+    """p3t_set_multipole_order(1): same lists, quadrupole left out; parity against the oracle's
+    order-1 walk, the north_star bound against eq. 3, and back to order 2 on the same context."""
+    w = cfg1
+    T = oracle.Tree(w.pos_mass, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        a2 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).cpu().numpy().astype(np.float64)
+        ctx.set_multipole_order(1)
+        a1 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).cpu().numpy().astype(np.float64)
+        npp, npc = ctx.list_lengths()
+        f1 = T.force(w.r_out, w.r_in, w.theta, 0, want_abs=True, order=1)
+        assert np.array_equal(npp, f1["npp"]) and np.array_equal(npc, f1["npc"])
+        ref = f1["acc_pot"]
+        assert np.linalg.norm(a1[:, :3] - ref[:, :3]) <= 1e-6 * np.linalg.norm(ref[:, :3])
+        assert np.all(np.linalg.norm(a1[:, :3] - ref[:, :3], axis=1) <= 1e-6 * f1["abs_sum"] + 1e-30)
+        assert np.all(np.abs(a1[:, 3] - ref[:, 3]) <= 2e-6 * np.abs(ref[:, 3]))
+        d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
+        e1 = _rel(a1[:, :3], d["acc_reg"]); e2 = _rel(a2[:, :3], d["acc_reg"])
+        assert np.median(e1) < 2e-3 and np.percentile(e1, 99) < 2e-2 and np.median(e1) > 3 * np.median(e2)
+        check_neighbours(ctx, w)
+        ctx.set_multipole_order(2)
+        b2 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).cpu().numpy().astype(np.float64)
+        assert np.array_equal(a2, b2)
+        with pytest.raises(p3t.P3TError):
+            ctx.set_multipole_order(3)
