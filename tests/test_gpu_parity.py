@@ -427,3 +427,55 @@ def test_monopole_only_variant(p3t, cfg1):
         assert np.array_equal(a2, b2)
         with pytest.raises(p3t.P3TError):
             ctx.set_multipole_order(3)
+
+
+def test_randomised_shapes_and_tree_parameters(p3t):
+    """60 seeded small problems of awkward shape (7-fold duplicates, a line, a needle, a coarse lattice with many
+    coincident points, a tight core in a wide halo) with random N, key width, NLEAF / NCRIT, r_out and theta:
+    cells, groups, interaction lists, neighbour CSR and k-NN ids bit-exact, force within the R15 bound."""
+    import torch
+    rng = np.random.default_rng(20211122)
+
+    def make(n, kind):
+        if kind == 0: pos = rng.random((n, 3))
+        elif kind == 1: pos = np.repeat(rng.random((n // 7 + 1, 3)), 7, axis=0)[:n]
+        elif kind == 2: pos = np.c_[rng.random(n), np.zeros(n), np.zeros(n)]
+        elif kind == 3: pos = rng.normal(size=(n, 3)) * np.array([1, 1e-3, 1e-6])
+        elif kind == 4: pos = np.round(rng.random((n, 3)) * 8) / 8
+        else: pos = np.r_[rng.normal(size=(n - n // 10, 3)) * 0.01, rng.random((n // 10, 3)) * 100]
+        pm = np.zeros((n, 4), np.float32); pm[:, :3] = pos[:n]; pm[:, 3] = rng.random(n) + 0.1
+        return pm
+
+    for trial in range(60):
+        n = int(rng.choice([1, 2, 3, 17, 33, 64, 65, 100, 257, 1000, 3000]))
+        kind = int(rng.integers(0, 6)); bits = int(rng.choice([30, 63]))
+        nleaf = int(rng.choice([1, 4, 16, 33, 64]))
+        ncrit = int(rng.choice([c for c in (1, 8, 32, 64) if c >= nleaf]))
+        pm = make(n, kind)
+        ext = float(np.ptp(pm[:, :3], axis=0).max()) or 1.0
+        r_out = float(np.float32(ext * rng.choice([1e-3, 0.02, 0.1, 0.5]))); r_in = float(np.float32(0.1) * np.float32(r_out))
+        theta = float(rng.choice([0.3, 0.4, 0.8]))
+        tag = f"trial {trial}: n={n} kind={kind} bits={bits} nleaf={nleaf} ncrit={ncrit} r_out={r_out} theta={theta}"
+        T = oracle.Tree(pm, bits, nleaf, ncrit)
+        with p3t.Context(0, nleaf=nleaf, ncrit=ncrit) as ctx:
+            ctx.build_tree(_cuda(pm), bits)
+            st = ctx.stats()
+            assert (st["n_nodes"], st["n_leaves"], st["max_level"], st["n_groups"]) == (T.n_nodes, T.n_leaves, T.max_level, T.n_groups), tag
+            on, gn = T.nodes(), ctx.nodes()
+            assert all(np.array_equal(on[k], gn[k]) for k in on), tag
+            og, gg = T.groups(), ctx.groups()
+            assert np.array_equal(og["begin"], gg["begin"]) and np.array_equal(og["end"], gg["end"]), tag
+            a = ctx.regular_force(r_out, r_in, theta, 0).cpu().numpy().astype(np.float64)
+            f = T.force(r_out, r_in, theta, 0, want_abs=True)
+            npp, npc = ctx.list_lengths()
+            assert np.array_equal(npp, f["npp"]) and np.array_equal(npc, f["npc"]), tag
+            assert np.all(np.isfinite(a)), tag
+            assert np.all(np.linalg.norm(a[:, :3] - f["acc_pot"][:, :3], axis=1) <= 2e-6 * f["abs_sum"] + 1e-30), tag
+            off, idx = ctx.neighbours()
+            ooff, oidx = oracle.neighbours(pm, r_out)
+            assert np.array_equal(ooff, off.cpu().numpy()) and np.array_equal(oidx, idx.cpu().numpy()), tag
+            if n > 7:
+                s = np.arange(0, n, 3, dtype=np.int32)
+                g = ctx.core_quantities(torch.from_numpy(s).cuda(), 6)
+                o = oracle.knn_density(pm, s, 6)
+                assert np.array_equal(g["nbr"].cpu().numpy(), o["nbr"]) and np.array_equal(g["d2k"].cpu().numpy(), o["d2k"]), tag
