@@ -192,6 +192,11 @@ const char* p3t_last_error(p3t_ctx* ctx);     /* text of the last CUDA failure (
 int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, double* r_buff,
                       double* dt_reg, double* dt_max);
 
+/* Host helper, eq. 18-19: R_min = 4 r_h / (N rho_core^(1/3)), dT_min = 0.01 sqrt(eta / 0.02)
+ * sqrt(R_min^3): the regularisation parameters that p3t_core_quantities' rho_core feeds (r_h = half-mass
+ * radius, eta = 0.02 in the paper).  Either output may be NULL. */
+int p3t_regularisation_params(int64_t n, double r_h, double rho_core, double eta, double* r_min, double* dt_min);
+
 #ifdef __cplusplus
 }
 #endif

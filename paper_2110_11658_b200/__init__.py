@@ -24,7 +24,7 @@ SYMBOLS = [
     "p3t_create", "p3t_destroy", "p3t_set_tree_params", "p3t_set_multipole_order", "p3t_build_tree", "p3t_regular_force",
     "p3t_regular_force_ex", "p3t_irregular_force", "p3t_core_quantities", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
-    "p3t_get_list_lengths", "p3t_pipe_bench", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
+    "p3t_get_list_lengths", "p3t_pipe_bench", "p3t_strerror", "p3t_last_error", "p3t_params_from_n", "p3t_regularisation_params",
 ]
 
 
@@ -90,6 +90,7 @@ def lib() -> C.CDLL:
     L.p3t_strerror.argtypes = [C.c_int]; L.p3t_strerror.restype = C.c_char_p
     L.p3t_last_error.argtypes = [vp]; L.p3t_last_error.restype = C.c_char_p
     L.p3t_params_from_n.argtypes = [i64, dbl] + [C.POINTER(dbl)] * 5
+    L.p3t_regularisation_params.argtypes = [i64, dbl, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
     for s in SYMBOLS:
         if s not in ("p3t_strerror", "p3t_last_error"):
             getattr(L, s).restype = C.c_int
@@ -312,3 +313,12 @@ def pipe_bench(device: int = 0) -> dict:
     peak = sms.value * 4 * 32 / cyc[0] * mhz.value * 1e6
     return dict(cycles=dict(zip(PIPE_BENCH_LABELS, cyc)), sm_clock_mhz=mhz.value, num_sms=sms.value,
                 fp32_lane_instr_per_s=peak, nominal_lane_instr_per_s=sms.value * 128 * mhz.value * 1e6)
+
+
+def regularisation_params(n: int, r_h: float, rho_core: float, eta: float = 0.02):
+    """(R_min, dT_min) of eq. 18-19."""
+    a, b = C.c_double(), C.c_double()
+    rc = lib().p3t_regularisation_params(int(n), float(r_h), float(rho_core), float(eta), C.byref(a), C.byref(b))
+    if rc != 0:
+        raise P3TError(rc, "p3t_regularisation_params")
+    return a.value, b.value

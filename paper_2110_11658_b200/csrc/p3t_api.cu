@@ -440,4 +440,14 @@ int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, doubl
     return P3T_OK;
 }
 
+// eq. 18-19: the regularisation parameters that the core quantities feed
+int p3t_regularisation_params(int64_t n, double r_h, double rho_core, double eta, double* r_min, double* dt_min)
+{
+    if (n < 1 || !(r_h > 0.0) || !(rho_core > 0.0) || !(eta > 0.0)) return P3T_EINVAL;
+    const double rm = 4.0 * r_h / ((double)n * cbrt(rho_core));               // eq. 18
+    if (r_min) *r_min = rm;
+    if (dt_min) *dt_min = 0.01 * sqrt(eta / 0.02) * sqrt(rm * rm * rm);       // eq. 19
+    return P3T_OK;
+}
+
 }  // extern "C"
