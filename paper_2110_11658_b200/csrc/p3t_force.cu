@@ -390,8 +390,8 @@ __global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
     }
 }
 
-// Work items: the c <= 64 targets of a group are cut into chunks of 32, 32, 16 and c mod 16 targets,
-// which run with k = 1, 1, 2 and 2 / 4 / 8 lanes per target: every chunk but the last fills its
+// Work items: the c <= 64 targets of a group are cut into chunks of 32, 32, 16 and c mod 16 targets
+// (25 .. 31 left-over targets stay together), which run with k = 1, 1, 2 and 2 / 4 / 8 lanes per target: every chunk but the last fills its
 // warp, and a chunk costs list length / k.  Persistent grid, dynamic
 // scheduling; the chunks are handed out in four passes, k = 1 first and k = 8 last, so that the
 // kernel ends on its cheapest items and the warps finish together.
@@ -418,8 +418,8 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         const int full = n >> 5, r = n & 31;
         int tb, len;
         if (j < 2)       { tb = 32 * j;                len = j < full ? 32 : 0; }
-        else if (j == 2) { tb = 32 * full;             len = r & 16; }
-        else             { tb = 32 * full + (r & 16);  len = r & 15; }
+        else if (j == 2) { tb = 32 * full;             len = r >= 25 ? r : (r & 16); }      // 25..31 left over: one k = 1 item costs the same as 16 + rest
+        else             { tb = 32 * full + (r & 16);  len = r >= 25 ? 0 : (r & 15); }
         if (len == 0) continue;
         force_item<SPLIT, MONO>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1);
         __syncwarp();
