@@ -84,6 +84,7 @@ int p3t_destroy(p3t_ctx* c)
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
     for (int k = 0; k < 2; ++k) if (c->evi[k]) cudaEventDestroy(c->evi[k]);
     for (int k = 0; k < 2; ++k) if (c->evc[k]) cudaEventDestroy(c->evc[k]);
+    if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
     (void)cudaGetLastError();
     delete c;
     return P3T_OK;
@@ -320,10 +321,15 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
     P3T_CUDA(c, cudaMemcpyAsync(d_pm, pos_mass_host, (size_t)n * 16, cudaMemcpyHostToDevice, c->stream));
     if ((rc = p3t_build_tree(c, n, d_pm, key_bits)) != P3T_OK) return rc;
     if ((rc = p3t_regular_force(c, r_out, r_in, theta, pot_mode, d_out)) != P3T_OK) return rc;
+    // The CSR offsets were final before the force call's one host synchronisation (they size the lists):
+    // their copy goes to a second stream and overlaps the force kernel that is still running.
+    if (nb_offsets_host) {
+        if (!c->copy_stream) P3T_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->copy_stream));
+    }
     P3T_CUDA(c, cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
     const int64_t total = c->nb_total_host;                  // known on the host since the force call sized the lists
     if (nb_total) *nb_total = total;
-    if (nb_offsets_host) P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
     int over = 0;
     if (nb_indices_host) {
         if (total > nb_cap) over = 1;
@@ -331,6 +337,7 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
     }
     p3t_devinfo h;
     if ((rc = sync_and_check(c, &h)) != P3T_OK) return rc;
+    if (nb_offsets_host) P3T_CUDA(c, cudaStreamSynchronize(c->copy_stream));
     return over ? P3T_ERANGE : P3T_OK;
 }
 

@@ -41,6 +41,7 @@ struct p3t_buf { void* p; size_t bytes; };
 struct p3t_ctx {
     int device;
     cudaStream_t stream;
+    cudaStream_t copy_stream;        // p3t_step_host: device-to-host copies that overlap the force kernel (created on first use)
     int num_sms;
     int nleaf, ncrit;
     int order;               // multipole order of the p-c terms: 2 (default) or 1
