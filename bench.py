@@ -12,8 +12,11 @@ with cutoff, neighbour lists, scatter), i.e. what the host integrator asks for o
 Prints ONE JSON line (rank 0).  `value` times the path with inputs resident in HBM; `e2e` times
 p3t_step_host with pinned HOST buffers (H2D of positions, D2H of forces and neighbour lists inside
 the timed region).  `roofline` is for the dominant kernel (walk + force), an FP32-ALU-bound kernel;
-`cpu_baseline` is the fp64 oracle on the host cores, on a bounded sample.  Multi-GPU: the path does
-not shard in this build ("replicas only"): every rank runs an independent replica.
+`cpu_baseline` is the fp64 oracle on the host cores, on a bounded sample.  Multi-GPU: by default every
+rank runs an independent replica ("replicas only", weak scaling; north_star is a one-GPU path).
+`--mode sharded` splits the target groups of ONE cluster among the ranks
+(paper_2110_11658_b200.shard; strong scaling, one all-gather of 16 B per particle); with one GPU,
+`--mode sharded --sim-ranks R` runs the R shards in turn and reports each rank's time.
 """
 from __future__ import annotations
 
@@ -318,6 +321,100 @@ def run_ours(args, w, rank, world, local_rank, dist):
     ctx.close()
 
 
+def run_sharded(args, w, rank, world, local_rank, dist):
+    """One cluster, target groups split among the ranks: every rank builds the whole tree, evaluates
+    its own Morton range of groups (cost-balanced from the warm-up step's list lengths) and all-gathers acc_pot."""
+    import torch
+    import paper_2110_11658_b200 as p3t
+    from paper_2110_11658_b200 import shard
+
+    p3t.lib()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    n = w.n
+    pm_dev = torch.from_numpy(w.pos_mass).to(dev)
+    out_dev = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    sim = world == 1
+    nranks = max(2, args.sim_ranks) if sim else world
+    ctx = p3t.Context(local_rank)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(r):
+        ctx.build_tree(pm_dev, 63)
+        cuts, _ = ctx.shard_cuts()                        # one small D2H after the build
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0, out=out_dev)
+        if sim:                                           # the rank's half of the exchange; no peers on one GPU
+            ctx.shard_pack(out_dev, chunk)
+        else:
+            shard.exchange(ctx, out_dev, cuts)
+        return cuts
+
+    # step 0 with cuts by particle count, then cuts balanced by the measured cost of every group
+    nominal = None
+    chunk = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    if sim:
+        costs = None
+        for r in range(nranks):
+            ctx.set_shard(r, nranks)
+            step(r)
+            gb, c = shard.gather_group_costs(ctx)
+            costs = c if costs is None else costs + c
+    else:
+        ctx.set_shard(rank, nranks)
+        step(rank)
+        gb, costs = shard.gather_group_costs(ctx)
+    nominal = shard.balanced_cuts(gb, n, costs, nranks)
+
+    sampler = ClockSampler(local_rank)
+    per_rank, launches, n_int = [], 0, 0
+    for r in (range(nranks) if sim else [rank]):
+        ctx.set_shard(r, nranks, nominal)
+        for _ in range(max(3, args.warmup)):
+            step(r)
+        torch.cuda.synchronize()
+        l0 = ctx.stats()["launches"]
+        barrier()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for k in range(args.steps):
+            flush.zero_()
+            ev[k][0].record()
+            step(r)
+            ev[k][1].record()
+        barrier()
+        st = ctx.stats()
+        per_rank.append(float(sum(a.elapsed_time(b) for a, b in ev)))
+        launches += int(st["launches"] - l0)
+        n_int += st["n_pp"] + st["n_pc"]
+    clocks = sampler.stop()
+    total_ms = float(sum(per_rank))                       # simulated: one GPU did every shard in turn
+    total_ms_max, units = reduce_over_ranks(total_ms, float(n) * args.steps / (1 if sim else world), dist)
+    if rank != 0:
+        return
+    line = {
+        "metric": "regular_force_particles_per_s", "value": units / (total_ms_max * 1e-3), "unit": "particles/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms_max / args.steps,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "n": n, "r_out": w.r_out, "r_in": w.r_in, "theta": w.theta, "key_bits": 63,
+                   "l2": "flushed between timed iterations (512 MiB write)",
+                   "parallelism": (f"sharded, {nranks} ranks SIMULATED on one GPU: the shards run in turn, no exchange" if sim
+                                   else f"sharded by target group over {world} ranks, all-gather of acc_pot")},
+        "gpu_launches": launches, "clocks": clocks, "interactions_per_step": n_int if sim else None,
+    }
+    if sim:
+        ms = [t / args.steps for t in per_rank]
+        line["simulated"] = {"ranks": nranks, "ms_per_rank": ms, "cuts": [int(c) for c in nominal],
+                             "projected_ms_per_step": max(ms), "imbalance": max(ms) / (sum(ms) / nranks),
+                             "note": "projection = slowest shard (tree build included on every rank); the all-gather of "
+                                     "16 B x n is not included"}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -328,6 +425,9 @@ def main():
     ap.add_argument("--theta", type=float, default=None)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", choices=["replicas", "sharded"], default="replicas",
+                    help="N > 1: independent replicas (weak scaling, default) or one cluster sharded by target group (strong)")
+    ap.add_argument("--sim-ranks", type=int, default=4, help="--mode sharded on ONE GPU: number of ranks whose shards are run in turn")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -343,7 +443,7 @@ def main():
         torch.cuda.set_device(local_rank)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     w = workloads.make_config(args.config, n_override=args.n, theta=args.theta)
-    run_ours(args, w, rank, world, local_rank, dist)
+    (run_sharded if args.mode == "sharded" else run_ours)(args, w, rank, world, local_rank, dist)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

@@ -40,6 +40,7 @@ extern "C" {
 
 #define P3T_MAX_N   (1ll << 30)
 #define P3T_MAX_NCRIT 64
+#define P3T_MAX_RANKS 64   /* p3t_set_shard */
 
 typedef struct p3t_ctx p3t_ctx;      /* opaque; owns all device scratch */
 
@@ -85,6 +86,32 @@ int p3t_set_tree_params(p3t_ctx* ctx, int nleaf, int ncrit);
  * only (a cheaper point on the accuracy-throughput curve: same walk and lists, the
  * quadrupole of the accepted cells left out).  Takes effect at the next p3t_regular_force. */
 int p3t_set_multipole_order(p3t_ctx* ctx, int order);
+
+/* Multi-GPU (PAPER.md:277-291 names it as future work): the path shards by target group
+ * with no data-path collective.  Every rank calls p3t_build_tree with ALL n bodies (the build is
+ * deterministic, so all ranks hold the identical tree) and p3t_regular_force then walks and evaluates only
+ * the groups of this rank: those whose first sorted particle lies in [cut_rank, cut_rank+1), where cut_r is
+ * the first group boundary at or after a nominal sorted position -- r n / nranks when nominal_cuts is NULL,
+ * else nominal_cuts[r] (HOST int64[nranks + 1], copied; e.g. balanced by the previous step's list lengths).
+ * In a sharded context p3t_regular_force writes acc_pot (and kicks vel) only for the owned particles --
+ * the other entries are unspecified -- neighbour rows and list lengths of the other particles / groups
+ * are empty, and the statistics count the own interactions.  nranks = 1 restores the whole path.
+ * 1 <= nranks <= P3T_MAX_RANKS, 0 <= rank < nranks.  Takes effect at the next p3t_build_tree. */
+int p3t_set_shard(p3t_ctx* ctx, int rank, int nranks, const int64_t* nominal_cuts);
+
+/* The group-aligned cuts of ALL ranks after p3t_build_tree, identical on every rank: cuts_host[r]
+ * (HOST int64[nranks + 1]) = first sorted position of rank r, cuts_host[nranks] = n; group_cuts_host
+ * (HOST int32[nranks + 1], may be NULL) = the same as group indices.  Synchronises.  P3T_ESTATE if the
+ * context is not sharded or not built. */
+int p3t_get_shard_cuts(p3t_ctx* ctx, int64_t* cuts_host, int32_t* group_cuts_host);
+
+/* The exchange step: p3t_shard_pack gathers the owned entries of a per-particle DEVICE float4[n] array in
+ * original order (acc_pot of p3t_regular_force) into one contiguous DEVICE chunk of cuts[rank+1] - cuts[rank]
+ * float4 in sorted order; p3t_shard_unpack scatters the chunk of rank from_rank (as received from it, e.g. by
+ * an NCCL all-gather) back into original order.  After unpacking every rank's chunk the array is complete and
+ * equal, bit for bit, to that of an unsharded context.  16-byte aligned pointers.  Do not synchronise. */
+int p3t_shard_pack(p3t_ctx* ctx, const void* acc_pot, void* chunk);
+int p3t_shard_unpack(p3t_ctx* ctx, int from_rank, const void* chunk, void* acc_pot);
 
 /* Steps a1-a6: bounding cube, Morton keys (key_bits = 30 or 63), stable radix sort,
  * body permutation, canonical octree, monopole + traceless quadrupole moments, target groups.

@@ -25,6 +25,7 @@ SYMBOLS = [
     "p3t_regular_force_ex", "p3t_irregular_force", "p3t_core_quantities", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_pipe_bench", "p3t_strerror", "p3t_last_error", "p3t_params_from_n", "p3t_regularisation_params",
+    "p3t_set_shard", "p3t_get_shard_cuts", "p3t_shard_pack", "p3t_shard_unpack",
 ]
 
 
@@ -86,6 +87,10 @@ def lib() -> C.CDLL:
     L.p3t_get_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     L.p3t_get_groups.argtypes = [vp, vp, vp]
     L.p3t_get_list_lengths.argtypes = [vp, vp, vp]
+    L.p3t_set_shard.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.p3t_get_shard_cuts.argtypes = [vp, vp, vp]
+    L.p3t_shard_pack.argtypes = [vp, vp, vp]
+    L.p3t_shard_unpack.argtypes = [vp, C.c_int, vp, vp]
     L.p3t_pipe_bench.argtypes = [C.c_int, C.POINTER(dbl), C.c_int, C.POINTER(dbl), C.POINTER(C.c_int)]
     L.p3t_strerror.argtypes = [C.c_int]; L.p3t_strerror.restype = C.c_char_p
     L.p3t_last_error.argtypes = [vp]; L.p3t_last_error.restype = C.c_char_p
@@ -133,6 +138,7 @@ class Context:
         self._check(lib().p3t_create(C.byref(h), device, sp), "p3t_create", ctx=None)
         self._h = h
         self.n = 0
+        self.shard = (0, 1)
         self._check(lib().p3t_set_tree_params(self._h, nleaf, ncrit), "p3t_set_tree_params")
 
     # -- plumbing --
@@ -174,6 +180,34 @@ class Context:
     def set_multipole_order(self, order: int):
         """2 = monopole + quadrupole (default), 1 = monopole only."""
         self._check(lib().p3t_set_multipole_order(self._h, order), "p3t_set_multipole_order")
+
+    # -- multi-GPU: target groups split among ranks (SURVEY 8e; the exchange is in paper_2110_11658_b200.shard) --
+    def set_shard(self, rank: int, nranks: int, nominal_cuts=None):
+        """This context evaluates the groups of one Morton range (rank of nranks); takes effect at the next
+        build_tree.  nominal_cuts: nranks + 1 sorted positions (default r n / nranks)."""
+        import numpy as np
+        c = None
+        if nominal_cuts is not None:
+            c = np.ascontiguousarray(nominal_cuts, dtype=np.int64)
+            assert c.shape == (nranks + 1,)
+        self._check(lib().p3t_set_shard(self._h, rank, nranks, None if c is None else _np_ptr(c)), "p3t_set_shard")
+        self.shard = (rank, nranks)
+
+    def shard_cuts(self):
+        """(cuts, group_cuts): numpy int64 / int32 [nranks + 1], the group-aligned ranges of all ranks."""
+        import numpy as np
+        nr = self.shard[1]
+        c = np.empty(nr + 1, np.int64); g = np.empty(nr + 1, np.int32)
+        self._check(lib().p3t_get_shard_cuts(self._h, _np_ptr(c), _np_ptr(g)), "p3t_get_shard_cuts")
+        return c, g
+
+    def shard_pack(self, acc_pot, chunk):
+        """chunk[: cuts[rank+1] - cuts[rank]] = the owned rows of acc_pot, in sorted order."""
+        self._check(lib().p3t_shard_pack(self._h, self._dev_f32(acc_pot, 4), self._dev_f32(chunk, 4)), "p3t_shard_pack")
+
+    def shard_unpack(self, from_rank: int, chunk, acc_pot):
+        """Scatter the chunk of rank from_rank into acc_pot (original order)."""
+        self._check(lib().p3t_shard_unpack(self._h, from_rank, self._dev_f32(chunk, 4), self._dev_f32(acc_pot, 4)), "p3t_shard_unpack")
 
     def regular_force(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, out=None,
                       r_buff: float = 0.0, half_dt: float = 0.0, vel=None):

@@ -54,7 +54,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     if (!c) return P3T_ENOMEM;
     memset(c, 0, sizeof(*c));
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
-    c->nleaf = 16; c->ncrit = 64; c->order = 2;
+    c->nleaf = 16; c->ncrit = 64; c->order = 2; c->shard_nranks = 1;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
     for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
@@ -78,7 +78,7 @@ int p3t_destroy(p3t_ctx* c)
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->nbcnt, &c->part, &c->spill, &c->pcpool, &c->pppool, &c->glist,
-                        &c->info, &c->stage_in, &c->stage_out, &c->core };
+                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
@@ -101,6 +101,23 @@ int p3t_set_multipole_order(p3t_ctx* c, int order)
 {
     if (!c || (order != 1 && order != 2)) return P3T_EINVAL;
     c->order = order;
+    return P3T_OK;
+}
+
+int p3t_set_shard(p3t_ctx* c, int rank, int nranks, const int64_t* nominal_cuts)
+{
+    if (!c || nranks < 1 || nranks > P3T_MAX_RANKS || rank < 0 || rank >= nranks) return P3T_EINVAL;
+    if (c->sticky) return P3T_ECUDA;
+    c->shard_rank = rank; c->shard_nranks = nranks; c->shard_has_nominal = 0;
+    if (nominal_cuts && nranks > 1) {
+        P3T_CUDA(c, cudaSetDevice(c->device));
+        int rc = p3t_reserve(c, &c->shard_nominal, (size_t)(nranks + 1) * 8);
+        if (rc) return rc;
+        P3T_CUDA(c, cudaMemcpyAsync(c->shard_nominal.p, nominal_cuts, (size_t)(nranks + 1) * 8, cudaMemcpyHostToDevice, c->stream));
+        P3T_CUDA(c, cudaStreamSynchronize(c->stream));       // the caller's array may go away
+        c->shard_has_nominal = 1;
+    }
+    c->state = 0;                                            // the shard takes effect at the next build
     return P3T_OK;
 }
 

@@ -401,7 +401,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
     __shared__ tile_smem smem[FORCE_WARPS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     tile_smem& S = smem[w];
-    const int ng = A.info->n_groups;
+    const int ng = A.info->shard_g1 - A.info->shard_g0;          // all groups unless the context is sharded (p3t_shard.cu)
     // cursor ranges of the passes: [0, 2 ng) chunks 0-1 (k = 1), [2 ng, 3 ng) chunk 2 (k = 2), [3 ng, 4 ng) chunk 3 (the rest)
     for (;;) {
         int c = 0;
@@ -414,6 +414,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         if (c < 2 * ng)      { g = c >> 1; j = c & 1; }
         else if (c < 3 * ng) { g = c - 2 * ng; j = 2; }
         else                 { g = c - 3 * ng; j = 3; }
+        g += A.info->shard_g0;
         const int gb = A.gbegin[g], n = A.gbegin[g + 1] - gb;
         const int full = n >> 5, r = n & 31;
         int tb, len;
@@ -541,6 +542,12 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     if ((rc = p3t_reserve(ctx, &ctx->nbcur, (size_t)nsb * 8 + 64))) return rc;
 
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
+    if (ctx->shard_nranks > 1) {
+        // a sharded context walks only its own groups: rows and list lengths of the others are empty
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcount.p, 0, (size_t)n * 4, ctx->stream));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpp.p, 0, ((size_t)n + 1) * 4, ctx->stream));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpc.p, 0, ((size_t)n + 1) * 4, ctx->stream));
+    }
     // a10, sizes: neighbour counts (range search only) -> CSR offsets, so that the lists can be written in place
     if ((rc = p3t_launch_walk_count(ctx, r_list, theta))) return rc;
     k_nb_blocksum<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), INFO(ctx));
@@ -585,7 +592,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     // a8, a9, a11: the force kernel.  A problem with fewer work items (about 1.4 per 32 particles) than
     // three per resident warp shares every item among nseg warps (SPLIT), so that small N still fills the GPU.
     const long long warps = (long long)per_sm * ctx->num_sms * FORCE_WARPS;
-    const long long items = (long long)n * 14 / 320 + 1;
+    const long long items = (long long)n / ctx->shard_nranks * 14 / 320 + 1;
     int nseg = 1;
     while (nseg < 8 && items * nseg < 3 * warps) nseg *= 2;
     A.nseg = nseg; A.n = n; A.nbcnt = nullptr; A.part = nullptr;

@@ -34,6 +34,7 @@ struct p3t_devinfo {
     int32_t  pool_overflow;  // a walker warp ran out of list space (the call is repeated with larger pools)
     uint32_t need_pc, need_pp; // largest per-warp list space used, in entries
     uint32_t minmax[6];      // order-preserving uint encodings of min xyz / max xyz
+    int32_t  shard_g0, shard_g1; // target groups of this context's shard (all groups unless p3t_set_shard)
 };
 
 struct p3t_buf { void* p; size_t bytes; };
@@ -86,6 +87,10 @@ struct p3t_ctx {
     int irr_done;
     p3t_stats last;
     float r_out, r_in, theta, r_list;
+    int shard_rank, shard_nranks;    // p3t_set_shard: this context walks the groups of one Morton range
+    p3t_buf shard_nominal;           // int64[nranks+1]: caller's cuts in sorted positions (unused when shard_has_nominal = 0)
+    p3t_buf shard_cuts;              // int32[2][nranks+1]: group-aligned cuts as group index / sorted position
+    int shard_has_nominal;
     int64_t launches;                // kernels launched so far
 };
 
@@ -108,6 +113,8 @@ int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
 // p3t_tree.cu : a4-a6
 int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
+// p3t_shard.cu : SURVEY 8e, target groups split among the ranks of a node
+int p3t_launch_shard_range(p3t_ctx* ctx);
 // p3t_walk.cu : a7 (interaction lists), a10 (neighbour counts)
 int p3t_walk_init(p3t_ctx* ctx);
 int p3t_launch_walk_count(p3t_ctx* ctx, float r_list, float theta);   // r_list: neighbour search radius (>= r_out)

@@ -379,7 +379,7 @@ __global__ void __launch_bounds__(1024) k_group_scan(tree_args A, int nb)
         if (threadIdx.x == 0) s_run += tot;
         __syncthreads();
     }
-    if (threadIdx.x == 0) { A.gbegin[s_run] = A.n; A.info->n_groups = s_run; }
+    if (threadIdx.x == 0) { A.gbegin[s_run] = A.n; A.info->n_groups = s_run; A.info->shard_g0 = 0; A.info->shard_g1 = s_run; }
 }
 
 __global__ void __launch_bounds__(GC_THREADS) k_group_compact(tree_args A)
@@ -442,5 +442,6 @@ int p3t_launch_tree(p3t_ctx* ctx)
     k_group_compact<<<gcb, GC_THREADS, 0, st>>>(A);
     P3T_CUDA(ctx, cudaGetLastError());
     ctx->launches += 9;
+    if (ctx->shard_nranks > 1) return p3t_launch_shard_range(ctx);
     return P3T_OK;
 }

@@ -237,11 +237,11 @@ __global__ void __launch_bounds__(WALK_THREADS) k_walk(walk_args A)
     int32_t* spill = A.spill + wg * SPILL_CAP;
     long long pc_ptr = wg * A.cap_pc, pp_ptr = wg * A.cap_pp;
     const long long pc_base = pc_ptr, pp_base = pp_ptr, pc_end = pc_ptr + A.cap_pc, pp_end = pp_ptr + A.cap_pp;
-    const int ng = A.info->n_groups;
+    const int g0 = A.info->shard_g0, ng = A.info->shard_g1;      // all groups unless the context is sharded (p3t_shard.cu)
     uint32_t* cursor = MODE == WALK_LISTS ? &A.info->group_cursor : &A.info->group_cursor2;
     for (;;) {
         int g = 0;
-        if (lane == 0) g = (int)atomicAdd(cursor, 1u);
+        if (lane == 0) g = g0 + (int)atomicAdd(cursor, 1u);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ng) break;
         walk_group<MODE>(A, S, &csm[MODE == WALK_COUNT ? w : 0], spill, g, A.gbegin[g], A.gbegin[g + 1], s_lt, pc_ptr, pc_end, pp_ptr, pp_end);
