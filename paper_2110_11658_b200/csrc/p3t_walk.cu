@@ -139,7 +139,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
         const bool leaf  = valid && open && link.y < 0;
         const bool acc   = MODE == WALK_LISTS && valid && !open;
         // children of opened internal cells go on the stack
-        {
+        if (__any_sync(0xffffffffu, inner)) {
             int c = inner ? link.y : 0, x = c;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
@@ -160,10 +160,12 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
         }
         // opened leaves: inclusive scan of their particle counts; particle k of this iteration's leaves
         // belongs to the first lane whose inclusive count exceeds k (binary search by shuffle)
-        int lc_incl = leaf ? -link.y : 0;
+        int lc_incl = leaf ? -link.y : 0, src_total = 0;
+        if (__any_sync(0xffffffffu, leaf)) {
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, lc_incl, o); if (lane >= o) lc_incl += y; }
-        const int src_total = __shfl_sync(0xffffffffu, lc_incl, 31);
+            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, lc_incl, o); if (lane >= o) lc_incl += y; }
+            src_total = __shfl_sync(0xffffffffu, lc_incl, 31);
+        }
         const int lc_excl = lc_incl - (leaf ? -link.y : 0);
         npp += src_total;
         for (int k0 = 0; k0 < src_total; k0 += 32) {
