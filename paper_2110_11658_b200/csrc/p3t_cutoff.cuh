@@ -14,6 +14,7 @@ struct walk_consts {
     float rem;                             // c^3 (1+c)^3  (> 0)
     float c;                               // r_in / (r_out - r_in)
     double dk140, ds1, dsc[6], drem, dc;   // the same in fp64 (cutoff_psi64)
+    double dlog1c;                         // log(1 + c)
     float theta;
     int   pot_mode;
 };
@@ -44,7 +45,7 @@ __device__ __forceinline__ float cutoff_psi64(const walk_consts& K, float xf, fl
 {
     const double x = (double)xf;
     const double sx = x * (K.dsc[0] + x * (K.dsc[1] + x * (K.dsc[2] + x * (K.dsc[3] + x * (K.dsc[4] + x * K.dsc[5])))));
-    const double integral = (K.ds1 - sx) - K.drem * log((1.0 + K.dc) / (x + K.dc));
+    const double integral = (K.ds1 - sx) - K.drem * (K.dlog1c - log(x + K.dc));
     return (float)(-(double)W * (double)rinv - K.dk140 * integral);
 }
 
@@ -65,7 +66,7 @@ static inline void make_consts(walk_consts& K, float r_out, float r_in, float th
     for (int k = 0; k < 6; ++k) { K.dsc[k] = b[k] / (k + 1); K.sc[k] = (float)K.dsc[k]; s1 += b[k] / (k + 1); }
     K.s1 = (float)s1; K.ds1 = s1;
     K.drem = c * c * c * c1 * c1 * c1; K.rem = (float)K.drem;
-    K.c = (float)c; K.dc = c;
+    K.c = (float)c; K.dc = c; K.dlog1c = log(c1);
     // psi(r_in) = -(140/D) [ S(1) + rem ln((1+c)/c) ... ] with W(0) = 0; here the remainder enters with a minus sign
     K.psi_in = (float)(-(140.0 / D) * (s1 - c * c * c * c1 * c1 * c1 * log(c1 / c)));
     K.theta = theta;

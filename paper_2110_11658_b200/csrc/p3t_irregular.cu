@@ -29,10 +29,12 @@ struct irr_args {
 
 struct irr_sum { double ax, ay, az, jx, jy, jz, ph; };
 
-__device__ __forceinline__ void irr_term(const irr_args& A, const float4 pi, const float4 vi, int j, irr_sum& S)
+struct irr_src { float4 p, v; };
+
+__device__ __forceinline__ void irr_term(const irr_args& A, const float4 pi, const float4 vi, const irr_src src, irr_sum& S)
 {
     const walk_consts& K = A.K;
-    const float4 pj = A.spm[A.rank[j]], vj = A.vel[j];
+    const float4 pj = src.p, vj = src.v;
     const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (!(r2 > 0.0f)) return;                                    // coincident pair (R8)
@@ -58,6 +60,32 @@ __device__ __forceinline__ void irr_term(const irr_args& A, const float4 pi, con
     S.ph += (double)(m * ph);
 }
 
+// The entries first + k stride, k < cnt, of one row, in order.  The kernel is bound by the latency of the
+// dependent gathers index -> rank -> (position, velocity): they are staged over four iterations, so that every
+// load issued in an iteration depends only on values that arrived during earlier ones (indices are clamped to
+// the row, which keeps every staged load valid without predicates).
+__device__ __forceinline__ void irr_row(const irr_args& A, const float4 pi, const float4 vi, const int32_t* __restrict__ idx,
+                                        int first, int cnt, int stride, irr_sum& S)
+{
+    if (cnt <= 0) return;
+    const int last = cnt - 1;
+    int j1 = idx[first], j2 = idx[first + min(1, last) * stride], j3 = idx[first + min(2, last) * stride],
+        j4 = idx[first + min(3, last) * stride];
+    int r1 = A.rank[j1], r2 = A.rank[j2], r3 = A.rank[j3];
+    irr_src c1, c2;
+    c1.p = A.spm[r1]; c1.v = A.vel[j1];
+    c2.p = A.spm[r2]; c2.v = A.vel[j2];
+#pragma unroll 1
+    for (int k = 0; k < cnt; ++k) {
+        const irr_src cur = c1;
+        c1 = c2;
+        c2.p = A.spm[r3]; c2.v = A.vel[j3];                    // entry k + 2
+        r3 = A.rank[j4]; j3 = j4;                              // entry k + 3
+        j4 = idx[first + min(k + 4, last) * stride];           // entry k + 4
+        irr_term(A, pi, vi, cur, S);
+    }
+}
+
 __global__ void __launch_bounds__(256) k_irregular(irr_args A)
 {
     // threads take the particles in Morton order: the rows of a warp are neighbours in space, so they
@@ -67,8 +95,7 @@ __global__ void __launch_bounds__(256) k_irregular(irr_args A)
     float4 pi = make_float4(0, 0, 0, 0), vi = pi;
     if (sp < A.n) { i = (int)A.order[sp]; b = A.nboff[i]; len = (int)(A.nboff[i + 1] - b); pi = A.spm[sp]; vi = A.vel[i]; }
     irr_sum S = { 0, 0, 0, 0, 0, 0, 0 };
-    if (len <= 32)
-        for (int k = 0; k < len; ++k) irr_term(A, pi, vi, A.nbidx[b + k], S);
+    if (len <= 32) irr_row(A, pi, vi, A.nbidx + b, 0, len, 1, S);
     // rows longer than a warp: all 32 lanes share the row, partial sums reduced by shuffle (fixed order)
     uint32_t m = __ballot_sync(0xffffffffu, len > 32);
     while (m) {
@@ -81,7 +108,7 @@ __global__ void __launch_bounds__(256) k_irregular(irr_args A)
         v.x = __shfl_sync(0xffffffffu, vi.x, src); v.y = __shfl_sync(0xffffffffu, vi.y, src);
         v.z = __shfl_sync(0xffffffffu, vi.z, src); v.w = 0.0f;
         irr_sum R = { 0, 0, 0, 0, 0, 0, 0 };
-        for (int k = lane; k < rl; k += 32) irr_term(A, p, v, A.nbidx[rb + k], R);
+        irr_row(A, p, v, A.nbidx + rb, lane, (rl - lane + 31) >> 5, 32, R);
         double* r = &R.ax;
 #pragma unroll
         for (int c = 0; c < 7; ++c)
