@@ -48,7 +48,7 @@ struct __align__(16) warp_smem {
     int   ppid[64];             // WALK_LISTS: sorted positions of leaf particles, likewise
 };
 struct __align__(16) count_smem {   // WALK_COUNT: positions of the leaf particles of one round
-    float x[32], y[32], z[32]; int j[32];
+    float x[32], y[32], z[32];
 };
 
 __device__ __forceinline__ int stack_get(const warp_smem& S, const int32_t* spill, int i)
@@ -186,13 +186,26 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
                 list_flush(S.ppid, fill_pp, A.pppool, pp_ptr, pp_end, lane, ovf);
             } else {
                 // R10 neighbour predicate, bit-specified fp32, for the 32 particles of this round
-                if (lane < m) { const float4 p = A.spm[j]; C->x[lane] = p.x; C->y[lane] = p.y; C->z[lane] = p.z; C->j[lane] = j; }
+                // only the particles within r_out of the group box can be anyone's neighbour: the box distance below is
+                // built from the same monotone fp32 operations as R10's d2, so it never exceeds the d2 to a target
+                // inside the box and the cull is exact
+                bool keep = false; float4 p = make_float4(0, 0, 0, 0);
+                if (lane < m) {
+                    p = A.spm[j];
+                    const float fx = fmaxf(fmaxf(0.0f, __fsub_rn(glo[0], p.x)), __fsub_rn(p.x, ghi[0]));
+                    const float fy = fmaxf(fmaxf(0.0f, __fsub_rn(glo[1], p.y)), __fsub_rn(p.y, ghi[1]));
+                    const float fz = fmaxf(fmaxf(0.0f, __fsub_rn(glo[2], p.z)), __fsub_rn(p.z, ghi[2]));
+                    keep = fmaf(fz, fz, fmaf(fy, fy, __fmul_rn(fx, fx))) < A.rout2;
+                }
+                const uint32_t km = __ballot_sync(0xffffffffu, keep);
+                if (keep) { const int q = __popc(km & lt_mask); C->x[q] = p.x; C->y[q] = p.y; C->z[q] = p.z; }
+                const int ms = __popc(km);
                 __syncwarp();
                 // both target slots of the lane in one packed operation; d = x_i - x_j here, the exact negative of
                 // R10's x_j - x_i, so d2 has the same bits.  Self (always met: its own leaf is opened) is counted
                 // and taken off at the end, which spares the index test in the loop.
                 const f2 TX = pk(tx[0], tx[1]), TY = pk(ty[0], ty[1]), TZ = pk(tz[0], tz[1]);
-                for (int e = 0; e < m; ++e) {
+                for (int e = 0; e < ms; ++e) {
                     const float px = C->x[e], py = C->y[e], pz = C->z[e];
                     const f2 dx = sub2(TX, pk(px, px)), dy = sub2(TY, pk(py, py)), dz = sub2(TZ, pk(pz, pz));
                     const f2 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
