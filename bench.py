@@ -39,7 +39,7 @@ if str(ROOT) not in sys.path:
 INSTR_PP, INSTR_PC = 15, 37
 FLOP_PP, FLOP_PC = 20, 60
 # DRAM traffic of the dominant kernel from the committed ncu capture (profiles/), per launch, by workload
-TRAFFIC_NCU = {"plummer1m_kroupa": 1714.2e6}
+TRAFFIC_NCU = {"plummer1m_kroupa": 1515.9e6}
 
 
 def peaks():
