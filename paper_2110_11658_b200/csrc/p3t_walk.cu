@@ -145,8 +145,13 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
             for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
             const int total = __shfl_sync(0xffffffffu, x, 31);
             if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
-            int w = top + x - c;
-            for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
+            const int w = top + x - c;
+            if (top + total <= STACK_CAP) {                    // warp-uniform: everything stays in shared memory
+#pragma unroll
+                for (int k = 0; k < 8; ++k) if (k < c) S.stack[w + k] = link.x + k;
+            } else {
+                for (int k = 0; k < c; ++k) stack_put(S, spill, w + k, link.x + k);
+            }
             top += total;
         }
         // accepted cells: their ids go on the particle-cell list
