@@ -135,7 +135,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     if (cap > 0x7fffff00ll) cap = 0x7fffff00ll;
     c->node_cap = cap;
     const size_t N = (size_t)n, C = (size_t)cap;
-    const size_t ntiles = (N + P3T_SORT_TILE - 1) / P3T_SORT_TILE;
+    const size_t ntiles = (N + P3T_SORT_TILE_MIN - 1) / P3T_SORT_TILE_MIN;
     int rc;
 #define RES(buf, bytes) if ((rc = p3t_reserve(c, &c->buf, (bytes))) != P3T_OK) return rc
     RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16); RES(rank, N * 4);

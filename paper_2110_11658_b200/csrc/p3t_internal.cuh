@@ -9,8 +9,8 @@
 #define P3T_RADIX_BITS 8
 #define P3T_RADIX      256
 #define P3T_SORT_THREADS 256
-#define P3T_SORT_ITEMS   16                                  // keys per thread in one sort tile
-#define P3T_SORT_TILE    (P3T_SORT_THREADS * P3T_SORT_ITEMS) // 4096 keys per block
+#define P3T_SORT_ITEMS_MIN 4                                 // keys per thread in one sort tile: 4 (n <= 2^18) or 8
+#define P3T_SORT_TILE_MIN  (P3T_SORT_THREADS * P3T_SORT_ITEMS_MIN) // the smallest tile sizes the histogram buffer
 
 // device-side counters written by the build and force kernels (one 256-byte record)
 struct p3t_devinfo {

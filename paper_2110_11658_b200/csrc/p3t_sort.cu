@@ -107,15 +107,16 @@ __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pm, int
 //     k_scan   exclusive scan of every digit row, row totals
 //     k_scatter stable ranking inside the tile (warp match + per-warp counters) and scatter
 // ---------------------------------------------------------------------------------------------
+template <int ITEMS>
 __global__ void __launch_bounds__(P3T_SORT_THREADS) k_hist(const uint64_t* __restrict__ keys, int n, int shift,
                                                            uint32_t* __restrict__ hist, int ntiles)
 {
     __shared__ uint32_t h[P3T_RADIX];
     h[threadIdx.x] = 0;
     __syncthreads();
-    const int base = blockIdx.x * P3T_SORT_TILE;
+    const int base = blockIdx.x * (P3T_SORT_THREADS * ITEMS);
 #pragma unroll 4
-    for (int k = 0; k < P3T_SORT_ITEMS; ++k) {
+    for (int k = 0; k < ITEMS; ++k) {
         int i = base + k * P3T_SORT_THREADS + threadIdx.x;
         if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
     }
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(256) k_scan_rows(uint32_t* __restrict__ hist, 
     if (lane == 0) totals[d] = run;
 }
 
-template <bool FIRST>
+template <bool FIRST, int ITEMS>
 __global__ void __launch_bounds__(P3T_SORT_THREADS) k_scatter(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                                                               uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                               int n, int shift, const uint32_t* __restrict__ hist, int ntiles,
@@ -163,17 +164,17 @@ __global__ void __launch_bounds__(P3T_SORT_THREADS) k_scatter(const uint64_t* __
         s_scan[threadIdx.x] = add + x - v + hist[(size_t)threadIdx.x * ntiles + blockIdx.x];
     }
     __syncthreads();
-    const int base = blockIdx.x * P3T_SORT_TILE + w * (32 * P3T_SORT_ITEMS);
-    uint64_t key[P3T_SORT_ITEMS];
-    uint32_t rank[P3T_SORT_ITEMS];
+    const int base = blockIdx.x * (P3T_SORT_THREADS * ITEMS) + w * (32 * ITEMS);
+    uint64_t key[ITEMS];
+    uint32_t rank[ITEMS];
 #pragma unroll
-    for (int r = 0; r < P3T_SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
         key[r] = i < n ? kin[i] : ~0ull;
     }
     const uint32_t lt = (1u << lane) - 1u;
 #pragma unroll
-    for (int r = 0; r < P3T_SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
         uint32_t d = i < n ? ((uint32_t)(key[r] >> shift) & 255u) : 256u;
         uint32_t peers = __match_any_sync(0xffffffffu, d);
@@ -192,7 +193,7 @@ __global__ void __launch_bounds__(P3T_SORT_THREADS) k_scatter(const uint64_t* __
     }
     __syncthreads();
 #pragma unroll
-    for (int r = 0; r < P3T_SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
         if (i < n) {
             uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
@@ -224,10 +225,14 @@ int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pm)
     return P3T_OK;
 }
 
-int p3t_launch_sort(p3t_ctx* ctx)
+// Tiles of 2048 keys (8 per thread); 1024 below 2^18 particles, where the shorter serial chain of a block and
+// the larger grid matter more than the size of the histogram (measured: sort 0.19 -> 0.12 ms at N = 2^14).
+template <int ITEMS>
+static int sort_passes(p3t_ctx* ctx)
 {
     const int n = (int)ctx->n;
-    const int ntiles = (n + P3T_SORT_TILE - 1) / P3T_SORT_TILE;
+    const int tile = P3T_SORT_THREADS * ITEMS;
+    const int ntiles = (n + tile - 1) / tile;
     const int passes = (3 * ctx->bits + P3T_RADIX_BITS - 1) / P3T_RADIX_BITS;     // 8 (63-bit) or 4 (30-bit)
     uint32_t* hist = P<uint32_t>(ctx->hist);
     uint32_t* totals = hist + (size_t)P3T_RADIX * ntiles;
@@ -236,10 +241,10 @@ int p3t_launch_sort(p3t_ctx* ctx)
         const int shift = p * P3T_RADIX_BITS;
         uint64_t* kin = P<uint64_t>(ctx->keys[cur]);  uint64_t* kout = P<uint64_t>(ctx->keys[cur ^ 1]);
         uint32_t* vin = P<uint32_t>(ctx->idx[cur]);   uint32_t* vout = P<uint32_t>(ctx->idx[cur ^ 1]);
-        k_hist<<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, n, shift, hist, ntiles);
+        k_hist<ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, n, shift, hist, ntiles);
         k_scan_rows<<<P3T_RADIX / 8, 256, 0, ctx->stream>>>(hist, ntiles, totals);
-        if (p == 0) k_scatter<true><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
-        else        k_scatter<false><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
+        if (p == 0) k_scatter<true, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
+        else        k_scatter<false, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
         cur ^= 1;
         ctx->launches += 3;
     }
@@ -250,6 +255,11 @@ int p3t_launch_sort(p3t_ctx* ctx)
         t = ctx->idx[0]; ctx->idx[0] = ctx->idx[1]; ctx->idx[1] = t;
     }
     return P3T_OK;
+}
+
+int p3t_launch_sort(p3t_ctx* ctx)
+{
+    return ctx->n <= (1 << 18) ? sort_passes<P3T_SORT_ITEMS_MIN>(ctx) : sort_passes<8>(ctx);
 }
 
 int p3t_launch_permute(p3t_ctx* ctx, const float4* pm)
