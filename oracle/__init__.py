@@ -73,6 +73,8 @@ def lib() -> C.CDLL:
         _lib.p3t_o_tree_force_order.restype = None
         _lib.p3t_o_tree_force_order.argtypes = [vp, C.c_int, f32, f32, f32, f32, C.c_int, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_pc_term.restype = None; _lib.p3t_o_pc_term.argtypes = [vp, vp, vp, vp]
+        _lib.p3t_o_pc_octupole.restype = None; _lib.p3t_o_pc_octupole.argtypes = [vp, vp, vp, vp]
+        _lib.p3t_o_tree_octupoles.restype = None; _lib.p3t_o_tree_octupoles.argtypes = [vp, vp, vp]
         _lib.p3t_o_open_test.restype = C.c_int
         _lib.p3t_o_open_test.argtypes = [vp, vp, vp, vp, vp, f32, f32, f32, f32]
         _lib.p3t_o_interleave.restype = C.c_uint64
@@ -218,6 +220,14 @@ class Tree:
         lib().p3t_o_tree_moments64(self._h, _p(mass), _p(com), _p(quad))
         return dict(mass=mass, com=com, quad=quad)
 
+    def octupoles(self):
+        """Raw third moments about the COM per node, order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz:
+        dict(oct32 [nn,10] fp32-rounded, oct64 [nn,10])."""
+        nn = self.n_nodes
+        f = np.zeros((nn, 10), np.float32); d = np.zeros((nn, 10))
+        lib().p3t_o_tree_octupoles(self._h, _p(f), _p(d))
+        return dict(oct32=f, oct64=d)
+
     def groups(self):
         ng = self.n_groups
         b = np.zeros(ng, np.int32); e = np.zeros(ng, np.int32)
@@ -244,6 +254,16 @@ def pc_term(xi, com_m, quad) -> np.ndarray:
     cm = np.ascontiguousarray(com_m, dtype=np.float32); q = np.ascontiguousarray(quad, dtype=np.float32)
     out = np.zeros(4)
     lib().p3t_o_pc_term(_p(xi), _p(cm), _p(q), _p(out))
+    return out
+
+
+def pc_octupole(xi, com_m, oct) -> np.ndarray:
+    """The octupole term alone: {ax, ay, az, phi}."""
+    xi = np.ascontiguousarray(xi, dtype=np.float64)
+    cm = np.ascontiguousarray(com_m, dtype=np.float32); t = np.ascontiguousarray(oct, dtype=np.float32)
+    assert t.shape == (10,)
+    out = np.zeros(4)
+    lib().p3t_o_pc_octupole(_p(xi), _p(cm), _p(t), _p(out))
     return out
 
 

@@ -74,6 +74,8 @@ void p3t_o_tree_nodes(const p3t_o_tree* t, int32_t* level, int32_t* begin, int32
 void p3t_o_tree_moments(const p3t_o_tree* t, float* com_m, float* quad, float* clo, float* chi, float* delta);
 /* unrounded fp64 moments: mass, com[3], quad[6] */
 void p3t_o_tree_moments64(const p3t_o_tree* t, double* mass, double* com, double* quad);
+/* raw third moments about the COM per node [nn][10]: fp32-rounded and fp64 (either may be NULL) */
+void p3t_o_tree_octupoles(const p3t_o_tree* t, float* foct, double* oct);
 void p3t_o_tree_groups(const p3t_o_tree* t, int32_t* begin, int32_t* end, float* glo, float* ghi);
 
 /* Tree force for ng groups (ids into the group list; NULL = all).  acc_pot: n x 4 fp64 in
@@ -90,13 +92,15 @@ void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list, float r_out, f
                                int64_t ng, const int64_t* group_ids, double* acc_pot,
                                int64_t* npp, int64_t* npc, double* abs_sum);
 
-/* the same with the multipole order chosen: 2 = monopole + quadrupole, 1 = monopole only */
+/* the same with the multipole order chosen: 2 = monopole + quadrupole, 1 = monopole only, 3 = + octupole */
 void p3t_o_tree_force_order(const p3t_o_tree* t, int order, float r_list, float r_out, float r_in, float theta, int pot_mode,
                             int64_t ng, const int64_t* group_ids, double* acc_pot,
                             int64_t* npp, int64_t* npc, double* abs_sum);
 
 /* single particle-cell term (fp64) from fp32 node data: out = {ax, ay, az, phi} */
 void p3t_o_pc_term(const double xi[3], const float com_m[4], const float quad[6], double out[4]);
+/* octupole term of the same expansion, ADDED to out; T = raw third moment about the COM, order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz */
+void p3t_o_pc_octupole(const double xi[3], const float com_m[4], const float T[10], double out[4]);
 /* the fp32 opening test alone (R7): returns 1 = open */
 int  p3t_o_open_test(const float glo[3], const float ghi[3], const float com[3], const float clo[3],
                      const float chi[3], float l, float delta, float theta, float r_out);

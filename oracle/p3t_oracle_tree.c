@@ -159,10 +159,13 @@ p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pm, int key_bits, int nleaf
      * M = sum m; COM = sum m x / M; Q_ab = sum m (3 d_a d_b - |d|^2 delta_ab), d = x - COM
      * (traceless quadrupole; order xx yy zz xy xz yz); tight AABB = exact min/max;
      * delta = |COM - c_geo|, c_geo,a = lo_a + (p_a + 1/2) l, l = side / 2^level.
-     * M, COM, Q, delta are rounded once to fp32. */
+     * M, COM, Q, delta are rounded once to fp32.
+     * SURVEY 8f NEXT-4 (octupole variant): T_abc = sum m d_a d_b d_c, the raw third moment about the COM,
+     * order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz, likewise rounded once to fp32. */
     int64_t nn = t->nn;
     t->mass = malloc(sizeof(double) * nn); t->com = malloc(sizeof(double) * 3 * nn); t->quad = malloc(sizeof(double) * 6 * nn);
     t->fcom_m = malloc(sizeof(float) * 4 * nn); t->fquad = malloc(sizeof(float) * 6 * nn);
+    t->oct = malloc(sizeof(double) * 10 * nn); t->foct = malloc(sizeof(float) * 10 * nn);
     t->clo = malloc(sizeof(float) * 3 * nn); t->chi = malloc(sizeof(float) * 3 * nn); t->delta = malloc(sizeof(float) * nn);
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t k = 0; k < nn; ++k) {
@@ -181,13 +184,16 @@ p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pm, int key_bits, int nleaf
             }
         }
         double c[3] = { s[0] / M, s[1] / M, s[2] / M };
-        double Q[6] = { 0, 0, 0, 0, 0, 0 };
+        double Q[6] = { 0, 0, 0, 0, 0, 0 }, T[10] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
         for (int32_t i = b; i < e; ++i) {
             const float* p = t->spm + 4 * (int64_t)i;
             double m = p[3], dx = p[0] - c[0], dy = p[1] - c[1], dz = p[2] - c[2];
             double d2 = dx * dx + dy * dy + dz * dz;
             Q[0] += m * (3 * dx * dx - d2); Q[1] += m * (3 * dy * dy - d2); Q[2] += m * (3 * dz * dz - d2);
             Q[3] += m * 3 * dx * dy; Q[4] += m * 3 * dx * dz; Q[5] += m * 3 * dy * dz;
+            T[0] += m * dx * dx * dx; T[1] += m * dy * dy * dy; T[2] += m * dz * dz * dz;
+            T[3] += m * dx * dx * dy; T[4] += m * dx * dx * dz; T[5] += m * dx * dy * dy;
+            T[6] += m * dy * dy * dz; T[7] += m * dx * dz * dz; T[8] += m * dy * dz * dz; T[9] += m * dx * dy * dz;
         }
         /* integer cell coordinates from the prefix (x highest in every 3-bit digit) */
         int lev = t->level[k];
@@ -205,6 +211,7 @@ p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pm, int key_bits, int nleaf
         for (int a = 0; a < 3; ++a) { t->com[3 * k + a] = c[a]; t->fcom_m[4 * k + a] = (float)c[a]; t->clo[3 * k + a] = clo[a]; t->chi[3 * k + a] = chi[a]; }
         t->fcom_m[4 * k + 3] = (float)M;
         for (int q = 0; q < 6; ++q) { t->quad[6 * k + q] = Q[q]; t->fquad[6 * k + q] = (float)Q[q]; }
+        for (int q = 0; q < 10; ++q) { t->oct[10 * k + q] = T[q]; t->foct[10 * k + q] = (float)T[q]; }
         t->delta[k] = (float)sqrt(dd);
     }
 
@@ -229,7 +236,7 @@ void p3t_o_tree_free(p3t_o_tree* t)
     if (!t) return;
     free(t->keys); free(t->order); free(t->spm); free(t->level); free(t->begin); free(t->end);
     free(t->first_child); free(t->n_child); free(t->prefix); free(t->mass); free(t->com); free(t->quad);
-    free(t->fcom_m); free(t->fquad); free(t->clo); free(t->chi); free(t->delta);
+    free(t->fcom_m); free(t->fquad); free(t->clo); free(t->chi); free(t->delta); free(t->oct); free(t->foct);
     free(t->gbegin); free(t->gend); free(t->glo); free(t->ghi); free(t);
 }
 
@@ -258,6 +265,12 @@ void p3t_o_tree_moments(const p3t_o_tree* t, float* com_m, float* quad, float* c
     memcpy(clo, t->clo, sizeof(float) * 3 * t->nn); memcpy(chi, t->chi, sizeof(float) * 3 * t->nn);
     memcpy(delta, t->delta, sizeof(float) * t->nn);
 }
+void p3t_o_tree_octupoles(const p3t_o_tree* t, float* foct, double* oct)
+{
+    if (foct) memcpy(foct, t->foct, sizeof(float) * 10 * t->nn);
+    if (oct) memcpy(oct, t->oct, sizeof(double) * 10 * t->nn);
+}
+
 void p3t_o_tree_moments64(const p3t_o_tree* t, double* mass, double* com, double* quad)
 {
     memcpy(mass, t->mass, sizeof(double) * t->nn); memcpy(com, t->com, sizeof(double) * 3 * t->nn);

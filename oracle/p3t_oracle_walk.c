@@ -57,6 +57,31 @@ void p3t_o_pc_term(const double xi[3], const float com_m[4], const float q[6], d
     for (int a = 0; a < 3; ++a) out[a] = -M * r[a] / R3 + Qr[a] / R5 - 2.5 * rQr * r[a] / R7;
 }
 
+/* SURVEY 8f NEXT-4, octupole variant: the third-order term of the same Taylor expansion.  With the raw third
+ * moment T_abc = sum m d_a d_b d_c about the COM (order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz), r = x_i - COM:
+ *   1/|r - d| = ... + (5/2) (d.r)^3 / R^7 - (3/2) |d|^2 (d.r) / R^5 + O(d^4)
+ *   t3 = T_abc r_a r_b r_c,  v_a = T_abc r_b r_c,  tau_a = T_bba,  u = tau.r
+ *   phi_3 = -(5/2) t3 / R^7 + (3/2) u / R^5
+ *   a_3   = -grad phi_3 = (15/2) v / R^7 - (35/2) t3 r / R^9 - (3/2) tau / R^5 + (15/2) u r / R^7
+ * fp64 arithmetic on the fp32-rounded node data; ADDED to out. */
+void p3t_o_pc_octupole(const double xi[3], const float com_m[4], const float T[10], double out[4])
+{
+    const double r[3] = { xi[0] - (double)com_m[0], xi[1] - (double)com_m[1], xi[2] - (double)com_m[2] };
+    const double x = r[0], y = r[1], z = r[2];
+    const double xxx = T[0], yyy = T[1], zzz = T[2], xxy = T[3], xxz = T[4], xyy = T[5], yyz = T[6], xzz = T[7], yzz = T[8], xyz = T[9];
+    /* v_a = T_abc r_b r_c */
+    const double v[3] = {
+        xxx * x * x + xyy * y * y + xzz * z * z + 2.0 * (xxy * x * y + xxz * x * z + xyz * y * z),
+        xxy * x * x + yyy * y * y + yzz * z * z + 2.0 * (xyy * x * y + xyz * x * z + yyz * y * z),
+        xxz * x * x + yyz * y * y + zzz * z * z + 2.0 * (xyz * x * y + xzz * x * z + yzz * y * z) };
+    const double tau[3] = { xxx + xyy + xzz, xxy + yyy + yzz, xxz + yyz + zzz };
+    const double t3 = v[0] * x + v[1] * y + v[2] * z;
+    const double u = tau[0] * x + tau[1] * y + tau[2] * z;
+    const double R2 = x * x + y * y + z * z, R = sqrt(R2), R5 = R2 * R2 * R, R7 = R5 * R2, R9 = R7 * R2;
+    out[3] += -2.5 * t3 / R7 + 1.5 * u / R5;
+    for (int a = 0; a < 3; ++a) out[a] += 7.5 * v[a] / R7 - 17.5 * t3 * r[a] / R9 - 1.5 * tau[a] / R5 + 7.5 * u * r[a] / R7;
+}
+
 typedef struct { int32_t* v; int64_t n, cap; } ilist;
 static void il_push(ilist* l, int32_t x)
 {
@@ -94,9 +119,9 @@ void p3t_o_tree_force_buffered(const p3t_o_tree* t, float r_list_f, float r_out_
     p3t_o_tree_force_order(t, 2, r_list_f, r_out_f, r_in_f, theta, pot_mode, ng, group_ids, acc_pot, npp, npc, abs_sum);
 }
 
-/* the monopole-only variant for the accuracy-throughput curve.  order 2 = monopole +
- * quadrupole (north_star), order 1 = the same walk with the quadrupole of every accepted cell left out
- * (R-S8 with Q = 0: phi = -M/R, a = -M r/R^3). */
+/* the variants for the accuracy-throughput curve.  order 2 = monopole + quadrupole
+ * (north_star), order 1 = the same walk with the quadrupole of every accepted cell left out (R-S8 with Q = 0:
+ * phi = -M/R, a = -M r/R^3), order 3 = the same walk with the octupole term of every accepted cell added. */
 void p3t_o_tree_force_order(const p3t_o_tree* t, int order, float r_list_f, float r_out_f, float r_in_f, float theta, int pot_mode,
                             int64_t ng, const int64_t* group_ids, double* acc_pot,
                             int64_t* npp, int64_t* npc, double* abs_sum)
@@ -121,6 +146,7 @@ void p3t_o_tree_force_order(const p3t_o_tree* t, int order, float r_list_f, floa
                 for (int64_t k = 0; k < pc.n; ++k) {
                     double o[4];
                     p3t_o_pc_term(xi, t->fcom_m + 4 * (int64_t)pc.v[k], order >= 2 ? t->fquad + 6 * (int64_t)pc.v[k] : zero_quad, o);
+                    if (order >= 3) p3t_o_pc_octupole(xi, t->fcom_m + 4 * (int64_t)pc.v[k], t->foct + 10 * (int64_t)pc.v[k], o);
                     a[0] += o[0]; a[1] += o[1]; a[2] += o[2]; phi += o[3];
                     asum += sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]);
                 }
