@@ -70,6 +70,8 @@ typedef struct p3t_stats {
     float   ms_irregular;    /* ... of the last p3t_irregular_force kernel (0 if none)  */
     float   ms_core;         /* ... of the last p3t_core_quantities kernels (0 if none)  */
     int64_t launches;        /* kernels this context has launched since p3t_create      */
+    float   ms_octupole;     /* ... of the octupole add kernel of the last force (order 3; else 0) */
+    float   reserved_;
 } p3t_stats;
 
 /* Create a context on CUDA device `device`, enqueuing on `cuda_stream` (a cudaStream_t passed as
@@ -84,7 +86,11 @@ int p3t_set_tree_params(p3t_ctx* ctx, int nleaf, int ncrit);
 
 /* Multipole order of the particle-cell terms: 2 = monopole + quadrupole (default, north_star), 1 = monopole
  * only (a cheaper point on the accuracy-throughput curve: same walk and lists, the
- * quadrupole of the accepted cells left out).  Takes effect at the next p3t_regular_force. */
+ * quadrupole of the accepted cells left out), 3 = + octupole (a more accurate point: the third-order term of
+ * the same Taylor expansion, from the raw third moments sum m d_a d_b d_c about each cell's centre of mass,
+ * added for every accepted cell of the same lists).  Orders 1 and 2 take effect at the next
+ * p3t_regular_force; order 3 needs the third moments, which p3t_build_tree computes when the order is 3:
+ * p3t_regular_force returns P3T_ESTATE until the tree has been built with that order set. */
 int p3t_set_multipole_order(p3t_ctx* ctx, int order);
 
 /* Multi-GPU (PAPER.md:277-291 names it as future work): the path shards by target group
@@ -199,6 +205,9 @@ int p3t_get_nodes(p3t_ctx* ctx, int32_t* level, int32_t* begin, int32_t* end,
 /* fp32 node data: com_m [n_nodes x 4], quad [n_nodes x 6] (xx yy zz xy xz yz, traceless),
  * clo / chi [n_nodes x 3] tight box, delta [n_nodes] = |COM - geometric centre| */
 int p3t_get_moments(p3t_ctx* ctx, float* com_m, float* quad, float* clo, float* chi, float* delta);
+/* octupole variant: fp32 raw third moments about the COM [n_nodes x 10], order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz;
+ * P3T_ESTATE unless the tree was built with multipole order 3 */
+int p3t_get_octupoles(p3t_ctx* ctx, float* oct);
 /* target groups as ranges of sorted positions, each [n_groups], ascending */
 int p3t_get_groups(p3t_ctx* ctx, int32_t* begin, int32_t* end);
 /* per-group list lengths of the last force call: npp[n_groups], npc[n_groups] (int32) */

@@ -25,7 +25,7 @@ SYMBOLS = [
     "p3t_regular_force_ex", "p3t_irregular_force", "p3t_core_quantities", "p3t_neighbours", "p3t_neighbours_copy", "p3t_neighbours_nbody6", "p3t_step_host",
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_pipe_bench", "p3t_strerror", "p3t_last_error", "p3t_params_from_n", "p3t_regularisation_params",
-    "p3t_set_shard", "p3t_get_shard_cuts", "p3t_shard_pack", "p3t_shard_unpack",
+    "p3t_set_shard", "p3t_get_shard_cuts", "p3t_shard_pack", "p3t_shard_unpack", "p3t_get_octupoles",
 ]
 
 
@@ -38,7 +38,7 @@ class Stats(C.Structure):
         ("cube_lo", C.c_float * 3), ("cube_side", C.c_float),
         ("ms_build", C.c_float), ("ms_force", C.c_float), ("ms_walk", C.c_float), ("ms_sort", C.c_float),
         ("ms_eval", C.c_float), ("ms_count", C.c_float), ("ms_irregular", C.c_float), ("ms_core", C.c_float),
-        ("launches", C.c_int64),
+        ("launches", C.c_int64), ("ms_octupole", C.c_float), ("reserved_", C.c_float),
     ]
 
     def as_dict(self) -> dict:
@@ -85,6 +85,7 @@ def lib() -> C.CDLL:
     L.p3t_get_keys.argtypes = [vp, vp, vp]
     L.p3t_get_nodes.argtypes = [vp, vp, vp, vp, vp, vp]
     L.p3t_get_moments.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.p3t_get_octupoles.argtypes = [vp, vp]
     L.p3t_get_groups.argtypes = [vp, vp, vp]
     L.p3t_get_list_lengths.argtypes = [vp, vp, vp]
     L.p3t_set_shard.argtypes = [vp, C.c_int, C.c_int, vp]
@@ -178,7 +179,8 @@ class Context:
         self._check(lib().p3t_build_tree(self._h, self.n, self._dev_f32(pos_mass, 4), key_bits), "p3t_build_tree")
 
     def set_multipole_order(self, order: int):
-        """2 = monopole + quadrupole (default), 1 = monopole only."""
+        """2 = monopole + quadrupole (default), 1 = monopole only, 3 = + octupole (needs a build_tree after the
+        call)."""
         self._check(lib().p3t_set_multipole_order(self._h, order), "p3t_set_multipole_order")
 
     # -- multi-GPU: target groups split among ranks (SURVEY 8e; the exchange is in paper_2110_11658_b200.shard) --
@@ -316,6 +318,13 @@ class Context:
         clo = np.empty((nn, 3), np.float32); chi = np.empty((nn, 3), np.float32); delta = np.empty(nn, np.float32)
         self._check(lib().p3t_get_moments(self._h, *[_np_ptr(x) for x in (com_m, quad, clo, chi, delta)]), "p3t_get_moments")
         return dict(com_m=com_m, quad=quad, clo=clo, chi=chi, delta=delta)
+
+    def octupoles(self):
+        """fp32 raw third moments [n_nodes, 10] (tree built with multipole order 3)."""
+        import numpy as np
+        t = np.empty((self.stats()["n_nodes"], 10), np.float32)
+        self._check(lib().p3t_get_octupoles(self._h, _np_ptr(t)), "p3t_get_octupoles")
+        return t
 
     def groups(self) -> dict:
         import numpy as np

@@ -16,7 +16,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libp3t.so"
-SOURCES = ["p3t_api.cu", "p3t_sort.cu", "p3t_tree.cu", "p3t_walk.cu", "p3t_force.cu", "p3t_irregular.cu", "p3t_core.cu", "p3t_shard.cu", "p3t_pipebench.cu"]
+SOURCES = ["p3t_api.cu", "p3t_sort.cu", "p3t_tree.cu", "p3t_walk.cu", "p3t_force.cu", "p3t_irregular.cu", "p3t_core.cu", "p3t_shard.cu", "p3t_octupole.cu", "p3t_pipebench.cu"]
 HEADERS = [CSRC / "p3t_internal.cuh", CSRC / "p3t_cutoff.cuh", CSRC / "p3t_f32x2.cuh", ROOT / "include" / "p3t.h"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

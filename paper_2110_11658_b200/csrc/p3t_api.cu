@@ -61,6 +61,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evw[k]);
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evi[k]);
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evc[k]);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evo[k]);
     if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
     int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
     if (rc == P3T_OK) rc = p3t_tree_init(c);
@@ -78,12 +79,13 @@ int p3t_destroy(p3t_ctx* c)
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->nbcnt, &c->part, &c->spill, &c->pcpool, &c->pppool, &c->glist,
-                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts };
+                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts, &c->o64, &c->noct, &c->octcnt };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
     for (int k = 0; k < 2; ++k) if (c->evi[k]) cudaEventDestroy(c->evi[k]);
     for (int k = 0; k < 2; ++k) if (c->evc[k]) cudaEventDestroy(c->evc[k]);
+    for (int k = 0; k < 2; ++k) if (c->evo[k]) cudaEventDestroy(c->evo[k]);
     if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
     (void)cudaGetLastError();
     delete c;
@@ -99,7 +101,7 @@ int p3t_set_tree_params(p3t_ctx* c, int nleaf, int ncrit)
 
 int p3t_set_multipole_order(p3t_ctx* c, int order)
 {
-    if (!c || (order != 1 && order != 2)) return P3T_EINVAL;
+    if (!c || order < 1 || order > 3) return P3T_EINVAL;
     c->order = order;
     return P3T_OK;
 }
@@ -127,7 +129,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     if (((uintptr_t)pos_mass & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
     P3T_CUDA(c, cudaSetDevice(c->device));
-    c->state = 0; c->nb_valid = 0; c->irr_done = 0; c->core_done = 0;
+    c->state = 0; c->nb_valid = 0; c->irr_done = 0; c->core_done = 0; c->oct_built = 0;
     c->n = n; c->key_bits = key_bits; c->bits = key_bits / 3;
     // hard bound on the cell count (data layout): leaves <= n, branching cells < n,
     // one-child chain cells <= levels * n / (nleaf + 1)
@@ -156,6 +158,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     P3T_CUDA(c, cudaEventRecord(c->ev[3], c->stream));
     if ((rc = p3t_launch_permute(c, pm)) != P3T_OK) return rc;
     if ((rc = p3t_launch_tree(c)) != P3T_OK) return rc;
+    if (c->order == 3 && (rc = p3t_launch_octupoles(c)) != P3T_OK) return rc;
     P3T_CUDA(c, cudaEventRecord(c->ev[1], c->stream));
     c->state = 1;
     return P3T_OK;
@@ -171,6 +174,10 @@ int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int p
     if (((uintptr_t)acc_pot & 15u) != 0 || ((uintptr_t)vel & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
     if (c->state < 1) return P3T_ESTATE;
+    if (c->order == 3 && !c->oct_built) {
+        snprintf(c->err, sizeof(c->err), "multipole order 3 needs a p3t_build_tree after p3t_set_multipole_order");
+        return P3T_ESTATE;
+    }
     P3T_CUDA(c, cudaSetDevice(c->device));
     c->nb_valid = 0; c->irr_done = 0;
     volatile float rl = r_out + r_buff;                        // one fp32 sum: the list radius of DESIGN.md section 10
@@ -255,6 +262,7 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         (void)cudaEventElapsedTime(&out->ms_walk, c->evw[2], c->evw[3]);
         (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->evw[2]);
         if (c->irr_done) (void)cudaEventElapsedTime(&out->ms_irregular, c->evi[0], c->evi[1]);
+        if (c->order == 3) (void)cudaEventElapsedTime(&out->ms_octupole, c->evo[0], c->evo[1]);
     }
     if (c->core_done) {
         (void)cudaEventElapsedTime(&out->ms_core, c->evc[0], c->evc[1]);

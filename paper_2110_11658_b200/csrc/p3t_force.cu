@@ -615,6 +615,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
         else      k_force<false, false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
+    if (ctx->order == 3 && (rc = p3t_launch_octupole_add(ctx, acc_pot, half_dt, vel))) return rc;   // octupole variant: third-order term of the accepted cells
     k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));

@@ -83,6 +83,9 @@ struct p3t_ctx {
     cudaEvent_t evi[2];              // irregular-force kernel begin/end
     cudaEvent_t evc[2];              // core-quantity kernels begin/end
     p3t_buf core;                    // double[6]: result of k_core_reduce
+    p3t_buf o64, noct, octcnt;       // octupole variant (p3t_octupole.cu): fp64 third moments [node][11], fp32 [node][3] float4, arrival counters
+    int oct_built;                   // the third moments belong to the current tree
+    cudaEvent_t evo[2];              // octupole add kernel begin/end
     int core_done;
     int irr_done;
     p3t_stats last;
@@ -113,6 +116,9 @@ int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
 // p3t_tree.cu : a4-a6
 int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
+// p3t_octupole.cu : SURVEY 8f NEXT-4, octupole variant
+int p3t_launch_octupoles(p3t_ctx* ctx);
+int p3t_launch_octupole_add(p3t_ctx* ctx, float4* acc_pot, float half_dt, float4* vel);
 // p3t_shard.cu : SURVEY 8e, target groups split among the ranks of a node
 int p3t_launch_shard_range(p3t_ctx* ctx);
 // p3t_walk.cu : a7 (interaction lists), a10 (neighbour counts)

@@ -426,7 +426,7 @@ def test_monopole_only_variant(p3t, cfg1):
         b2 = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).cpu().numpy().astype(np.float64)
         assert np.array_equal(a2, b2)
         with pytest.raises(p3t.P3TError):
-            ctx.set_multipole_order(3)
+            ctx.set_multipole_order(4)
 
 
 def test_randomised_shapes_and_tree_parameters(p3t):
