@@ -10,8 +10,8 @@
 //   k_octupoles   third moments of every cell in fp64: leaves from their particles, internal cells by the
 //                 parallel-axis rule, climbing with arrival counters like k_moments (p3t_tree.cu);
 //   k_octupole_add  streams the particle-cell lists that k_walk wrote and adds the term to acc_pot.
-// This is a first, plain version (scalar fp32, one warp per 32 targets, node data read through L1 as warp-wide
-// broadcasts): it is NOT tuned like k_force; DESIGN.md section 10 reports its time beside the default path's.
+// This is a first, plain version (scalar fp32, one warp per 32 targets, the data of 32 cells staged in shared
+// memory): it is NOT tuned like k_force; DESIGN.md section 10 reports its time beside the default path's.
 #include "p3t_internal.cuh"
 #include <stdlib.h>
 
@@ -123,6 +123,7 @@ struct octadd_args {
 
 __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
 {
+    __shared__ float4 s_node[OCT_THREADS / 32][4][32];
     const int lane = threadIdx.x & 31;
     const int g0 = A.info->shard_g0, ng = A.info->shard_g1 - g0;
     const int nwarps = gridDim.x * (OCT_THREADS / 32);
@@ -137,14 +138,21 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
         const int32_t* list = A.pcpool + ((long long)gl.x << 5);
         const int npc = (int)gl.y;
         double ax = 0.0, ay = 0.0, az = 0.0, ph = 0.0;
+        float4 (*S)[32] = s_node[threadIdx.x >> 5];
         for (int e0 = 0; e0 < npc; e0 += 32) {
             const int m = min(32, npc - e0);
-            const int id = lane < m ? list[e0 + lane] : 0;
+            // the data of 32 cells go to shared memory, one cell per lane; the loop below reads them as broadcasts
+            __syncwarp();
+            if (lane < m) {
+                const int node = list[e0 + lane];
+                S[0][lane] = A.ncom[node];
+                S[1][lane] = A.noct[(size_t)node * 3]; S[2][lane] = A.noct[(size_t)node * 3 + 1]; S[3][lane] = A.noct[(size_t)node * 3 + 2];
+            }
+            __syncwarp();
             float fx = 0.0f, fy = 0.0f, fz = 0.0f, fp = 0.0f;        // fp32 over <= 32 entries, folded into fp64 (R-S9)
+#pragma unroll 2
             for (int q = 0; q < m; ++q) {
-                const int node = __shfl_sync(0xffffffffu, id, q);
-                const float4 cm = A.ncom[node];
-                const float4 t0 = A.noct[(size_t)node * 3], t1 = A.noct[(size_t)node * 3 + 1], t2 = A.noct[(size_t)node * 3 + 2];
+                const float4 cm = S[0][q], t0 = S[1][q], t1 = S[2][q], t2 = S[3][q];
                 const float xxx = t0.x, yyy = t0.y, zzz = t0.z, xxy = t0.w, xxz = t1.x, xyy = t1.y, yyz = t1.z, xzz = t1.w, yzz = t2.x, xyz = t2.y;
                 const float x = xi.x - cm.x, y = xi.y - cm.y, z = xi.z - cm.z;
                 const float R2 = fmaf(z, z, fmaf(y, y, x * x));
