@@ -6,6 +6,8 @@
 //     t3 = T_abc r_a r_b r_c,  v_a = T_abc r_b r_c,  tau_a = T_bba,  u = tau.r
 //     phi_3 = -(5/2) t3 / R^7 + (3/2) u / R^5
 //     a_3   = (15/2) v / R^7 - (35/2) t3 r / R^9 - (3/2) tau / R^5 + (15/2) u r / R^7
+// evaluated through the traceless form O = 5 T - sym(delta tau): phi_3 = -(1/2) O:rrr / R^7,
+//     a_3 = (3/2) O:rr / R^7 - (7/2) (O:rrr) r / R^9   (identical, a third fewer operations).
 // Two kernels, both outside the default path (which they leave untouched):
 //   k_octupoles   third moments of every cell in fp64: leaves from their particles, internal cells by the
 //                 parallel-axis rule, climbing with arrival counters like k_moments (p3t_tree.cu);
@@ -21,7 +23,7 @@ struct oct_args {
     const float4* spm; const int32_t *nbegin, *nend, *nfirst, *nnchild, *nparent;
     const double* m64;          // [node][13] from k_moments: M, sum m x (3), Q (6), COM (3)
     double* o64;                // [node][11]: tr S, T (10: xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz)
-    float4* noct;               // [node][3]: the ten components rounded once to fp32 (+ 2 x padding)
+    float4* noct;               // [node][3]: the ten components of the traceless form, rounded once to fp32 (+ 2 x padding)
     int32_t* cnt;               // arrival counters, zeroed by the host side
     p3t_devinfo* info;
 };
@@ -32,9 +34,13 @@ __device__ __forceinline__ void oct_store(const oct_args& A, int k, double tr, c
     o[0] = tr;
 #pragma unroll
     for (int q = 0; q < 10; ++q) o[1 + q] = T[q];
-    A.noct[(size_t)k * 3 + 0] = make_float4((float)T[0], (float)T[1], (float)T[2], (float)T[3]);
-    A.noct[(size_t)k * 3 + 1] = make_float4((float)T[4], (float)T[5], (float)T[6], (float)T[7]);
-    A.noct[(size_t)k * 3 + 2] = make_float4((float)T[8], (float)T[9], 0.0f, 0.0f);
+    // the force kernel reads the traceless form O_abc = 5 T_abc - (delta_ab tau_c + delta_ac tau_b + delta_bc tau_a),
+    // tau_a = T_bba, with which phi_3 = -(1/2) O:rrr / R^7 and a_3 = (3/2) O:rr / R^7 - (7/2) (O:rrr) r / R^9
+    // (O:rrr = 5 t3 - 3 R^2 u: the same term with a third fewer operations); made in fp64, rounded once
+    const double tx = T[0] + T[5] + T[7], ty = T[3] + T[1] + T[8], tz = T[4] + T[6] + T[2];
+    A.noct[(size_t)k * 3 + 0] = make_float4((float)(5.0 * T[0] - 3.0 * tx), (float)(5.0 * T[1] - 3.0 * ty), (float)(5.0 * T[2] - 3.0 * tz), (float)(5.0 * T[3] - ty));
+    A.noct[(size_t)k * 3 + 1] = make_float4((float)(5.0 * T[4] - tz), (float)(5.0 * T[5] - tx), (float)(5.0 * T[6] - tz), (float)(5.0 * T[7] - tx));
+    A.noct[(size_t)k * 3 + 2] = make_float4((float)(5.0 * T[8] - ty), (float)(5.0 * T[9]), 0.0f, 0.0f);
 }
 
 __global__ void __launch_bounds__(OCT_THREADS) k_octupoles(oct_args A)
@@ -156,19 +162,18 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
                 const float xxx = t0.x, yyy = t0.y, zzz = t0.z, xxy = t0.w, xxz = t1.x, xyy = t1.y, yyz = t1.z, xzz = t1.w, yzz = t2.x, xyz = t2.y;
                 const float x = xi.x - cm.x, y = xi.y - cm.y, z = xi.z - cm.z;
                 const float R2 = fmaf(z, z, fmaf(y, y, x * x));
-                const float ri = rsqrtf(R2), ri2 = ri * ri, ri5 = ri2 * ri2 * ri, ri7 = ri5 * ri2, ri9 = ri7 * ri2;
-                const float xx = x * x, yy = y * y, zz = z * z, xy = 2.0f * x * y, xz = 2.0f * x * z, yz = 2.0f * y * z;
-                const float vx = fmaf(xxx, xx, fmaf(xyy, yy, fmaf(xzz, zz, fmaf(xxy, xy, fmaf(xxz, xz, xyz * yz)))));
-                const float vy = fmaf(xxy, xx, fmaf(yyy, yy, fmaf(yzz, zz, fmaf(xyy, xy, fmaf(xyz, xz, yyz * yz)))));
-                const float vz = fmaf(xxz, xx, fmaf(yyz, yy, fmaf(zzz, zz, fmaf(xyz, xy, fmaf(xzz, xz, yzz * yz)))));
-                const float tx = xxx + xyy + xzz, ty = xxy + yyy + yzz, tz = xxz + yyz + zzz;
-                const float t3 = fmaf(vz, z, fmaf(vy, y, vx * x));
-                const float u = fmaf(tz, z, fmaf(ty, y, tx * x));
-                fp += fmaf(-2.5f * t3, ri7, 1.5f * u * ri5);
-                const float cr = fmaf(7.5f * u, ri7, -17.5f * t3 * ri9), c7 = 7.5f * ri7, c5 = -1.5f * ri5;
-                fx += fmaf(cr, x, fmaf(c7, vx, c5 * tx));
-                fy += fmaf(cr, y, fmaf(c7, vy, c5 * ty));
-                fz += fmaf(cr, z, fmaf(c7, vz, c5 * tz));
+                const float ri = rsqrtf(R2), ri2 = ri * ri, ri7 = ri2 * ri2 * ri2 * ri, ri9 = ri7 * ri2;
+                const float x2 = x + x, y2 = y + y;
+                const float xx = x * x, yy = y * y, zz = z * z, xy = x2 * y, xz = x2 * z, yz = y2 * z;
+                const float wx = fmaf(xxx, xx, fmaf(xyy, yy, fmaf(xzz, zz, fmaf(xxy, xy, fmaf(xxz, xz, xyz * yz)))));
+                const float wy = fmaf(xxy, xx, fmaf(yyy, yy, fmaf(yzz, zz, fmaf(xyy, xy, fmaf(xyz, xz, yyz * yz)))));
+                const float wz = fmaf(xxz, xx, fmaf(yyz, yy, fmaf(zzz, zz, fmaf(xyz, xy, fmaf(xzz, xz, yzz * yz)))));
+                const float o3 = fmaf(wz, z, fmaf(wy, y, wx * x));
+                fp = fmaf(-0.5f * o3, ri7, fp);
+                const float c1 = 1.5f * ri7, c2 = -3.5f * o3 * ri9;
+                fx += fmaf(c2, x, c1 * wx);
+                fy += fmaf(c2, y, c1 * wy);
+                fz += fmaf(c2, z, c1 * wz);
             }
             ax += (double)fx; ay += (double)fy; az += (double)fz; ph += (double)fp;
         }
@@ -213,13 +218,13 @@ extern "C" int p3t_get_octupoles(p3t_ctx* c, float* oct)
     P3T_CUDA(c, cudaMemcpyAsync(&h, c->info.p, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     P3T_CUDA(c, cudaStreamSynchronize(c->stream));
     const size_t nn = (size_t)h.n_nodes;
-    float* t = (float*)malloc(nn * 48 + 16);
+    double* t = (double*)malloc(nn * 88 + 16);
     if (!t) return P3T_ENOMEM;
-    cudaError_t e = cudaMemcpyAsync(t, c->noct.p, nn * 48, cudaMemcpyDeviceToHost, c->stream);
+    cudaError_t e = cudaMemcpyAsync(t, c->o64.p, nn * 88, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { free(t); return p3t_fail_cuda(c, e, "p3t_get_octupoles copy", __LINE__); }
     for (size_t k = 0; k < nn; ++k)
-        for (int q = 0; q < 10; ++q) oct[10 * k + q] = t[12 * k + q];
+        for (int q = 0; q < 10; ++q) oct[10 * k + q] = (float)t[11 * k + 1 + q];
     free(t);
     return P3T_OK;
 }
