@@ -361,8 +361,12 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
         else if (total > 0) P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
     }
     p3t_devinfo h;
-    if ((rc = sync_and_check(c, &h)) != P3T_OK) return rc;
-    if (nb_offsets_host) P3T_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    rc = sync_and_check(c, &h);
+    if (nb_offsets_host && c->copy_stream) {                 // on every path: the caller's buffer must be quiet on return
+        cudaError_t e = cudaStreamSynchronize(c->copy_stream);
+        if (e != cudaSuccess && rc == P3T_OK) return p3t_fail_cuda(c, e, "copy stream", __LINE__);
+    }
+    if (rc != P3T_OK) return rc;
     return over ? P3T_ERANGE : P3T_OK;
 }
 

@@ -530,11 +530,11 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
                      float r_list, float half_dt, float4* vel)
 {
     const int n = (int)ctx->n;
-    static int per_sm = 0;
-    if (!per_sm) {
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false, false>, FORCE_THREADS, 0));
-        if (per_sm < 1) per_sm = 1;
+    if (!ctx->occ_force) {
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ_force, k_force<false, false>, FORCE_THREADS, 0));
+        if (ctx->occ_force < 1) ctx->occ_force = 1;
     }
+    const int per_sm = ctx->occ_force;
     int rc;
     const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
     if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;

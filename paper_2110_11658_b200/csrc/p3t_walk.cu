@@ -285,7 +285,7 @@ __global__ void k_walk_reset(p3t_devinfo* info, int mode)
 
 static int walk_blocks(p3t_ctx* ctx, int mode, int* out, bool limit_by_n = true)
 {
-    static int per_sm[2] = { 0, 0 };
+    int* per_sm = ctx->occ_walk;                             // per context: contexts may sit on different devices
     if (!per_sm[mode]) {
         if (mode == WALK_COUNT) P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], k_walk<WALK_COUNT>, WALK_THREADS, 0));
         else                    P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], k_walk<WALK_LISTS>, WALK_THREADS, 0));
