@@ -79,7 +79,7 @@ int p3t_destroy(p3t_ctx* c)
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->nbcnt, &c->part, &c->spill, &c->pcpool, &c->pppool, &c->glist,
-                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts, &c->o64, &c->noct, &c->octcnt };
+                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts, &c->o64, &c->noct, &c->octcnt, &c->psitab, &c->irrpv };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);

@@ -84,6 +84,9 @@ struct p3t_ctx {
     cudaEvent_t evi[2];              // irregular-force kernel begin/end
     cudaEvent_t evc[2];              // core-quantity kernels begin/end
     p3t_buf core;                    // double[6]: result of k_core_reduce
+    p3t_buf irrpv;                   // k_irregular<PV>: float4[n][2] position + velocity records, original order
+    p3t_buf psitab;                  // k_irregular: Hermite table of the pair-potential integral (p3t_irregular.cu)
+    float psitab_host[256 * 8]; float psitab_rout, psitab_rin;
     p3t_buf o64, noct, octcnt;       // octupole variant (p3t_octupole.cu): fp64 third moments [node][11], fp32 [node][3] float4, arrival counters
     int oct_built;                   // the third moments belong to the current tree
     cudaEvent_t evo[2];              // octupole add kernel begin/end

@@ -164,3 +164,22 @@ def test_buffered_lists_and_kick(p3t):
         assert torch.equal(b0, b1)
         with pytest.raises(p3t.P3TError):
             ctx.regular_force(w.r_out, w.r_in, w.theta, 0, r_buff=-1.0, vel=v_dev)
+
+
+@pytest.mark.parametrize("n,ncore,expect_pv", [(4000, 400, True), (60000, 300, False)])
+def test_row_length_classes_and_both_gather_paths(p3t, n, ncore, expect_pv):
+    """A tight clump inside r_out (rows of ncore - 1 entries: the all-lanes branch) in a Plummer halo whose rows are
+    short (thread per row) or medium (eight lanes per row), with the lists at >= 4 entries per particle (packed
+    position + velocity records) and below (rank indirection): every branch of k_irregular against the oracle."""
+    w = workloads.make_config(1, n_override=n)
+    rng = np.random.default_rng(n)
+    pm = w.pos_mass.copy()
+    d = rng.normal(size=(ncore, 3)); d *= (0.3 * w.r_out) * rng.random((ncore, 1)) ** (1 / 3) / np.linalg.norm(d, axis=1, keepdims=True)
+    pm[:ncore, :3] = (np.array([0.2, -0.1, 0.05]) + d).astype(np.float32)
+    w.pos_mass = pm
+    # a second, looser clump gives rows of 33 .. 256 entries
+    d2 = rng.normal(size=(120, 3)); d2 *= (0.45 * w.r_out) / np.linalg.norm(d2, axis=1, keepdims=True) * rng.random((120, 1)) ** (1 / 3)
+    pm[ncore:ncore + 120, :3] = (np.array([-0.3, 0.2, 0.1]) + d2).astype(np.float32)
+    reg, acc, jerk, o, st = _check(p3t, w)
+    assert st["nb_max"] > 256
+    assert (st["nb_total"] >= 4 * n) == expect_pv
