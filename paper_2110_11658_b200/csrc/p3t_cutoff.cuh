@@ -13,7 +13,7 @@ struct walk_consts {
     float sc[6];                           // S(t) = t (sc0 + t (sc1 + ... t sc5))
     float rem;                             // c^3 (1+c)^3  (> 0)
     float c;                               // r_in / (r_out - r_in)
-    double dk140, ds1, dsc[6], drem, dc;   // the same in fp64 (cutoff_psi64)
+    double dk140, ds1, dsc[6], drem, dc;   // the same in fp64 (the table of p3t_irregular.cu)
     double dlog1c;                         // log(1 + c)
     float theta;
     int   pot_mode;
@@ -40,14 +40,7 @@ __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float
 // The closed form cancels: terms of order 1 give an integral of order 1e-2 .. 0 that is then multiplied
 // by 140 / D ~ 3000, so in fp32 a pair's psi carries ~1e-5 of its Newtonian potential.  That is
 // invisible in phi_R (dominated by the far field) but not in phi_I, which is made of near pairs only:
-// the irregular path evaluates it in fp64.
-__device__ __forceinline__ float cutoff_psi64(const walk_consts& K, float xf, float W, float rinv)
-{
-    const double x = (double)xf;
-    const double sx = x * (K.dsc[0] + x * (K.dsc[1] + x * (K.dsc[2] + x * (K.dsc[3] + x * (K.dsc[4] + x * K.dsc[5])))));
-    const double integral = (K.ds1 - sx) - K.drem * (K.dlog1c - log(x + K.dc));
-    return (float)(-(double)W * (double)rinv - K.dk140 * integral);
-}
+// the irregular path interpolates the integral from a table made in fp64 (p3t_irregular.cu).
 
 static inline void make_consts(walk_consts& K, float r_out, float r_in, float theta, int pot_mode, float r_list = -1.0f)
 {
