@@ -214,6 +214,24 @@ def run_ours(args, w, rank, world, local_rank, dist):
         irr_ms.append(ctx.stats()["ms_irregular"])
     irr_ms = float(np.median(irr_ms[1:]))
 
+    # ---- SURVEY 8f NEXT-2 (outside the step): lists out to r_out + r_buff (eq. 20-21: r_buff = 3 tau sigma, r_cut = 4 tau,
+    # sigma = 1/sqrt(2) => r_buff = 0.53 r_out) and the leapfrog half-kick fused into the force epilogue ----
+    r_buff = float(np.float32(0.75 * 2.0 ** -0.5 * w.r_out))
+    kick_dev = vel_dev.clone()
+    buf_ms = []
+    for k in range(4):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.build_tree(pm_dev, 63)
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0, out=out_dev, r_buff=r_buff, half_dt=1.0e-4, vel=kick_dev)
+        e1.record()
+        stb = ctx.stats()
+        buf_ms.append(e0.elapsed_time(e1))
+    buf_ms = float(np.median(buf_ms[1:]))
+    ctx.build_tree(pm_dev, 63)                            # back to the plain lists for the legs below
+    ctx.regular_force(w.r_out, w.r_in, w.theta, 0, out=out_dev)
+
     # ---- SURVEY 8f NEXT-3 (outside the step): sampled 6-NN core quantities, the paper's sample size ----
     ns = int(min(n, np.sqrt(5000.0 * n)))
     sample_dev = torch.from_numpy(workloads.sample_targets(n, ns).astype(np.int32)).to(dev)
@@ -297,6 +315,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
                 "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n + 8 * (n + 1) + 4 * int(nb_total)},
         "next1_irregular": {"ms": irr_ms, "list_entries_per_s": st["nb_total"] / (irr_ms * 1e-3) if irr_ms > 0 else None,
                             "note": "p3t_irregular_force (F_I, jerk, phi_I over the neighbour lists); not part of the timed step"},
+        "next2_buffered_kick": {"ms_per_step": buf_ms, "r_buff": r_buff, "neighbours_total": stb["nb_total"], "neighbours_max": stb["nb_max"],
+                                "note": "p3t_regular_force_ex: lists out to r_out + r_buff (eq. 20-21) and the half-kick in the force epilogue; not part of the timed step"},
         "next3_core": {"ms": core_ms, "sample": ns, "k": 6, "r_core": core["r_core"], "rho_core": core["rho_core"], "n_core": core["n_core"],
                        "note": "p3t_core_quantities (k-NN on the octree + Casertano-Hut reductions); not part of the timed step"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "roofline_build": roofline_build,

@@ -497,12 +497,18 @@ __global__ void __launch_bounds__(256) k_nb_offsets(const int32_t* __restrict__ 
     for (int k = 0; k < 16; ++k) { int i = base + k; if (i < n) off[i] = run; run += v[k]; }
 }
 
-// rows ascending in original id: rank sort (ids inside a row are distinct), out of place.
-// Each lane sorts its own short row; rows longer than 16 are done by the whole warp.
-__global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
-                                                     int32_t* __restrict__ idx, int n)
+// Rows ascending in original id, out of place (ids inside a row are distinct).  Each lane rank-sorts its own short
+// row (<= 16 entries); rows of 17 .. 32 are rank-sorted by the warp; longer rows (a King core has hundreds of
+// entries per row, and the rank sort is quadratic) go through a bitonic network in the warp's shared memory, up
+// to SORT_SMEM entries; beyond that the quadratic sort again (not met by the paper's workloads).
+#define SORTROWS_THREADS 128
+#define SORT_SMEM 2048
+__global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
+                                                                  int32_t* __restrict__ idx, int n)
 {
+    __shared__ int32_t s_row[SORTROWS_THREADS / 32][SORT_SMEM];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    int32_t* s = s_row[threadIdx.x >> 5];
     long long b = 0; int len = 0;
     if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
     if (len <= 16) {
@@ -517,11 +523,30 @@ __global__ void __launch_bounds__(256) k_nb_sortrows(const long long* __restrict
         const int src = __ffs(m) - 1; m &= m - 1;
         const long long rb = __shfl_sync(0xffffffffu, b, src);
         const int rl = __shfl_sync(0xffffffffu, len, src);
-        for (int a = lane; a < rl; a += 32) {
-            const int v = raw[rb + a]; int r = 0;
-            for (int c = 0; c < rl; ++c) r += raw[rb + c] < v;
-            idx[rb + r] = v;
+        if (rl <= 32 || rl > SORT_SMEM) {
+            for (int a = lane; a < rl; a += 32) {
+                const int v = raw[rb + a]; int r = 0;
+                for (int c = 0; c < rl; ++c) r += raw[rb + c] < v;
+                idx[rb + r] = v;
+            }
+            continue;
         }
+        int P = 64;
+        while (P < rl) P <<= 1;
+        for (int a = lane; a < P; a += 32) s[a] = a < rl ? raw[rb + a] : 0x7fffffff;
+        __syncwarp();
+        for (int k = 2; k <= P; k <<= 1)
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                for (int t = lane; t < (P >> 1); t += 32) {
+                    const int lo = 2 * t - (t & (j - 1)), hi = lo + j;        // the t-th pair of this stage
+                    const int x = s[lo], y = s[hi];
+                    const bool up = (lo & k) == 0;
+                    if ((x > y) == up) { s[lo] = y; s[hi] = x; }
+                }
+                __syncwarp();
+            }
+        for (int a = lane; a < rl; a += 32) idx[rb + a] = s[a];
+        __syncwarp();
     }
 }
 
@@ -616,7 +641,7 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
     if (ctx->order == 3 && (rc = p3t_launch_octupole_add(ctx, acc_pot, half_dt, vel))) return rc;   // octupole variant: third-order term of the accepted cells
-    k_nb_sortrows<<<(n + 255) / 256, 256, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    k_nb_sortrows<<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
     ctx->launches += 2;

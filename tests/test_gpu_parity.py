@@ -479,3 +479,23 @@ def test_randomised_shapes_and_tree_parameters(p3t):
                 g = ctx.core_quantities(torch.from_numpy(s).cuda(), 6)
                 o = oracle.knn_density(pm, s, 6)
                 assert np.array_equal(g["nbr"].cpu().numpy(), o["nbr"]) and np.array_equal(g["d2k"].cpu().numpy(), o["d2k"]), tag
+
+
+def test_neighbour_rows_of_every_sort_class(p3t):
+    """k_nb_sortrows: rows of <= 16 (per lane), 17 .. 32 (warp rank sort), 33 .. 2048 (bitonic network in shared
+    memory) and > 2048 entries (quadratic fallback), all bit-exact against the brute-force CSR."""
+    w = workloads.make_config(1, n_override=8000)
+    rng = np.random.default_rng(8)
+    pm = w.pos_mass.copy()
+    used = 0
+    for k, rad in ((2300, 0.45), (700, 0.4), (90, 0.3), (25, 0.2)):
+        d = rng.normal(size=(k, 3)); d *= (rad * w.r_out) * rng.random((k, 1)) ** (1 / 3) / np.linalg.norm(d, axis=1, keepdims=True)
+        pm[used:used + k, :3] = (rng.normal(size=3) * 0.4 + d).astype(np.float32)
+        used += k
+    w.pos_mass = pm
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0)
+        off, idx = check_neighbours(ctx, w)
+        lens = np.diff(off)
+        assert lens.max() > 2048 and np.any((lens > 32) & (lens <= 2048)) and np.any((lens > 16) & (lens <= 32)) and np.any(lens <= 16)
