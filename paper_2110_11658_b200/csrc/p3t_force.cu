@@ -503,12 +503,14 @@ __global__ void __launch_bounds__(256) k_nb_offsets(const int32_t* __restrict__ 
 // to SORT_SMEM entries; beyond that the quadratic sort again (not met by the paper's workloads).
 #define SORTROWS_THREADS 128
 #define SORT_SMEM 2048
+// LONG = false: no row is longer than 32 (the host knows the longest row): no shared memory, full occupancy.
+template <bool LONG>
 __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
                                                                   int32_t* __restrict__ idx, int n)
 {
-    __shared__ int32_t s_row[SORTROWS_THREADS / 32][SORT_SMEM];
+    __shared__ int32_t s_row[LONG ? SORTROWS_THREADS / 32 : 1][LONG ? SORT_SMEM : 1];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
-    int32_t* s = s_row[threadIdx.x >> 5];
+    int32_t* s = s_row[LONG ? threadIdx.x >> 5 : 0];
     long long b = 0; int len = 0;
     if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
     if (len <= 16) {
@@ -523,7 +525,7 @@ __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long lon
         const int src = __ffs(m) - 1; m &= m - 1;
         const long long rb = __shfl_sync(0xffffffffu, b, src);
         const int rl = __shfl_sync(0xffffffffu, len, src);
-        if (rl <= 32 || rl > SORT_SMEM) {
+        if (!LONG || rl <= 32 || rl > SORT_SMEM) {
             for (int a = lane; a < rl; a += 32) {
                 const int v = raw[rb + a]; int r = 0;
                 for (int c = 0; c < rl; ++c) r += raw[rb + c] < v;
@@ -641,7 +643,8 @@ int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
     if (ctx->order == 3 && (rc = p3t_launch_octupole_add(ctx, acc_pot, half_dt, vel))) return rc;   // octupole variant: third-order term of the accepted cells
-    k_nb_sortrows<<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    if (h.nb_max > 32) k_nb_sortrows<true><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    else               k_nb_sortrows<false><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
     ctx->launches += 2;
