@@ -16,7 +16,7 @@ from pathlib import Path
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-_SOURCES = ["p3t_oracle_direct.c", "p3t_oracle_tree.c", "p3t_oracle_walk.c"]
+_SOURCES = ["p3t_oracle_direct.c", "p3t_oracle_grid.c", "p3t_oracle_tree.c", "p3t_oracle_walk.c"]
 _HEADERS = ["p3t_oracle.h", "p3t_oracle_tree_priv.h"]
 _LIB = _HERE / "libp3t_oracle.so"
 NLEAF_DEFAULT = 16
@@ -53,12 +53,16 @@ def lib() -> C.CDLL:
         _lib.p3t_o_direct.argtypes = [i64, vp, d, d, i64, vp, vp, vp, vp, vp]
         _lib.p3t_o_irregular.restype = i64
         _lib.p3t_o_irregular.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp, vp]
+        _lib.p3t_o_irregular_cand.restype = i64
+        _lib.p3t_o_irregular_cand.argtypes = [i64, vp, vp, d, d, i64, vp, vp, vp, vp, vp, vp, vp, vp]
         _lib.p3t_o_knn_density.restype = None
         _lib.p3t_o_knn_density.argtypes = [i64, vp, i64, vp, C.c_int, vp, vp, vp]
         _lib.p3t_o_core_quantities.restype = None
         _lib.p3t_o_core_quantities.argtypes = [i64, vp, i64, vp, vp, vp]
         _lib.p3t_o_neighbours.restype = i64
         _lib.p3t_o_neighbours.argtypes = [i64, vp, f32, C.c_int, i64, vp, vp, vp]
+        _lib.p3t_o_neighbours_grid.restype = i64
+        _lib.p3t_o_neighbours_grid.argtypes = [i64, vp, f32, i64, vp, vp, vp]
         _lib.p3t_o_tree_build.restype = vp
         _lib.p3t_o_tree_build.argtypes = [i64, vp, C.c_int, C.c_int, C.c_int]
         _lib.p3t_o_tree_free.restype = None; _lib.p3t_o_tree_free.argtypes = [vp]
@@ -131,13 +135,20 @@ def direct(pos_mass, r_out: float, r_in: float, targets=None):
     return dict(acc_reg=ar, phi_reg=pr, acc_irr=ai, phi_newt=pn, coincident=int(co))
 
 
-def irregular(pos_mass, vel, r_out: float, r_in: float, targets=None):
-    """Irregular acceleration, jerk, potential over the neighbour sphere (eq. 1, 2, 5, 7); fp64 arrays."""
+def irregular(pos_mass, vel, r_out: float, r_in: float, targets=None, candidates=None):
+    """Irregular acceleration, jerk, potential over the neighbour sphere (eq. 1, 2, 5, 7); fp64 arrays.
+    candidates = (offsets, indices): CSR rows over the targets that contain every target's neighbour sphere
+    (e.g. neighbours_grid at a slightly larger radius); None = every j is tested."""
     pm = _pm(pos_mass); v = _pm(vel)
     t = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
     nt = pm.shape[0] if t is None else t.shape[0]
     acc = np.zeros((nt, 3)); jerk = np.zeros((nt, 3)); phi = np.zeros(nt); ab = np.zeros(nt); an = np.zeros(nt)
-    coinc = lib().p3t_o_irregular(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(acc), _p(jerk), _p(phi), _p(ab), _p(an))
+    co = ci = None
+    if candidates is not None:
+        co = np.ascontiguousarray(candidates[0], dtype=np.int64); ci = np.ascontiguousarray(candidates[1], dtype=np.int32)
+        assert co.shape[0] == nt + 1
+    coinc = lib().p3t_o_irregular_cand(pm.shape[0], _p(pm), _p(v), float(r_out), float(r_in), nt, _p(t), _p(co), _p(ci),
+                                       _p(acc), _p(jerk), _p(phi), _p(ab), _p(an))
     return dict(acc_irr=acc, jerk_irr=jerk, phi_irr=phi, abs_jerk=ab, abs_newt=an, coincident=int(coinc))
 
 
@@ -169,6 +180,24 @@ def neighbours(pos_mass, r_out: float, targets=None, fp32_predicate: bool = True
     total = lib().p3t_o_neighbours(n, _p(pm), float(np.float32(r_out)), int(fp32_predicate), nt, _p(tg), _p(counts), None)
     idx = np.zeros(max(int(total), 1), dtype=np.int32)
     lib().p3t_o_neighbours(n, _p(pm), float(np.float32(r_out)), int(fp32_predicate), nt, _p(tg), _p(counts), _p(idx))
+    off = np.zeros(nt + 1, dtype=np.int64)
+    np.cumsum(counts, out=off[1:])
+    return off, idx[: int(total)]
+
+
+def neighbours_grid(pos_mass, r_out: float, targets=None):
+    """The rows of `neighbours` (fp32 predicate) with candidates from a uniform cell grid (large N):
+    (offsets int64 [nt+1], indices int32)."""
+    pm = _pm(pos_mass)
+    n = pm.shape[0]
+    tg = None if targets is None else np.ascontiguousarray(targets, dtype=np.int64)
+    nt = n if tg is None else tg.shape[0]
+    counts = np.zeros(nt, dtype=np.int64)
+    total = lib().p3t_o_neighbours_grid(n, _p(pm), float(np.float32(r_out)), nt, _p(tg), _p(counts), None)
+    if total < 0:
+        raise ValueError("p3t_o_neighbours_grid: invalid arguments or out of memory")
+    idx = np.zeros(max(int(total), 1), dtype=np.int32)
+    lib().p3t_o_neighbours_grid(n, _p(pm), float(np.float32(r_out)), nt, _p(tg), _p(counts), _p(idx))
     off = np.zeros(nt + 1, dtype=np.int64)
     np.cumsum(counts, out=off[1:])
     return off, idx[: int(total)]

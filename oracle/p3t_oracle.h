@@ -8,6 +8,7 @@
  *
  * Part I   (p3t_oracle_direct.c)  plain definitions: cutoff K/W (eq. 6), pair potential psi,
  *          direct O(N^2) split sums (eq. 1, 3, 4), brute-force neighbour lists.
+ *          (p3t_oracle_grid.c)    the same neighbour lists with a uniform cell grid for large N.
  * Part II  (p3t_oracle_tree.c)    a reference octree, step by step: cube, Morton keys, order,
  *          canonical topology, moments, sibling-run groups, opening rule, evaluation.
  *          The paper names only the library (Bonsai) and theta; every
@@ -44,6 +45,12 @@ int64_t p3t_o_irregular(int64_t n, const float* pos_mass, const float* vel, doub
                         int64_t nt, const int64_t* targets,
                         double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt);
 
+/* the same sums with the candidates j of every target restricted to caller-given CSR rows that contain its
+ * neighbour sphere (cand_off[nt + 1], cand_idx; NULL = every j): same predicate, same arithmetic per pair */
+int64_t p3t_o_irregular_cand(int64_t n, const float* pos_mass, const float* vel, double r_out, double r_in,
+                             int64_t nt, const int64_t* targets, const int64_t* cand_off, const int32_t* cand_idx,
+                             double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt);
+
 /* sampled K-nearest-neighbour densities (Casertano & Hut 1985) and the core
  * quantities built from them.  sample: ns original ids.  nbr[ns*K] (may be NULL),
  * d2k[ns] fp32, rho[ns] fp64.  out[6] = density centre (3), R_core, rho_core, N_core. */
@@ -56,6 +63,12 @@ void p3t_o_core_quantities(int64_t n, const float* pos_mass, int64_t ns, const i
  * if indices != NULL rows are written back to back (ascending j) and must hold sum(counts). */
 int64_t p3t_o_neighbours(int64_t n, const float* pos_mass, float r_out, int fp32_predicate,
                          int64_t nt, const int64_t* targets, int64_t* counts, int32_t* indices);
+
+/* The same lists (fp32 predicate of R10) with the candidates restricted by a uniform cell grid of edge
+ * >= 1.001 r_out, independent of the octree (p3t_oracle_grid.c): for the sizes at which the
+ * double loop above takes hours.  Same outputs; returns the total or -1 (allocation failure, r_out <= 0). */
+int64_t p3t_o_neighbours_grid(int64_t n, const float* pos_mass, float r_out,
+                              int64_t nt, const int64_t* targets, int64_t* counts, int32_t* indices);
 
 /* ---- Part II ---- */
 typedef struct p3t_o_tree p3t_o_tree;

@@ -174,49 +174,72 @@ int64_t p3t_o_neighbours(int64_t n, const float* pm, float r_out, int fp32_predi
  * vel: n x 4 fp32 (vx, vy, vz, unused).  Outputs (any may be NULL): acc_irr[3 nt], jerk_irr[3 nt],
  * phi_irr[nt] = sum m_j (-1/r - psi(r)); conditioning of the sums: abs_jerk[nt] = sum of |jerk term|,
  * abs_newt[nt] = sum m_j (|v|/r^3 + 3 |d.v|/r^4), the size of the unweighted (K = 1) jerk terms. */
+/* one pair of the sums above, added to the accumulators of target i; returns 1 if the pair is coincident */
+typedef struct { double a[3], jk[3], phi, ab, an; } irr_acc;
+static int irr_pair(const float* pm, const float* vel, double r_out, double r_in, int64_t i, int64_t j, irr_acc* S)
+{
+    const double D = r_out - r_in;
+    const double d[3] = { (double)pm[4 * j] - pm[4 * i], (double)pm[4 * j + 1] - pm[4 * i + 1], (double)pm[4 * j + 2] - pm[4 * i + 2] };
+    const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    if (r2 >= r_out * r_out) return 0;
+    if (r2 == 0.0) return 1;
+    const double v[3] = { (double)vel[4 * j] - vel[4 * i], (double)vel[4 * j + 1] - vel[4 * i + 1], (double)vel[4 * j + 2] - vel[4 * i + 2] };
+    const double m = pm[4 * j + 3], r = sqrt(r2), r3 = r2 * r, r5 = r3 * r2;
+    const double dv = d[0] * v[0] + d[1] * v[1] + d[2] * v[2];
+    const double x = (r - r_in) / D;
+    const double K = 1.0 - p3t_o_W(x);
+    const double Kdot = -p3t_o_dW(x) * dv / (r * D);
+    double tn = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        S->a[c] += m * K * d[c] / r3;
+        const double term = m * (K * (v[c] / r3 - 3.0 * dv * d[c] / r5) + Kdot * d[c] / r3);
+        S->jk[c] += term; tn += term * term;
+    }
+    S->ab += sqrt(tn);
+    S->an += m * (sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) / r3 + 3.0 * fabs(dv) / (r2 * r2));
+    S->phi += m * (-1.0 / r - p3t_o_psi(r, r_out, r_in));
+    return 0;
+}
+
+/* cand_off / cand_idx (may be NULL = every j): a caller-given SUPERSET of the neighbour sphere of every target,
+ * as CSR rows over the nt targets (e.g. the rows of p3t_o_neighbours_grid at a radius a little above r_out).
+ * The predicate r2 < r_out^2 and the arithmetic of every pair are the same either way; the candidates only
+ * spare the O(N) scan per target at N = 2^20. */
+int64_t p3t_o_irregular_cand(int64_t n, const float* pm, const float* vel, double r_out, double r_in,
+                             int64_t nt, const int64_t* targets, const int64_t* cand_off, const int32_t* cand_idx,
+                             double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt)
+{
+    int64_t coincident = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : coincident)
+    for (int64_t t = 0; t < nt; ++t) {
+        const int64_t i = targets ? targets[t] : t;
+        irr_acc S;
+        memset(&S, 0, sizeof(S));
+        if (cand_off) {
+            for (int64_t e = cand_off[t]; e < cand_off[t + 1]; ++e) {
+                const int64_t j = cand_idx[e];
+                if (j != i) coincident += irr_pair(pm, vel, r_out, r_in, i, j, &S);
+            }
+        } else {
+            for (int64_t j = 0; j < n; ++j)
+                if (j != i) coincident += irr_pair(pm, vel, r_out, r_in, i, j, &S);
+        }
+        for (int c = 0; c < 3; ++c) {
+            if (acc_irr) acc_irr[3 * t + c] = S.a[c];
+            if (jerk_irr) jerk_irr[3 * t + c] = S.jk[c];
+        }
+        if (phi_irr) phi_irr[t] = S.phi;
+        if (abs_jerk) abs_jerk[t] = S.ab;
+        if (abs_newt) abs_newt[t] = S.an;
+    }
+    return coincident;
+}
+
 int64_t p3t_o_irregular(int64_t n, const float* pm, const float* vel, double r_out, double r_in,
                         int64_t nt, const int64_t* targets,
                         double* acc_irr, double* jerk_irr, double* phi_irr, double* abs_jerk, double* abs_newt)
 {
-    int64_t coincident = 0;
-    const double D = r_out - r_in;
-#pragma omp parallel for schedule(dynamic, 16) reduction(+ : coincident)
-    for (int64_t t = 0; t < nt; ++t) {
-        const int64_t i = targets ? targets[t] : t;
-        const double xi[3] = { pm[4 * i], pm[4 * i + 1], pm[4 * i + 2] };
-        const double vi[3] = { vel[4 * i], vel[4 * i + 1], vel[4 * i + 2] };
-        double a[3] = { 0, 0, 0 }, jk[3] = { 0, 0, 0 }, phi = 0.0, ab = 0.0, an = 0.0;
-        for (int64_t j = 0; j < n; ++j) {
-            if (j == i) continue;
-            const double d[3] = { pm[4 * j] - xi[0], pm[4 * j + 1] - xi[1], pm[4 * j + 2] - xi[2] };
-            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-            if (r2 >= r_out * r_out) continue;
-            if (r2 == 0.0) { ++coincident; continue; }
-            const double v[3] = { vel[4 * j] - vi[0], vel[4 * j + 1] - vi[1], vel[4 * j + 2] - vi[2] };
-            const double m = pm[4 * j + 3], r = sqrt(r2), r3 = r2 * r, r5 = r3 * r2;
-            const double dv = d[0] * v[0] + d[1] * v[1] + d[2] * v[2];
-            const double x = (r - r_in) / D;
-            const double K = 1.0 - p3t_o_W(x);
-            const double Kdot = -p3t_o_dW(x) * dv / (r * D);
-            double tn = 0.0;
-            for (int c = 0; c < 3; ++c) {
-                a[c] += m * K * d[c] / r3;
-                const double term = m * (K * (v[c] / r3 - 3.0 * dv * d[c] / r5) + Kdot * d[c] / r3);
-                jk[c] += term; tn += term * term;
-            }
-            ab += sqrt(tn);
-            an += m * (sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) / r3 + 3.0 * fabs(dv) / (r2 * r2));
-            phi += m * (-1.0 / r - p3t_o_psi(r, r_out, r_in));
-        }
-        for (int c = 0; c < 3; ++c) {
-            if (acc_irr) acc_irr[3 * t + c] = a[c];
-            if (jerk_irr) jerk_irr[3 * t + c] = jk[c];
-        }
-        if (phi_irr) phi_irr[t] = phi;
-        if (abs_jerk) abs_jerk[t] = ab;
-        if (abs_newt) abs_newt[t] = an;
-    }
-    return coincident;
+    return p3t_o_irregular_cand(n, pm, vel, r_out, r_in, nt, targets, NULL, NULL, acc_irr, jerk_irr, phi_irr, abs_jerk, abs_newt);
 }
 
 /* core quantities by a sampled 6-nearest-neighbour search (section 2.5,

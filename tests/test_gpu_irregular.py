@@ -30,7 +30,7 @@ def _cuda(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
 
 
-def _check(p3t, w, targets=None, r_out=None):
+def _check(p3t, w, targets=None, r_out=None, grid=False):
     r_out = w.r_out if r_out is None else r_out
     r_in = float(np.float32(0.1) * np.float32(r_out))
     vel = workloads.velocities_for(w)
@@ -42,7 +42,9 @@ def _check(p3t, w, targets=None, r_out=None):
         off, idx = ctx.neighbours()
         off = off.cpu().numpy(); idx = idx.cpu().numpy()
         st = ctx.stats()
-    o = oracle.irregular(w.pos_mass, vel, r_out, r_in, targets=targets)
+    # grid: every target at N = 2^20 -- the oracle tests only the candidates of its cell-grid search at 1.01 r_out
+    cand = oracle.neighbours_grid(w.pos_mass, 1.01 * r_out, targets=targets) if grid else None
+    o = oracle.irregular(w.pos_mass, vel, r_out, r_in, targets=targets, candidates=cand)
     sel = slice(None) if targets is None else targets
     a, j = acc[sel], jerk[sel]
     ea = np.linalg.norm(a[:, :3] - o["acc_irr"], axis=1)
@@ -60,8 +62,8 @@ def _check(p3t, w, targets=None, r_out=None):
     rows = np.repeat(np.arange(w.n), np.diff(off))
     pos = w.pos_mass[:, :3].astype(np.float64)
     rij = np.linalg.norm(pos[idx] - pos[rows], axis=1)
-    newt = np.zeros(w.n)
-    np.add.at(newt, rows[rij > 0], w.pos_mass[idx[rij > 0], 3].astype(np.float64) / rij[rij > 0])
+    nz = rij > 0
+    newt = np.bincount(rows[nz], weights=w.pos_mass[idx[nz], 3].astype(np.float64) / rij[nz], minlength=w.n)
     assert np.all(np.abs(a[:, 3] - o["phi_irr"]) <= 3e-6 * np.abs(o["phi_irr"]) + 3e-7 * newt[sel] + 1e-30)
     assert np.all(j[:, 3] == 0)
     # empty rows give exact zeros (lists are often empty)
@@ -95,6 +97,13 @@ def test_king_core_sampled(p3t):
     w = workloads.make_config(4, n_override=131072)
     t = workloads.sample_targets(w.n, 4096)
     _check(p3t, w, targets=t)
+
+
+def test_king_core_full_size(p3t):
+    """Config 4 itself (King W0 = 9, N = 2^20, 1.66e7 list entries, rows of up to ~500): EVERY particle."""
+    w = workloads.make_config(4)
+    reg, acc, jerk, o, st = _check(p3t, w, grid=True)
+    assert st["nb_max"] > 256 and st["nb_total"] > 1.5e7
 
 
 def test_state_and_arguments(p3t):

@@ -206,3 +206,57 @@ def test_coincident_pair_reading_R8():
     assert d["phi_reg"][0] == pytest.approx(0.25 * oracle.psi(0.0, R_OUT, R_IN) - 0.25)
     off, idx = oracle.neighbours(pm, R_OUT)
     assert list(idx[off[0]:off[1]]) == [1] and list(idx[off[1]:off[2]]) == [0] and off[3] == off[2]
+
+
+# ---- S10: the uniform-cell-grid search gives exactly the brute-force rows ----
+def _grid_equals_brute(pm, r_out, targets=None):
+    off, idx = oracle.neighbours(pm, r_out, targets=targets)
+    goff, gidx = oracle.neighbours_grid(pm, r_out, targets=targets)
+    assert np.array_equal(off, goff) and np.array_equal(idx, gidx)
+    return off
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 16384), (4, 12000)])
+def test_grid_neighbours_equal_brute_force_on_the_workloads(cfg, n):
+    """Plummer (config 1) and the King W0 = 9 core (config 4's recipe at small N, with the radius of the
+    2^20 run scaled so that the core rows hold hundreds of entries)."""
+    w = workloads.make_config(cfg, n_override=n)
+    r_out = w.r_out if cfg == 1 else 0.05
+    off = _grid_equals_brute(w.pos_mass, r_out)
+    if cfg == 4:
+        assert np.diff(off).max() > 200
+    tg = workloads.sample_targets(w.n, 777)
+    _grid_equals_brute(w.pos_mass, r_out, targets=tg)
+
+
+def test_grid_neighbours_awkward_shapes():
+    rng = np.random.default_rng(7)
+    n = 3000
+    shapes = {
+        "duplicates": np.repeat(rng.random((n // 7 + 1, 3)), 7, axis=0)[:n],
+        "lattice": np.round(rng.random((n, 3)) * 8) / 8,            # many coincident points, distances on cell edges
+        "line": np.c_[rng.random(n), np.zeros(n), np.zeros(n)],
+        "needle": rng.normal(size=(n, 3)) * np.array([1, 1e-3, 1e-6]),
+        "core+halo": np.r_[rng.normal(size=(n - n // 10, 3)) * 0.01, rng.random((n // 10, 3)) * 100],
+        "negative": rng.random((n, 3)) - 37.5,
+    }
+    for name, pos in shapes.items():
+        pm = np.zeros((n, 4), np.float32); pm[:, :3] = pos; pm[:, 3] = 1.0 / n
+        ext = float(np.ptp(pm[:, :3], axis=0).max())
+        for frac in (1e-3, 0.02, 0.125, 0.5, 3.0):                 # 3.0: r_out larger than the whole box (one cell)
+            off = _grid_equals_brute(pm, float(np.float32(ext * frac)))
+            if frac == 3.0:
+                assert off[-1] == n * (n - 1), name
+    # exact cell-edge distances: a unit lattice with r_out = 1 (strict <: face neighbours are NOT members), then just above
+    g = np.stack(np.meshgrid(*[np.arange(9.0)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    pm = np.zeros((len(g), 4), np.float32); pm[:, :3] = g; pm[:, 3] = 1.0
+    off = _grid_equals_brute(pm, 1.0)
+    assert off[-1] == 0
+    off = _grid_equals_brute(pm, float(np.nextafter(np.float32(1.0), np.float32(2.0))))
+    assert off[-1] == 2 * 3 * 8 * 81
+    # a radius so small that the box would need more than 2^20 cells per axis (the edge is enlarged)
+    pm = np.zeros((5, 4), np.float32); pm[:, 0] = [0, 1e-7, 2e-7, 1.0, 1.0 + 1e-7]; pm[:, 3] = 1
+    off = _grid_equals_brute(pm, 1.5e-7)
+    assert list(np.diff(off)) == [1, 2, 1, 1, 1]
+    with pytest.raises(ValueError):
+        oracle.neighbours_grid(pm, 0.0)

@@ -113,3 +113,21 @@ def test_velocity_generator_is_virialised():
     # Plummer sphere in Henon units: <v^2> = 2 T / M = 1/2 (E = -1/4); isotropic
     assert abs((v * v).sum(axis=1).mean() - 0.5) < 0.02
     assert np.abs(v.mean(axis=0)).max() < 0.02
+
+
+def test_candidate_rows_give_the_same_sums():
+    """oracle.irregular(candidates=grid rows at 1.01 r_out) == the scan over every j (which the pins above fix):
+    identical bits, since the pairs inside r_out are visited in the same (ascending j) order."""
+    w = workloads.make_config(4, n_override=6000)
+    vel = workloads.velocities_for(w)
+    r_out, r_in = 0.05, 0.005
+    full = oracle.irregular(w.pos_mass, vel, r_out, r_in)
+    cand = oracle.neighbours_grid(w.pos_mass, 1.01 * r_out)
+    part = oracle.irregular(w.pos_mass, vel, r_out, r_in, candidates=cand)
+    for k in ("acc_irr", "jerk_irr", "phi_irr", "abs_jerk", "abs_newt"):
+        assert np.array_equal(full[k], part[k]), k
+    assert full["coincident"] == part["coincident"]
+    tg = workloads.sample_targets(w.n, 500)
+    cand_t = oracle.neighbours_grid(w.pos_mass, 1.01 * r_out, targets=tg)
+    sub = oracle.irregular(w.pos_mass, vel, r_out, r_in, targets=tg, candidates=cand_t)
+    assert np.array_equal(sub["jerk_irr"], full["jerk_irr"][tg])
