@@ -49,8 +49,11 @@ double p3t_o_psi(double r, double r_out, double r_in)
         S1 += q[k] / pw;
         Sx += q[k] * pow(x, pw) / pw;
     }
-    double integral = (S1 - Sx) + rem * log((1.0 + c) / (x + c));
-    return -p3t_o_W(x) / r - (140.0 / D) * integral;
+    /* r_in = 0 (c = 0): the remainder -c^3 (1+c)^3 is exactly 0 and so is its term (the limit of rem ln(1/x), x -> 0;
+     * written out so that 0 * inf never appears) */
+    double integral = (S1 - Sx) + (rem != 0.0 ? rem * log((1.0 + c) / (x + c)) : 0.0);
+    /* r = 0 is reached only with r_in = 0: W(x)/r ~ 35 x^4 / r -> 0 */
+    return -(r > 0.0 ? p3t_o_W(x) / r : 0.0) - (140.0 / D) * integral;
 }
 
 /* eq. 1, 3, 4, G = 1.  Reading R1: attractive gravity, so the vector in the

@@ -159,7 +159,7 @@ p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pm, int key_bits, int nleaf
      * M = sum m; COM = sum m x / M; Q_ab = sum m (3 d_a d_b - |d|^2 delta_ab), d = x - COM
      * (traceless quadrupole; order xx yy zz xy xz yz); tight AABB = exact min/max;
      * delta = |COM - c_geo|, c_geo,a = lo_a + (p_a + 1/2) l, l = side / 2^level.
-     * M, COM, Q, delta are rounded once to fp32.
+     * M, COM, Q, delta are rounded once to fp32.  M = 0 (all masses zero): reading R-S6a below.
      * SURVEY 8f NEXT-4 (octupole variant): T_abc = sum m d_a d_b d_c, the raw third moment about the COM,
      * order xxx yyy zzz xxy xxz xyy yyz xzz yzz xyz, likewise rounded once to fp32. */
     int64_t nn = t->nn;
@@ -184,6 +184,9 @@ p3t_o_tree* p3t_o_tree_build(int64_t n, const float* pm, int key_bits, int nleaf
             }
         }
         double c[3] = { s[0] / M, s[1] / M, s[2] / M };
+        if (M == 0.0)                      /* reading R-S6a: a cell of massless particles (tracers) has no centre of mass; */
+            for (int a = 0; a < 3; ++a)    /* it takes the position of its first particle in sorted order (Q = 0, delta from it) */
+                c[a] = t->spm[4 * (int64_t)b + a];
         double Q[6] = { 0, 0, 0, 0, 0, 0 }, T[10] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
         for (int32_t i = b; i < e; ++i) {
             const float* p = t->spm + 4 * (int64_t)i;

@@ -34,7 +34,8 @@ __device__ __forceinline__ float cutoff_W(float x)
 __device__ __forceinline__ float cutoff_psi(const walk_consts& K, float x, float W, float rinv)
 {
     float sx = x * (K.sc[0] + x * (K.sc[1] + x * (K.sc[2] + x * (K.sc[3] + x * (K.sc[4] + x * K.sc[5])))));
-    float integral = (K.s1 - sx) - K.rem * __logf((1.0f + K.c) / (x + K.c));
+    // r_in = 0: rem = 0 and its term is identically 0 (never 0 * log(1 / 0))
+    float integral = (K.s1 - sx) - (K.rem > 0.0f ? K.rem * __logf((1.0f + K.c) / (x + K.c)) : 0.0f);
     return -W * rinv - K.k140 * integral;
 }
 // The closed form cancels: terms of order 1 give an integral of order 1e-2 .. 0 that is then multiplied
@@ -61,7 +62,7 @@ static inline void make_consts(walk_consts& K, float r_out, float r_in, float th
     K.drem = c * c * c * c1 * c1 * c1; K.rem = (float)K.drem;
     K.c = (float)c; K.dc = c; K.dlog1c = log(c1);
     // psi(r_in) = -(140/D) [ S(1) + rem ln((1+c)/c) ... ] with W(0) = 0; here the remainder enters with a minus sign
-    K.psi_in = (float)(-(140.0 / D) * (s1 - c * c * c * c1 * c1 * c1 * log(c1 / c)));
+    K.psi_in = (float)(-(140.0 / D) * (s1 - (c > 0.0 ? c * c * c * c1 * c1 * c1 * log(c1 / c) : 0.0)));   // r_in = 0: the remainder term is exactly 0
     K.theta = theta;
     K.pot_mode = pot_mode;
 }

@@ -220,8 +220,9 @@ int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* j
         for (int k = 0; k <= PSI_TAB; ++k) {
             const double x = (double)k / PSI_TAB;
             const double sx = x * (K.dsc[0] + x * (K.dsc[1] + x * (K.dsc[2] + x * (K.dsc[3] + x * (K.dsc[4] + x * K.dsc[5])))));
-            I[k] = k == PSI_TAB ? 0.0 : (K.ds1 - sx) - K.drem * (K.dlog1c - log(x + K.dc));
-            dI[k] = -x * x * x * (1.0 - x) * (1.0 - x) * (1.0 - x) / (x + K.dc) / PSI_TAB;
+            // r_in = 0 (c = 0): the remainder term is exactly 0, and t^3 / (t + c) = t^2 also at t = 0
+            I[k] = k == PSI_TAB ? 0.0 : (K.ds1 - sx) - (K.drem > 0.0 ? K.drem * (K.dlog1c - log(x + K.dc)) : 0.0);
+            dI[k] = -(x + K.dc > 0.0 ? x * x * x / (x + K.dc) : 0.0) * (1.0 - x) * (1.0 - x) * (1.0 - x) / PSI_TAB;
         }
         float* h = ctx->psitab_host;
         for (int k = 0; k < PSI_TAB; ++k) {

@@ -24,8 +24,9 @@ __global__ void __launch_bounds__(256) k_cube(const float4* __restrict__ pm, int
         float4 p = __ldg(pm + i);
         float v[3] = { p.x + 0.0f, p.y + 0.0f, p.z + 0.0f };              // -0 -> +0
         // finite test: |v| <= FLT_MAX is false for NaN and Inf
+        // a negative mass is rejected too (cell masses could cancel); zero masses (tracers) are legal: R-S6a
         bad |= !(fabsf(p.x) <= 3.402823466e38f) | !(fabsf(p.y) <= 3.402823466e38f) |
-               !(fabsf(p.z) <= 3.402823466e38f) | !(fabsf(p.w) <= 3.402823466e38f);
+               !(fabsf(p.z) <= 3.402823466e38f) | !(p.w >= 0.0f && p.w <= 3.402823466e38f);
 #pragma unroll
         for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], v[a]); hi[a] = fmaxf(hi[a], v[a]); }
     }

@@ -218,13 +218,12 @@ __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-w
 
 // R-S6 output of one cell: fp32 rounding of the fp64 moments, delta, and the walk's link word
 __device__ void store_node(const tree_args& A, int k, int level, int b, int e, int first, int nchild,
-                           double M, const double s[3], const double Q[6], const float clo[3], const float chi[3])
+                           double M, const double s[3], const double c[3], const double Q[6], const float clo[3], const float chi[3])
 {
     double* m = A.m64 + (size_t)k * 13;
     m[0] = M; m[1] = s[0]; m[2] = s[1]; m[3] = s[2];
 #pragma unroll
     for (int q = 0; q < 6; ++q) m[4 + q] = Q[q];
-    const double c[3] = { s[0] / M, s[1] / M, s[2] / M };
     m[10] = c[0]; m[11] = c[1]; m[12] = c[2];       // the parent reads the quotient instead of dividing again (same bits)
     // geometric centre from the integer cell coordinates (prefix of the first key)
     const uint64_t prefix = level == 0 ? 0ull : (A.keys[b] >> (3 * (A.B - level)));
@@ -266,7 +265,9 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
             clo[0] = fminf(clo[0], p.x); clo[1] = fminf(clo[1], p.y); clo[2] = fminf(clo[2], p.z);
             chi[0] = fmaxf(chi[0], p.x); chi[1] = fmaxf(chi[1], p.y); chi[2] = fmaxf(chi[2], p.z);
         }
-        const double c[3] = { s[0] / M, s[1] / M, s[2] / M };
+        // R-S6a: a cell of massless particles takes the position of its first particle (sorted order) as its centre
+        const bool massless = M == 0.0;
+        const double c[3] = { massless ? (double)p0.x : s[0] / M, massless ? (double)p0.y : s[1] / M, massless ? (double)p0.z : s[2] / M };
         double Q[6] = { 0, 0, 0, 0, 0, 0 };
         for (int i = b; i < e; ++i) {
             float4 p = A.spm[i];
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
             Q[0] += m * (3 * dx * dx - d2); Q[1] += m * (3 * dy * dy - d2); Q[2] += m * (3 * dz * dz - d2);
             Q[3] += m * 3 * dx * dy; Q[4] += m * 3 * dx * dz; Q[5] += m * 3 * dy * dz;
         }
-        store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, Q, clo, chi);
+        store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, c, Q, clo, chi);
     }
     for (;;) {
         const int p = A.nparent[k];
@@ -295,7 +296,10 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
             clo[0] = fminf(clo[0], lo.x); clo[1] = fminf(clo[1], lo.y); clo[2] = fminf(clo[2], lo.z);
             chi[0] = fmaxf(chi[0], hi.x); chi[1] = fmaxf(chi[1], hi.y); chi[2] = fmaxf(chi[2], hi.z);
         }
-        const double cm[3] = { s[0] / M, s[1] / M, s[2] / M };
+        // R-S6a: massless cell: the centre of its first child, i.e. its first particle in sorted order
+        const bool massless = M == 0.0;
+        const double* m0 = A.m64 + (size_t)fc * 13;
+        const double cm[3] = { massless ? __ldcg(m0 + 10) : s[0] / M, massless ? __ldcg(m0 + 11) : s[1] / M, massless ? __ldcg(m0 + 12) : s[2] / M };
         double Q[6] = { 0, 0, 0, 0, 0, 0 };
         for (int c = fc; c < fc + nc; ++c) {
             const double* m = A.m64 + (size_t)c * 13;
@@ -305,7 +309,7 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
             Q[0] += __ldcg(m + 4) + Mc * (3 * dx * dx - d2); Q[1] += __ldcg(m + 5) + Mc * (3 * dy * dy - d2); Q[2] += __ldcg(m + 6) + Mc * (3 * dz * dz - d2);
             Q[3] += __ldcg(m + 7) + Mc * 3 * dx * dy; Q[4] += __ldcg(m + 8) + Mc * 3 * dx * dz; Q[5] += __ldcg(m + 9) + Mc * 3 * dy * dz;
         }
-        store_node(A, k, A.nlevel[k], A.nbegin[k], A.nend[k], fc, nc, M, s, Q, clo, chi);
+        store_node(A, k, A.nlevel[k], A.nbegin[k], A.nend[k], fc, nc, M, s, cm, Q, clo, chi);
     }
 }
 

@@ -528,3 +528,59 @@ def test_neighbour_rows_of_every_sort_class(p3t):
         off, idx = check_neighbours(ctx, w)
         lens = np.diff(off)
         assert lens.max() > 2048 and np.any((lens > 32) & (lens <= 2048)) and np.any((lens > 16) & (lens <= 32)) and np.any(lens <= 16)
+
+
+def test_massless_particles(p3t):
+    """tracers with m = 0 (reading R-S6a: a massless cell takes its first particle as its centre), incl.
+    massless cells alone far away: finite forces, cells / lists / CSR bit-exact, force within the R15 bound."""
+    w = workloads.make_config(1, n_override=6000)
+    pm = w.pos_mass.copy()
+    pm[500:560, 3] = 0.0
+    far = np.array([[50.0, 50.0, 50.0, 0.0], [50.001, 50.0, 50.0, 0.0], [-40.0, 3.0, 1.0, 0.0]], dtype=np.float32)
+    pm = np.vstack([pm, far]).astype(np.float32)
+
+    class W: pass
+    v = W(); v.pos_mass = pm; v.n = pm.shape[0]; v.r_out = w.r_out; v.r_in = w.r_in; v.theta = 0.4
+    for nleaf, ncrit in ((16, 64), (2, 8)):
+        T = oracle.Tree(pm, 63, nleaf, ncrit)
+        with p3t.Context(0, nleaf=nleaf, ncrit=ncrit) as ctx:
+            ctx.build_tree(_cuda(pm), 63)
+            check_build(ctx, T, pm, 63)
+            a, _ = check_force(ctx, T, v, 0, per_particle=False)
+            assert np.all(np.isfinite(a))
+            check_neighbours(ctx, v)
+    # a negative mass is rejected by the bounding-cube reduction
+    bad = pm.copy(); bad[7, 3] = -1.0e-3
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(bad), 63)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.stats()
+        assert e.value.code == p3t.EINVAL
+
+
+def test_r_in_zero(p3t):
+    """r_in = 0 (the cutoff reaches down to r = 0) incl. coincident pairs: finite, equal to the oracle."""
+    w = workloads.make_config(1, n_override=4000)
+    pm = w.pos_mass.copy()
+    pm[10] = pm[11]; pm[10, 3] = pm[11, 3]                      # a coincident pair
+    class W: pass
+    v = W(); v.pos_mass = pm; v.n = pm.shape[0]; v.r_out = w.r_out; v.r_in = 0.0; v.theta = 0.4
+    T = oracle.Tree(pm, 63, NLEAF, NCRIT)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(pm), 63)
+        for pot_mode in (0, 1):
+            a, _ = check_force(ctx, T, v, pot_mode)
+            assert np.all(np.isfinite(a))
+        d = oracle.direct(pm, v.r_out, 0.0)
+        a = ctx.regular_force(v.r_out, 0.0, 1e-3, 0).cpu().numpy().astype(np.float64)
+        assert np.abs(a[:, 3] / d["phi_reg"] - 1).max() < 2e-6
+        # irregular side: the psi table at c = 0
+        vel = workloads.velocities_for(w)
+        ctx.regular_force(v.r_out, 0.0, 0.4, 0)
+        acc, jerk = ctx.irregular_force(_cuda(vel))
+        o = oracle.irregular(pm, vel, v.r_out, 0.0)
+        acc = acc.cpu().numpy().astype(np.float64)
+        assert np.all(np.isfinite(acc)) and np.all(np.isfinite(jerk.cpu().numpy()))
+        assert np.linalg.norm(acc[:, :3] - o["acc_irr"]) <= 1e-6 * np.linalg.norm(o["acc_irr"])
+        tot = np.abs(o["phi_irr"]).max()
+        assert np.abs(acc[:, 3] - o["phi_irr"]).max() <= 3e-6 * tot

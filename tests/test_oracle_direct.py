@@ -260,3 +260,19 @@ def test_grid_neighbours_awkward_shapes():
     assert list(np.diff(off)) == [1, 2, 1, 1, 1]
     with pytest.raises(ValueError):
         oracle.neighbours_grid(pm, 0.0)
+
+
+# ---- reading R6 at r_in = 0 (the cutoff reaches down to r = 0; the remainder term of psi vanishes) ----
+def test_psi_with_r_in_zero():
+    r_out = 0.05
+    # closed form: c = 0, t^3 (1-t)^3 / t = t^2 (1-t)^3, integral over [0, 1] = 1/60  =>  psi(0) r_out = -140/60 = -7/3
+    assert oracle.psi(0.0, r_out, 0.0) * r_out == pytest.approx(-7.0 / 3.0, rel=1e-13)
+    for r in (1e-6, 0.003, 0.02, 0.049):
+        x_of = lambda s: s / r_out
+        tail, _ = integrate.quad(lambda s: oracle.W(x_of(s)) / (s * s), r, r_out, epsabs=0, epsrel=1e-12)
+        assert oracle.psi(r, r_out, 0.0) == pytest.approx(-tail - 1.0 / r_out, rel=1e-10)
+    pm = np.array([[0, 0, 0, 0.5], [0, 0, 0, 0.25], [0.01, 0, 0, 0.25]], dtype=np.float32)
+    d = oracle.direct(pm, r_out, 0.0)
+    assert np.all(np.isfinite(d["phi_reg"])) and np.all(np.isfinite(d["acc_reg"]))
+    r = float(pm[2, 0])
+    assert d["phi_reg"][0] == pytest.approx(0.25 * oracle.psi(0.0, r_out, 0.0) + 0.25 * oracle.psi(r, r_out, 0.0))

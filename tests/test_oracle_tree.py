@@ -345,3 +345,32 @@ def test_monopole_only_variant(cfg1):
     o = oracle.pc_term(xi, cm, np.zeros(6, np.float32))
     r = xi - cm[:3]; R = np.linalg.norm(r)
     assert np.allclose(o[:3], -2.0 * r / R ** 3, rtol=1e-14) and np.isclose(o[3], -2.0 / R, rtol=1e-14)
+
+
+# ---- reading R-S6a: massless particles (tracers) ----
+def test_massless_cells_take_their_first_particle_as_centre():
+    pm = _small(2000)
+    pm[100:140, 3] = 0.0                                         # some tracers inside the cluster
+    far = np.array([[50.0, 50.0, 50.0, 0.0], [50.001, 50.0, 50.0, 0.0], [-40.0, 3.0, 1.0, 0.0]], dtype=np.float32)
+    pm = np.vstack([pm, far]).astype(np.float32)                 # massless cells far away (alone in their octants)
+    T = oracle.Tree(pm, 63, 4, 16)
+    m = T.moments(); nd = T.nodes(); m64 = T.moments64()
+    k, o = T.keys()
+    spm = pm[o]
+    assert np.all(np.isfinite(m["com_m"])) and np.all(np.isfinite(m["quad"])) and np.all(np.isfinite(m["delta"]))
+    massless = np.nonzero(m64["mass"] == 0.0)[0]
+    assert len(massless) >= 2
+    for c in massless:
+        assert np.array_equal(m["com_m"][c, :3], spm[nd["begin"][c], :3]) and np.all(m["quad"][c] == 0) and m["com_m"][c, 3] == 0
+    # every other cell: the mass-weighted mean as before
+    c = int(np.nonzero(m64["mass"] > 0)[0][-1])
+    b, e = nd["begin"][c], nd["end"][c]
+    w = spm[b:e, 3].astype(np.float64)
+    assert np.allclose(m64["com"][c], (w[:, None] * spm[b:e, :3]).sum(0) / w.sum(), rtol=1e-14)
+    # the force on the tracers and from the cluster is still eq. 3: theta -> 0 is the direct sum
+    ro, ri = float(np.float32(0.05)), float(np.float32(0.005))
+    f = T.force(ro, ri, 1e-7, 0)                                  # the cube is 128 wide here: every cell opens only for a tiny angle
+    d = oracle.direct(pm, ro, ri)
+    assert np.abs(f["acc_pot"][:, :3] - d["acc_reg"]).max() <= 1e-11 * np.abs(d["acc_reg"]).max()
+    f4 = T.force(0.05, 0.005, 0.4, 0)
+    assert np.all(np.isfinite(f4["acc_pot"]))
