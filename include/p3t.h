@@ -16,7 +16,8 @@
  *  - Every call returns P3T_OK (0) or a negative error code; no exceptions, no exit, no stdout.
  *  - "DEVICE pointer": memory of the context's CUDA device.  "HOST pointer": ordinary host memory
  *    (pinned or pageable).  "ANY pointer": either one (copied with cudaMemcpyDefault).
- *  - Calls enqueue work on the context's stream and do NOT synchronise unless stated.
+ *  - Calls enqueue work on the context's stream and do NOT synchronise unless stated.  p3t_build_tree does not;
+ *    p3t_regular_force / _ex synchronise once, at their end (see there); the accessors synchronise.
  *  - The library never frees caller memory and writes only to the output arguments named below.
  *  - One context per host thread; a context is bound to one device and one stream.
  *  - Every step runs in the library's CUDA kernels; there is no CPU fallback.
@@ -31,8 +32,9 @@ extern "C" {
 
 #define P3T_OK       0
 #define P3T_EINVAL  -1   /* bad argument: n < 1, n > P3T_MAX_N, r_in < 0, r_in >= r_out, theta <= 0,
-                            key_bits not 30/63, null pointer, NaN/Inf position or mass (found by
-                            the bounding-cube reduction; reported by the next synchronising call) */
+                            key_bits not 30/63, null pointer, NaN/Inf position or mass, negative mass
+                            (found by the bounding-cube reduction of p3t_build_tree; reported by the next
+                            synchronising call, p3t_regular_force included, which then writes nothing) */
 #define P3T_ESTATE  -2   /* force before build, neighbours before force, ... */
 #define P3T_ENOMEM  -3   /* device allocation failed */
 #define P3T_ECUDA   -4   /* a CUDA call failed; sticky; text via p3t_last_error */
@@ -131,7 +133,14 @@ int p3t_build_tree(p3t_ctx* ctx, int64_t n, const float* pos_mass, int key_bits)
  * acc_pot: DEVICE pointer, n x {ax, ay, az, phi} fp32, caller-owned, ORIGINAL particle order.
  * pot_mode 0: phi = regular potential (its gradient is -a; R6); 1: unsplit Newtonian
  * potential -sum m_j / r_ij.  Requires a prior build; theta, r_out, r_in may change between
- * calls without a rebuild.  Also produces the neighbour lists returned by p3t_neighbours. */
+ * calls without a rebuild.  Also produces the neighbour lists returned by p3t_neighbours.
+ * r_in = 0 is legal (the cutoff then reaches down to r = 0); masses of 0 are legal (tracers; DESIGN.md R-S6a).
+ * SYNCHRONISES the stream once, at its end: the whole call is enqueued first (the list walk runs on a second
+ * stream of the context beside the force kernel and is joined back), then the host waits, so that on return
+ * acc_pot, vel and the lists are complete and every error of the build or the walk is reported by THIS call:
+ * P3T_EINVAL for NaN/Inf/negative input (nothing was written, vel is not kicked), P3T_ECUDA for an exceeded
+ * internal capacity (walk stack, cell count: outputs unspecified).  List buffers sized by the previous call that
+ * turn out too small are regrown and the missing part is redone inside the call (normally only the first call). */
 int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float* acc_pot);
 
 /* p3t_regular_force with the neighbour search reaching r_list = r_out + r_buff
@@ -213,13 +222,6 @@ int p3t_get_groups(p3t_ctx* ctx, int32_t* begin, int32_t* end);
 /* per-group list lengths of the last force call: npp[n_groups], npc[n_groups] (int32) */
 int p3t_get_list_lengths(p3t_ctx* ctx, int32_t* npp, int32_t* npc);
 
-/* Micro-benchmarks of the FP32 pipe (the ALU roofline of the force kernel and the
- * per-instruction costs behind it).  cycles_out: HOST double[n_out >= 8], SM-clock cycles per SM
- * sub-partition of: [0] FFMA (best case: operands in the reuse cache), [1] FFMA2 with two distinct register pairs, [2] FFMA2 with three, [3] FMUL2,
- * [4] one FMUL2 + one FFMA, [5] eight FMUL2 + two MUFU.RSQ, [6] MUFU.RSQ, [7] FFMA with three distinct registers.  sm_clock_mhz / num_sms: HOST,
- * may be NULL (the device's nominal maximum clock, which the cycle counts assume).  Synchronises; ~20 ms. */
-int p3t_pipe_bench(int device, double* cycles_out, int n_out, double* sm_clock_mhz, int* num_sms);
-
 const char* p3t_strerror(int code);
 const char* p3t_last_error(p3t_ctx* ctx);     /* text of the last CUDA failure ("" if none) */
 
@@ -227,11 +229,6 @@ const char* p3t_last_error(p3t_ctx* ctx);     /* text of the last CUDA failure (
  * r_buff = 3 tau sigma, dt_reg = largest 2^-k <= tau, dt_max = dt_reg / 4.  Any output may be NULL. */
 int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, double* r_buff,
                       double* dt_reg, double* dt_max);
-
-/* Host helper, eq. 18-19: R_min = 4 r_h / (N rho_core^(1/3)), dT_min = 0.01 sqrt(eta / 0.02)
- * sqrt(R_min^3): the regularisation parameters that p3t_core_quantities' rho_core feeds (r_h = half-mass
- * radius, eta = 0.02 in the paper).  Either output may be NULL. */
-int p3t_regularisation_params(int64_t n, double r_h, double rho_core, double eta, double* r_min, double* dt_min);
 
 #ifdef __cplusplus
 }

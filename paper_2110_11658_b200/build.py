@@ -16,8 +16,10 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libp3t.so"
-SOURCES = ["p3t_api.cu", "p3t_sort.cu", "p3t_tree.cu", "p3t_walk.cu", "p3t_force.cu", "p3t_irregular.cu", "p3t_core.cu", "p3t_shard.cu", "p3t_octupole.cu", "p3t_pipebench.cu"]
-HEADERS = [CSRC / "p3t_internal.cuh", CSRC / "p3t_cutoff.cuh", CSRC / "p3t_f32x2.cuh", ROOT / "include" / "p3t.h"]
+SOURCES = ["p3t_api.cu", "p3t_sort.cu", "p3t_tree.cu", "p3t_walk.cu", "p3t_force.cu", "p3t_irregular.cu", "p3t_core.cu", "p3t_shard.cu", "p3t_octupole.cu"]
+DIAG_LIB = PKG / "libp3t_diag.so"          # diagnostics (include/p3t_diag.h): its own library, not linked into libp3t.so
+DIAG_SOURCES = ["p3t_pipebench.cu"]
+HEADERS = [CSRC / "p3t_internal.cuh", CSRC / "p3t_cutoff.cuh", CSRC / "p3t_f32x2.cuh", ROOT / "include" / "p3t.h", ROOT / "include" / "p3t_diag.h"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC",
@@ -33,9 +35,9 @@ def _nvcc() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
-    srcs = [CSRC / s for s in SOURCES]
+    srcs = [CSRC / s for s in SOURCES + DIAG_SOURCES]
     deps = srcs + HEADERS + [Path(__file__)]
-    if not force and LIB.exists() and all(LIB.stat().st_mtime >= d.stat().st_mtime for d in deps):
+    if not force and LIB.exists() and DIAG_LIB.exists() and all(min(LIB.stat().st_mtime, DIAG_LIB.stat().st_mtime) >= d.stat().st_mtime for d in deps):
         return LIB
     objdir = PKG / "build"
     objdir.mkdir(exist_ok=True)
@@ -56,12 +58,14 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     (objdir / "ptxas.log").write_text("\n".join(log))
     if verbose:
         print("\n".join(log))
-    tmp = LIB.with_suffix(f".{os.getpid()}.tmp.so")
-    cmd = [nvcc, "-shared", "-o", str(tmp), *objs, "-cudart", "shared", "-Xcompiler", "-fPIC"]
-    r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    if r.returncode != 0:
-        raise RuntimeError(f"link failed:\n{r.stdout}")
-    os.replace(tmp, LIB)
+    ndiag = len(DIAG_SOURCES)
+    for lib, group in ((LIB, objs[:-ndiag]), (DIAG_LIB, objs[-ndiag:])):
+        tmp = lib.with_suffix(f".{os.getpid()}.tmp.so")
+        cmd = [nvcc, "-shared", "-o", str(tmp), *group, "-cudart", "shared", "-Xcompiler", "-fPIC"]
+        r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"link failed:\n{r.stdout}")
+        os.replace(tmp, lib)
     return LIB
 
 

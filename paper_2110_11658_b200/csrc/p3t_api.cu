@@ -55,6 +55,14 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     memset(c, 0, sizeof(*c));
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
     c->nleaf = 16; c->ncrit = 64; c->order = 2; c->shard_nranks = 1;
+    // diagnostics knobs (measurement only; the defaults are the product): P3T_OVERLAP=0 runs the list walk and the force
+    // kernel one after the other, P3T_WALK_CTAS sets the CTAs per SM left to the walk while they overlap
+    const char* ev = getenv("P3T_OVERLAP");
+    c->overlap = ev ? atoi(ev) != 0 : 1;
+    ev = getenv("P3T_WALK_CTAS");
+    c->walk_ctas_per_sm = ev && atoi(ev) > 0 ? atoi(ev) : 1;
+    ev = getenv("P3T_TEST_FAULT");                         // fault injection for the tests of the error / repair paths
+    c->test_fault = ev ? atoi(ev) : 0;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
     for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[k]);
@@ -79,7 +87,7 @@ int p3t_destroy(p3t_ctx* c)
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
                         &c->gflag, &c->gbegin, &c->gnpp, &c->gnpc, &c->nbcount, &c->nboff, &c->nbidx, &c->nbcur, &c->nbcnt, &c->part, &c->spill, &c->pcpool, &c->pppool, &c->glist,
-                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->shard_nominal, &c->shard_cuts, &c->o64, &c->noct, &c->octcnt, &c->psitab, &c->irrpv };
+                        &c->info, &c->stage_in, &c->stage_out, &c->core, &c->gready, &c->shard_nominal, &c->shard_cuts, &c->o64, &c->noct, &c->octcnt, &c->psitab, &c->irrpv };
     for (p3t_buf* b : bufs) if (b->p) cudaFree(b->p);
     for (int k = 0; k < 6; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     for (int k = 0; k < 4; ++k) if (c->evw[k]) cudaEventDestroy(c->evw[k]);
@@ -87,6 +95,10 @@ int p3t_destroy(p3t_ctx* c)
     for (int k = 0; k < 2; ++k) if (c->evc[k]) cudaEventDestroy(c->evc[k]);
     for (int k = 0; k < 2; ++k) if (c->evo[k]) cudaEventDestroy(c->evo[k]);
     if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
+    if (c->walk_stream) {
+        cudaStreamSynchronize(c->walk_stream); cudaStreamDestroy(c->walk_stream);
+        cudaEventDestroy(c->ev_tree); cudaEventDestroy(c->ev_scan); cudaEventDestroy(c->ev_wdone);
+    }
     (void)cudaGetLastError();
     delete c;
     return P3T_OK;
@@ -141,7 +153,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     int rc;
 #define RES(buf, bytes) if ((rc = p3t_reserve(c, &c->buf, (bytes))) != P3T_OK) return rc
     RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16); RES(rank, N * 4);
-    RES(hist, (ntiles + 1) * P3T_RADIX * 4);
+    RES(hist, p3t_sort_scratch_bytes(n));
     RES(nlevel, C * 4); RES(nbegin, C * 4); RES(nend, C * 4); RES(nfirst, C * 4); RES(nnchild, C * 4);
     RES(m64, C * 104);
     RES(ncom, C * 16); RES(nlo, C * 16); RES(nhi, C * 16); RES(nq0, C * 16); RES(nq1, C * 8); RES(nlink, C * 8);
@@ -164,8 +176,8 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     return P3T_OK;
 }
 
-int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
-                         float half_dt, float* vel, float* acc_pot)
+static int force_check_args(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                            float half_dt, float* vel, float* acc_pot)
 {
     if (!c || !acc_pot) return P3T_EINVAL;
     if (!(r_in >= 0.0f) || !(r_in < r_out) || !(theta > 0.0f) || !isfinite(r_out) || !isfinite(theta)) return P3T_EINVAL;
@@ -182,8 +194,19 @@ int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int p
     c->nb_valid = 0; c->irr_done = 0;
     volatile float rl = r_out + r_buff;                        // one fp32 sum: the list radius of DESIGN.md section 10
     c->r_out = r_out; c->r_in = r_in; c->theta = theta; c->r_list = rl;
-    int rc = p3t_launch_force(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot, rl, half_dt, (float4*)vel);
+    return P3T_OK;
+}
+
+int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                         float half_dt, float* vel, float* acc_pot)
+{
+    int rc = force_check_args(c, r_out, r_in, theta, pot_mode, r_buff, half_dt, vel, acc_pot);
     if (rc != P3T_OK) return rc;
+    if ((rc = p3t_force_begin(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot, c->r_list, half_dt, (float4*)vel)) != P3T_OK) {
+        (void)p3t_force_finish(c);                           // whatever was enqueued is drained before the error is returned
+        return rc;
+    }
+    if ((rc = p3t_force_finish(c)) != P3T_OK) return rc;
     c->state = 2; c->nb_valid = 1;
     return P3T_OK;
 }
@@ -345,28 +368,34 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
     float* d_out = d_pm + (size_t)n * 4;
     P3T_CUDA(c, cudaMemcpyAsync(d_pm, pos_mass_host, (size_t)n * 16, cudaMemcpyHostToDevice, c->stream));
     if ((rc = p3t_build_tree(c, n, d_pm, key_bits)) != P3T_OK) return rc;
-    if ((rc = p3t_regular_force(c, r_out, r_in, theta, pot_mode, d_out)) != P3T_OK) return rc;
-    // The CSR offsets were final before the force call's one host synchronisation (they size the lists):
-    // their copy goes to a second stream and overlaps the force kernel that is still running.
-    if (nb_offsets_host) {
-        if (!c->copy_stream) P3T_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-        P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->copy_stream));
-    }
+    if ((rc = force_check_args(c, r_out, r_in, theta, pot_mode, 0.0f, 0.0f, nullptr, d_out)) != P3T_OK) return rc;
+    if ((rc = p3t_force_begin(c, r_out, r_in, theta, pot_mode, (float4*)d_out, c->r_list, 0.0f, nullptr)) != P3T_OK) { (void)p3t_force_finish(c); return rc; }
+    // The CSR offsets and the entry count are final once the offset scan is through (ev_scan), long before the force
+    // kernel ends: their copies go to a second stream and overlap it.  The host waits for that stream only.
+    if (!c->copy_stream) P3T_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    p3t_devinfo h;
+    P3T_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_scan, 0));
+    if (nb_offsets_host) P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->copy_stream));
+    P3T_CUDA(c, cudaMemcpyAsync(&h, c->info.p, sizeof(h), cudaMemcpyDeviceToHost, c->copy_stream));
+    cudaError_t e = cudaStreamSynchronize(c->copy_stream);
+    if (e != cudaSuccess) { (void)p3t_force_finish(c); return p3t_fail_cuda(c, e, "copy stream", __LINE__); }
+    int64_t total = (int64_t)h.nb_total;
+    const bool fits = total <= c->nb_cap && !h.bad_input;                 // else nothing was emitted: the repair pass of finish does it
     P3T_CUDA(c, cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
-    const int64_t total = c->nb_total_host;                  // known on the host since the force call sized the lists
-    if (nb_total) *nb_total = total;
     int over = 0;
     if (nb_indices_host) {
         if (total > nb_cap) over = 1;
-        else if (total > 0) P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
+        else if (total > 0 && fits) P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
     }
-    p3t_devinfo h;
-    rc = sync_and_check(c, &h);
-    if (nb_offsets_host && c->copy_stream) {                 // on every path: the caller's buffer must be quiet on return
-        cudaError_t e = cudaStreamSynchronize(c->copy_stream);
-        if (e != cudaSuccess && rc == P3T_OK) return p3t_fail_cuda(c, e, "copy stream", __LINE__);
+    if ((rc = p3t_force_finish(c)) != P3T_OK) return rc;            // synchronises the stream: the copies above are done
+    c->state = 2; c->nb_valid = 1;
+    if (c->pend.repaired || !fits) {                                // (first call of a context, normally) results changed after the copies
+        P3T_CUDA(c, cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
+        if (nb_indices_host && !over && total > 0)
+            P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
+        P3T_CUDA(c, cudaStreamSynchronize(c->stream));
     }
-    if (rc != P3T_OK) return rc;
+    if (nb_total) *nb_total = total;
     return over ? P3T_ERANGE : P3T_OK;
 }
 
@@ -473,16 +502,6 @@ int p3t_params_from_n(int64_t n, double sigma, double* tau, double* r_cut, doubl
     if (r_buff) *r_buff = 3.0 * t * sigma;                                    // eq. 20
     if (dt_reg) *dt_reg = dt;
     if (dt_max) *dt_max = dt / 4.0;                                           // eq. 24-25
-    return P3T_OK;
-}
-
-// eq. 18-19: the regularisation parameters that the core quantities feed
-int p3t_regularisation_params(int64_t n, double r_h, double rho_core, double eta, double* r_min, double* dt_min)
-{
-    if (n < 1 || !(r_h > 0.0) || !(rho_core > 0.0) || !(eta > 0.0)) return P3T_EINVAL;
-    const double rm = 4.0 * r_h / ((double)n * cbrt(rho_core));               // eq. 18
-    if (r_min) *r_min = rm;
-    if (dt_min) *dt_min = 0.01 * sqrt(eta / 0.02) * sqrt(rm * rm * rm);       // eq. 19
     return P3T_OK;
 }
 

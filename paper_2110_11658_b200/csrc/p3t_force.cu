@@ -41,6 +41,11 @@ struct force_args {
     float4* vel;                // in/out (may be NULL): velocities, original order, kicked by half_dt * F_R (eq. 12)
     float half_dt;
     p3t_devinfo* info;
+    int32_t* gready;            // per-group list state written by the walkers (p3t_internal.cuh: G_READY ...)
+    int base;                   // epoch of the call
+    int mode;                   // 0: the walkers run at the same time, wait for every group; 1: host repair pass
+    int evalall;                // repair pass: every group again (the lists were not emitted), else only the redone ones
+    long long nb_cap;           // capacity of nbraw in entries
     walk_consts K;
 };
 
@@ -185,7 +190,7 @@ __device__ __forceinline__ float pp_far_pair(target& T, f2 px, f2 py, f2 pz, f2 
 // (bit mask), run only by warps that have such a block in the tile (about one tile in eight).  nbrow[slot] counts the entries already written
 // to the target's CSR row (shared by the parts of a target).
 __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE], const int* ppj, uint32_t nearblocks,
-                                             long long rowbase, int* rowcnt, const force_args& A)
+                                             long long rowbase, int* rowcnt, const force_args& A, bool emit)
 {
     const walk_consts& K = A.K;
     while (nearblocks) {
@@ -198,7 +203,7 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
             if (d2 < K.rlist2) {
                 const int j = ppj[e];
                 if (T.id >= 0 && j != T.id) {                        // self excluded by index; idle lanes
-                    A.nbraw[rowbase + atomicAdd(rowcnt, 1)] = (int32_t)A.order[j];
+                    if (emit) A.nbraw[rowbase + atomicAdd(rowcnt, 1)] = (int32_t)A.order[j];
                     const float m = pp[3][e];
                     if (d2 >= K.rout2) {                               // buffer shell r_out <= r < r_list: on the list, wholly regular
                         const float ri = rsqrt_approx(d2), mr = m * ri, f = mr * ri * ri;
@@ -223,7 +228,7 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
 }
 
 __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], const int* ppj, int part, int k,
-                                        long long rowbase, int* rowcnt, const force_args& A)
+                                        long long rowbase, int* rowcnt, const force_args& A, bool emit)
 {
     uint32_t nearblocks = 0;                     // bit b: this lane's target came within r_out of block b
 #pragma unroll 2
@@ -236,7 +241,7 @@ __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], cons
         if (dmin < A.K.rlist2) nearblocks |= 1u << (e >> 2);
     }
     if (!__any_sync(0xffffffffu, nearblocks != 0)) return;
-    pp_near_pass(T, pp, ppj, nearblocks, rowbase, rowcnt, A);
+    pp_near_pass(T, pp, ppj, nearblocks, rowbase, rowcnt, A, emit);
 }
 
 // Software pipeline of the list stream: the ids of tile t+2 and the node / particle data of tile
@@ -245,7 +250,9 @@ __device__ __forceinline__ void eval_pp(target& T, const float (*pp)[TILE], cons
 struct pc_regs { float4 c, q0; float2 q1; };
 struct pp_regs { float4 p; int j; };
 
-__device__ __forceinline__ int load_id(const int32_t* ids, int e, int n) { return e < n ? ids[e] : -1; }
+// list ids and the group record were written by another SM during this kernel: read them past L1 (a line of glist
+// holds eight groups, some of them not yet published when the line is first fetched)
+__device__ __forceinline__ int load_id(const int32_t* ids, int e, int n) { return e < n ? __ldcg(ids + e) : -1; }
 
 __device__ __forceinline__ pc_regs gather_pc(const force_args& A, int id)
 {
@@ -285,7 +292,7 @@ __device__ __forceinline__ double shfl_xor_double(double v, int o)
 // `seg` takes the tiles seg, seg + nseg, ... of both lists; the partial sums go to A.part and are
 // added in segment order by k_force_final (bit-reproducible), the row cursors are global.
 template <bool SPLIT, bool MONO>
-__device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te, int seg, int nseg)
+__device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int te, int seg, int nseg, bool emit, bool kick)
 {
     const int lane = threadIdx.x & 31;
     const int c = te - tb;
@@ -305,7 +312,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     const long long rowbase = v ? A.nboff[orig] : 0;
     int* rowcnt = SPLIT ? A.nbcnt + (v ? T.id : tb) : &S.nbrow[T.slot];
     if (!SPLIT) S.nbrow[lane] = 0;
-    const uint4 rec = A.glist[g];
+    const uint4 rec = __ldcg(&A.glist[g]);
     __syncwarp();
     // ---- a8: particle-cell list; a lane sees TILE / k cells per tile: fold every k tiles ----
     {
@@ -342,7 +349,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
                 const int b = it & 1;
                 if (more) r = gather_pp(A, idn);
                 idn = load_id(ids, (t + 2 * nseg) * TILE + lane, n);
-                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, rowcnt, A);
+                eval_pp(T, S.pp[b], S.ppj[b], part, k, rowbase, rowcnt, A, emit);
                 if (((it + 1) & (2 * k - 1)) == 0) fold(T);
                 if (more) store_pp(S.pp[b ^ 1], S.ppj[b ^ 1], lane, r);
                 __syncwarp();
@@ -364,18 +371,19 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     // ---- a11: results to the caller's order ----
     const float4 a = make_float4((float)T.dax, (float)T.day, (float)T.daz, (float)T.dph);
     A.out[orig] = a;
-    if (A.vel) {                                // eq. 12: xdot += (dt_reg / 2) F_R, one fma per component
+    if (A.vel && kick) {                        // eq. 12: xdot += (dt_reg / 2) F_R, one fma per component
         float4 u = A.vel[orig];
         u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
         A.vel[orig] = u;
     }
 }
 
-// SPLIT epilogue (a11): the segments of every particle in segment order, then the kick
-__global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
+// SPLIT epilogue (a11): the segments of every particle in segment order, then the kick.  In the host's repair pass
+// (A.mode 1) the sums are written again for everybody (same values) but only the particles of redone groups are kicked.
+__global__ void __launch_bounds__(256) k_force_final(force_args A, int n, const int32_t* __restrict__ rank)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    if (i >= n || (A.info->bad_input | A.info->node_overflow)) return;
     double s[4] = { 0, 0, 0, 0 };
     for (int g = 0; g < A.nseg; ++g) {
         const double* q = A.part + ((size_t)g * n + i) * 4;
@@ -383,10 +391,41 @@ __global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
     }
     const float4 a = make_float4((float)s[0], (float)s[1], (float)s[2], (float)s[3]);
     A.out[i] = a;
-    if (A.vel) {
+    bool kick = A.vel != nullptr;
+    if (kick && A.mode == 1) {                                  // the group of particle i: last g with gbegin[g] <= rank[i]
+        const int sp = rank[i];
+        int lo = 0, hi = A.info->n_groups;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (A.gbegin[mid] <= sp) lo = mid; else hi = mid; }
+        kick = A.gready[lo] == A.base + G_REDONE;
+    }
+    if (kick) {
         float4 u = A.vel[i];
         u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);
         A.vel[i] = u;
+    }
+}
+
+// State of group g's lists for the item a warp has drawn.  The list walk (k_walk<WALK_LISTS>) runs at the same time on
+// the SM share the host left to it and publishes every group with a release; lane 0 waits here with an acquire.
+// Returns base + G_READY / G_FAILED / G_REDONE.  A wait that lasts longer than any walk can (no walker is resident:
+// another process holds the SMs) gives the group up -- it is marked failed, spin_abort makes every other waiting warp
+// give up at once, and the host's repair pass redoes those groups -- so the kernel always terminates.
+#define SPIN_TIMEOUT (1ll << 27)                 // SM cycles (~70 ms)
+__device__ __forceinline__ int group_state(const force_args& A, int g)
+{
+    int v = ld_acquire_gpu(&A.gready[g]);
+    if (A.mode == 1 || g_decided(v, A.base)) return v;
+    const long long t0 = clock64();
+    for (;;) {
+        __nanosleep(200);
+        v = ld_acquire_gpu(&A.gready[g]);
+        if (g_decided(v, A.base)) return v;
+        if (*(volatile int32_t*)&A.info->spin_abort || clock64() - t0 > SPIN_TIMEOUT) {
+            *(volatile int32_t*)&A.info->spin_abort = 1;
+            const int old = atomicCAS(&A.gready[g], v, A.base + G_FAILED);
+            if (old == v) return A.base + G_FAILED;
+            if (g_decided(old, A.base)) return old;            // the walker published in between
+        }
     }
 }
 
@@ -394,13 +433,19 @@ __global__ void __launch_bounds__(256) k_force_final(force_args A, int n)
 // (25 .. 31 left-over targets stay together), which run with k = 1, 1, 2 and 2 / 4 / 8 lanes per target: every chunk but the last fills its
 // warp, and a chunk costs list length / k.  Persistent grid, dynamic
 // scheduling; the chunks are handed out in four passes, k = 1 first and k = 8 last, so that the
-// kernel ends on its cheapest items and the warps finish together.
+// kernel ends on its cheapest items and the warps finish together.  The kernel is launched twice per call on the
+// same cursor: on the SMs' share that the list walk leaves free, and again (behind the walk, in its stream) on the rest.
 template <bool SPLIT, bool MONO>
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(force_args A)
 {
     __shared__ tile_smem smem[FORCE_WARPS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     tile_smem& S = smem[w];
+    // an invalid build or a failed count walk (its offsets size the rows): nothing is written, the host reports it
+    if (A.info->bad_input | A.info->node_overflow | A.info->stack_overflow) return;
+    // the neighbour total is final (the offset scan precedes this kernel): rows are emitted only if they fit
+    const bool emit = (long long)A.info->nb_total <= A.nb_cap;
+    if (!emit && threadIdx.x == 0) A.info->nb_overflow = 1;
     const int ng = A.info->shard_g1 - A.info->shard_g0;          // all groups unless the context is sharded (p3t_shard.cu)
     // cursor ranges of the passes: [0, 2 ng) chunks 0-1 (k = 1), [2 ng, 3 ng) chunk 2 (k = 2), [3 ng, 4 ng) chunk 3 (the rest)
     for (;;) {
@@ -422,7 +467,12 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_CTAS_PER_SM) k_force(forc
         else if (j == 2) { tb = 32 * full;             len = r >= 25 ? r : (r & 16); }      // 25..31 left over: one k = 1 item costs the same as 16 + rest
         else             { tb = 32 * full + (r & 16);  len = r >= 25 ? 0 : (r & 15); }
         if (len == 0) continue;
-        force_item<SPLIT, MONO>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1);
+        int st = 0;
+        if (lane == 0) st = group_state(A, g) - A.base;
+        st = __shfl_sync(0xffffffffu, st, 0);
+        const bool run = A.mode == 0 ? st == G_READY : (st == G_REDONE || (A.evalall && st == G_READY));
+        if (!run) continue;
+        force_item<SPLIT, MONO>(A, S, g, gb + tb, gb + tb + len, seg, SPLIT ? A.nseg : 1, emit, A.mode == 0 || st == G_REDONE);
         __syncwarp();
     }
 }
@@ -506,10 +556,11 @@ __global__ void __launch_bounds__(256) k_nb_offsets(const int32_t* __restrict__ 
 // LONG = false: no row is longer than 32 (the host knows the longest row): no shared memory, full occupancy.
 template <bool LONG>
 __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long long* __restrict__ off, const int32_t* __restrict__ raw,
-                                                                  int32_t* __restrict__ idx, int n)
+                                                                  int32_t* __restrict__ idx, int n, long long cap, const p3t_devinfo* info)
 {
     __shared__ int32_t s_row[LONG ? SORTROWS_THREADS / 32 : 1][LONG ? SORT_SMEM : 1];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    if ((long long)info->nb_total > cap || (info->bad_input | info->node_overflow | info->stack_overflow)) return;   // nothing was emitted
     int32_t* s = s_row[LONG ? threadIdx.x >> 5 : 0];
     long long b = 0; int len = 0;
     if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
@@ -553,100 +604,246 @@ __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long lon
 }
 
 
-int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
-                     float r_list, float half_dt, float4* vel)
+// ---------------------------------------------------------------------------------------------
+// Host side of a7-a11.  One call = p3t_force_begin (everything enqueued, no host synchronisation) + p3t_force_finish
+// (the call's one synchronisation, error report, repair of what an undersized buffer left out).
+//
+//   main stream:  reset | count walk, offset scan (a10) | k_force on (4 - w) CTAs per SM ............ | final, row sort
+//   walk stream:        | k_walk<LISTS> on w CTAs per SM (a7) ........ | k_force again on those w CTAs |
+//
+// The force kernel is FP32-pipe-bound with issue slots to spare, the list walk is issue- and latency-bound with the
+// FP32 pipe nearly idle: side by side on every SM the walk disappears behind the evaluation.  The force kernel draws
+// groups in the order the walkers produce them and waits for a group's state word (group_state).
+// Buffers whose size depends on the result (list pools, neighbour indices) are sized from the previous call with
+// head-room; a call that outgrows them marks what it could not do (G_FAILED groups, nb_overflow) and p3t_force_finish
+// redoes exactly that with larger buffers (normally only on the first call of a context).
+// ---------------------------------------------------------------------------------------------
+#include <atomic>
+static std::atomic<int> g_overlap_owner[64];      // per device: one overlapped call at a time in this process (two force
+                                                  // kernels waiting for two walks could fill the SMs and starve both walks)
+
+static int force_streams(p3t_ctx* ctx)
 {
-    const int n = (int)ctx->n;
-    if (!ctx->occ_force) {
-        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ_force, k_force<false, false>, FORCE_THREADS, 0));
-        if (ctx->occ_force < 1) ctx->occ_force = 1;
-    }
-    const int per_sm = ctx->occ_force;
-    int rc;
-    const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
-    if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;
-    if ((rc = p3t_reserve(ctx, &ctx->nboff, ((size_t)n + 1) * 8))) return rc;
-    if ((rc = p3t_reserve(ctx, &ctx->nbcur, (size_t)nsb * 8 + 64))) return rc;
+    if (ctx->walk_stream) return P3T_OK;
+    P3T_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->walk_stream, cudaStreamNonBlocking));
+    P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_tree, cudaEventDisableTiming));
+    P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_scan, cudaEventDisableTiming));
+    P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_wdone, cudaEventDisableTiming));
+    return P3T_OK;
+}
 
-    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ctx->stream));
-    if (ctx->shard_nranks > 1) {
-        // a sharded context walks only its own groups: rows and list lengths of the others are empty
-        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcount.p, 0, (size_t)n * 4, ctx->stream));
-        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpp.p, 0, ((size_t)n + 1) * 4, ctx->stream));
-        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpc.p, 0, ((size_t)n + 1) * 4, ctx->stream));
-    }
-    // a10, sizes: neighbour counts (range search only) -> CSR offsets, so that the lists can be written in place
-    if ((rc = p3t_launch_walk_count(ctx, r_list, theta))) return rc;
-    k_nb_blocksum<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), INFO(ctx));
-    k_nb_scansums<<<1, 1024, 0, ctx->stream>>>(P<long long>(ctx->nbcur), nsb, P<long long>(ctx->nboff) + n, INFO(ctx));
-    k_nb_offsets<<<nsb, 256, 0, ctx->stream>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), P<long long>(ctx->nboff));
-    P3T_CUDA(ctx, cudaGetLastError());
-    ctx->launches += 3;
-    // a7: interaction lists
-    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
-    if ((rc = p3t_launch_walk_lists(ctx, r_list, theta))) return rc;
-    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
-    // the one host synchronisation of this call: the neighbour total sizes the list buffers, and the
-    // walk reports whether its list pools were large enough (if not it is repeated, normally only on
-    // the first call of a context)
-    p3t_devinfo h;
-    for (int attempt = 0;; ++attempt) {
-        P3T_CUDA(ctx, cudaMemcpyAsync(&h, ctx->info.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
-        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        if (!h.pool_overflow) break;
-        if (attempt >= 4) { snprintf(ctx->err, sizeof(ctx->err), "interaction-list pools still too small after %d attempts", attempt); return P3T_ECUDA; }
-        ctx->pool_cap_pc = (((long long)h.need_pc + h.need_pc / 4 + 16384) + 31) & ~31ll;
-        ctx->pool_cap_pp = (((long long)h.need_pp + h.need_pp / 4 + 16384) + 31) & ~31ll;
-        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
-        if ((rc = p3t_launch_walk_lists(ctx, r_list, theta))) return rc;
-        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
-    }
-    const long long total = (long long)h.nb_total;
-    ctx->nb_total_host = total;
-    if ((rc = p3t_reserve(ctx, &ctx->nbidx, (size_t)total * 4 + 64))) return rc;
-    p3t_buf* raw = &ctx->stage_out;      // unsorted rows share the host-staging scratch
-    if ((rc = p3t_reserve(ctx, raw, (size_t)total * 4 + 64))) return rc;
-
-    force_args A;
+static void force_fill(p3t_ctx* ctx, force_args& A, int mode, int evalall)
+{
+    const p3t_pending& q = ctx->pend;
     A.spm = P<float4>(ctx->spm); A.order = P<uint32_t>(ctx->idx[0]);
     A.ncom = P<float4>(ctx->ncom); A.nq0 = P<float4>(ctx->nq0); A.nq1 = P<float2>(ctx->nq1);
     A.gbegin = P<int32_t>(ctx->gbegin); A.glist = P<uint4>(ctx->glist);
     A.pcpool = P<int32_t>(ctx->pcpool); A.pppool = P<int32_t>(ctx->pppool);
-    A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(*raw);
-    A.out = acc_pot; A.info = INFO(ctx);
-    make_consts(A.K, r_out, r_in, theta, pot_mode, r_list);
-    A.vel = vel; A.half_dt = half_dt; A.mp_order = ctx->order;
-    // a8, a9, a11: the force kernel.  A problem with fewer work items (about 1.4 per 32 particles) than
-    // three per resident warp shares every item among nseg warps (SPLIT), so that small N still fills the GPU.
-    const long long warps = (long long)per_sm * ctx->num_sms * FORCE_WARPS;
-    const long long items = (long long)n / ctx->shard_nranks * 14 / 320 + 1;
+    A.nboff = P<int64_t>(ctx->nboff); A.nbraw = P<int32_t>(ctx->stage_out);      // unsorted rows
+    A.out = q.acc_pot; A.info = INFO(ctx);
+    make_consts(A.K, q.r_out, q.r_in, q.theta, q.pot_mode, q.r_list);
+    A.vel = q.vel; A.half_dt = q.half_dt; A.mp_order = ctx->order;
+    A.gready = P<int32_t>(ctx->gready); A.base = ctx->epoch; A.mode = mode; A.evalall = evalall; A.nb_cap = ctx->nb_cap;
+    A.n = (int)ctx->n; A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
+    // A problem with fewer work items (about 1.4 per 32 particles) than three per resident warp shares every item
+    // among nseg warps (SPLIT), so that small N still fills the GPU.
+    const long long warps = (long long)ctx->occ_force * ctx->num_sms * FORCE_WARPS;
+    const long long items = (long long)ctx->n / ctx->shard_nranks * 14 / 320 + 1;
     int nseg = 1;
     while (nseg < 8 && items * nseg < 3 * warps) nseg *= 2;
-    A.nseg = nseg; A.n = n; A.nbcnt = nullptr; A.part = nullptr;
-    const bool mono = ctx->order < 2;
-    if (nseg > 1) {
-        if ((rc = p3t_reserve(ctx, &ctx->nbcnt, (size_t)n * 4))) return rc;
-        if ((rc = p3t_reserve(ctx, &ctx->part, (size_t)nseg * n * 32))) return rc;
-        A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
-        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcnt.p, 0, (size_t)n * 4, ctx->stream));
-        P3T_CUDA(ctx, cudaMemsetAsync(ctx->part.p, 0, (size_t)nseg * n * 32, ctx->stream));   // a segment beyond a short list writes nothing
-    }
-    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
-    if (nseg > 1) {
-        if (mono) k_force<true, true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
-        else      k_force<true, false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
-        k_force_final<<<(n + 255) / 256, 256, 0, ctx->stream>>>(A, n);
-        ctx->launches += 1;
+    A.nseg = nseg;
+}
+
+static void force_launch(const force_args& A, bool mono, int blocks, cudaStream_t st)
+{
+    if (A.nseg > 1) {
+        if (mono) k_force<true, true><<<blocks, FORCE_THREADS, 0, st>>>(A);
+        else      k_force<true, false><<<blocks, FORCE_THREADS, 0, st>>>(A);
     } else {
-        if (mono) k_force<false, true><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
-        else      k_force<false, false><<<per_sm * ctx->num_sms, FORCE_THREADS, 0, ctx->stream>>>(A);
+        if (mono) k_force<false, true><<<blocks, FORCE_THREADS, 0, st>>>(A);
+        else      k_force<false, false><<<blocks, FORCE_THREADS, 0, st>>>(A);
+    }
+}
+
+// what follows the force kernel on the main stream: SPLIT epilogue, octupole variant, row sort
+static int force_tail(p3t_ctx* ctx, const force_args& A, int mode, int evalall)
+{
+    const int n = (int)ctx->n;
+    int rc;
+    if (A.nseg > 1) {
+        k_force_final<<<(n + 255) / 256, 256, 0, ctx->stream>>>(A, n, P<int32_t>(ctx->rank));
+        ctx->launches += 1;
     }
     P3T_CUDA(ctx, cudaEventRecord(ctx->evw[1], ctx->stream));
-    if (ctx->order == 3 && (rc = p3t_launch_octupole_add(ctx, acc_pot, half_dt, vel))) return rc;   // octupole variant: third-order term of the accepted cells
-    if (h.nb_max > 32) k_nb_sortrows<true><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
-    else               k_nb_sortrows<false><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n);
+    if (ctx->order == 3 && (rc = p3t_launch_octupole_add(ctx, ctx->pend.acc_pot, ctx->pend.half_dt, ctx->pend.vel, ctx->epoch, mode, evalall))) return rc;
+    // rows ascending (any variant sorts every row correctly; the hint only picks the faster one)
+    if (ctx->nb_max_hint > 32) k_nb_sortrows<true><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n, A.nb_cap, INFO(ctx));
+    else                       k_nb_sortrows<false><<<(n + SORTROWS_THREADS - 1) / SORTROWS_THREADS, SORTROWS_THREADS, 0, ctx->stream>>>(P<long long>(ctx->nboff), A.nbraw, P<int32_t>(ctx->nbidx), n, A.nb_cap, INFO(ctx));
     P3T_CUDA(ctx, cudaGetLastError());
     P3T_CUDA(ctx, cudaEventRecord(ctx->ev[5], ctx->stream));
-    ctx->launches += 2;
+    ctx->launches += 1;
+    return P3T_OK;
+}
+
+static int reserve_split(p3t_ctx* ctx, const force_args& A)
+{
+    if (A.nseg <= 1) return P3T_OK;
+    int rc;
+    if ((rc = p3t_reserve(ctx, &ctx->nbcnt, (size_t)ctx->n * 4))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->part, (size_t)A.nseg * ctx->n * 32))) return rc;
+    return P3T_OK;
+}
+
+int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
+                    float r_list, float half_dt, float4* vel)
+{
+    const int n = (int)ctx->n;
+    int rc;
+    if (!ctx->occ_force) {
+        P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ_force, k_force<false, false>, FORCE_THREADS, 0));
+        if (ctx->occ_force < 1) ctx->occ_force = 1;
+    }
+    if ((rc = force_streams(ctx))) return rc;
+    p3t_pending& q = ctx->pend;
+    q.r_out = r_out; q.r_in = r_in; q.theta = theta; q.r_list = r_list; q.half_dt = half_dt; q.pot_mode = pot_mode;
+    q.acc_pot = acc_pot; q.vel = vel; q.active = 1; q.repaired = 0;
+    // ---- every buffer before anything is enqueued (a reallocation synchronises the stream) ----
+    const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
+    if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->nboff, ((size_t)n + 1) * 8))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->nbcur, (size_t)nsb * 8 + 64))) return rc;
+    if (ctx->gready.bytes < ((size_t)n + 2) * 4 || ctx->epoch > 0x3fffff00) {
+        if ((rc = p3t_reserve(ctx, &ctx->gready, ((size_t)n + 2) * 4))) return rc;
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gready.p, 0, ctx->gready.bytes, ctx->stream));
+        ctx->epoch = 0;
+    }
+    ctx->epoch += 4;
+    if (ctx->nb_cap == 0) ctx->nb_cap = 4ll * n > (1ll << 20) ? 4ll * n : (1ll << 20);      // first call: a guess (mean row of 4)
+    if (ctx->nb_total_host + ctx->nb_total_host / 4 + 4096 > ctx->nb_cap) ctx->nb_cap = ctx->nb_total_host + ctx->nb_total_host / 4 + 4096;
+    if ((rc = p3t_reserve(ctx, &ctx->nbidx, (size_t)ctx->nb_cap * 4 + 64))) return rc;
+    if ((rc = p3t_reserve(ctx, &ctx->stage_out, (size_t)ctx->nb_cap * 4 + 64))) return rc;
+    // overlapped unless switched off, or another context of this process is in the middle of an overlapped call
+    int overlapped = ctx->overlap && ctx->occ_force >= 2;
+    if (overlapped) {
+        int expect = 0;
+        overlapped = g_overlap_owner[ctx->device & 63].compare_exchange_strong(expect, 1) ? 1 : 0;
+    }
+    q.overlapped = overlapped;
+    int wsm = overlapped ? ctx->walk_ctas_per_sm : 0;
+    if (wsm >= ctx->occ_force) wsm = ctx->occ_force - 1;
+    if ((rc = p3t_walk_reserve(ctx, wsm))) return rc;
+    force_args A;
+    force_fill(ctx, A, 0, 0);
+    if ((rc = reserve_split(ctx, A))) return rc;
+    A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
+    const bool mono = ctx->order < 2;
+    cudaStream_t ms = ctx->stream, ws = overlapped ? ctx->walk_stream : ctx->stream;
+
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev[4], ms));
+    if (ctx->shard_nranks > 1) {
+        // a sharded context walks only its own groups: rows and list lengths of the others are empty
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcount.p, 0, (size_t)n * 4, ms));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpp.p, 0, ((size_t)n + 1) * 4, ms));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->gnpc.p, 0, ((size_t)n + 1) * 4, ms));
+    }
+    if (A.nseg > 1) {
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->nbcnt.p, 0, (size_t)n * 4, ms));
+        P3T_CUDA(ctx, cudaMemsetAsync(ctx->part.p, 0, (size_t)A.nseg * n * 32, ms));   // a segment beyond a short list writes nothing
+    }
+    if ((rc = p3t_launch_walk_reset(ctx, ms))) return rc;
+    if (ctx->test_fault & 1) P3T_CUDA(ctx, cudaMemsetAsync((char*)ctx->info.p + offsetof(p3t_devinfo, spin_abort), 1, 1, ms));
+    // a7 on the walk stream, from now on
+    if (overlapped) {
+        P3T_CUDA(ctx, cudaEventRecord(ctx->ev_tree, ms));
+        P3T_CUDA(ctx, cudaStreamWaitEvent(ws, ctx->ev_tree, 0));
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ws));
+        if ((rc = p3t_launch_walk_lists(ctx, r_list, theta, ws, ctx->epoch, 0, wsm))) return rc;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ws));
+    }
+    // a10, sizes: neighbour counts (range search only) -> CSR offsets, so that the lists can be written in place
+    if ((rc = p3t_launch_walk_count(ctx, r_list, theta, ms))) return rc;
+    k_nb_blocksum<<<nsb, 256, 0, ms>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), INFO(ctx));
+    k_nb_scansums<<<1, 1024, 0, ms>>>(P<long long>(ctx->nbcur), nsb, P<long long>(ctx->nboff) + n, INFO(ctx));
+    k_nb_offsets<<<nsb, 256, 0, ms>>>(P<int32_t>(ctx->nbcount), n, P<long long>(ctx->nbcur), P<long long>(ctx->nboff));
+    P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 3;
+    P3T_CUDA(ctx, cudaEventRecord(ctx->ev_scan, ms));
+    if (!overlapped) {
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ms));
+        if ((rc = p3t_launch_walk_lists(ctx, r_list, theta, ms, ctx->epoch, 0, 0))) return rc;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ms));
+    }
+    // a8, a9, a11: the force kernel, on the SMs' share the walk leaves free; again behind the walk on the rest
+    P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ms));
+    force_launch(A, mono, (ctx->occ_force - wsm) * ctx->num_sms, ms);
+    ctx->launches += 1;
+    if (overlapped) {
+        P3T_CUDA(ctx, cudaStreamWaitEvent(ws, ctx->ev_scan, 0));
+        force_launch(A, mono, wsm * ctx->num_sms, ws);
+        ctx->launches += 1;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->ev_wdone, ws));
+        P3T_CUDA(ctx, cudaStreamWaitEvent(ms, ctx->ev_wdone, 0));
+    }
+    P3T_CUDA(ctx, cudaGetLastError());
+    return force_tail(ctx, A, 0, 0);
+}
+
+int p3t_force_finish(p3t_ctx* ctx)
+{
+    p3t_pending& q = ctx->pend;
+    if (!q.active) return P3T_OK;
+    q.active = 0;
+    p3t_devinfo h;
+    cudaError_t e = cudaMemcpyAsync(&h, ctx->info.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (q.overlapped) { g_overlap_owner[ctx->device & 63].store(0); q.overlapped = 0; }
+    if (e != cudaSuccess) return p3t_fail_cuda(ctx, e, "force call", __LINE__);
+    int rc;
+    for (int attempt = 0;; ++attempt) {
+        if (h.bad_input) return P3T_EINVAL;
+        if (h.node_overflow || h.stack_overflow) {
+            snprintf(ctx->err, sizeof(ctx->err), "internal capacity exceeded (node_overflow=%d stack_overflow=%d)", h.node_overflow, h.stack_overflow);
+            return P3T_ECUDA;
+        }
+        ctx->nb_total_host = (long long)h.nb_total;
+        ctx->nb_max_hint = h.nb_max;
+        if (!h.pool_overflow && !h.nb_overflow && !h.spin_abort) break;
+        if (attempt >= 4) { snprintf(ctx->err, sizeof(ctx->err), "list buffers still too small after %d repair passes", attempt); return P3T_ECUDA; }
+        // ---- repair pass (stream order, no overlap): larger buffers, every list again, then only what is missing ----
+        q.repaired = 1;
+        const int evalall = h.nb_overflow ? 1 : 0;
+        if (h.pool_overflow) {
+            ctx->pool_cap_pc = (((long long)h.need_pc + h.need_pc / 4 + 16384) + 31) & ~31ll;
+            ctx->pool_cap_pp = (((long long)h.need_pp + h.need_pp / 4 + 16384) + 31) & ~31ll;
+        }
+        if (h.nb_overflow) {
+            ctx->nb_cap = ctx->nb_total_host + ctx->nb_total_host / 4 + 4096;
+            if ((rc = p3t_reserve(ctx, &ctx->nbidx, (size_t)ctx->nb_cap * 4 + 64))) return rc;
+            if ((rc = p3t_reserve(ctx, &ctx->stage_out, (size_t)ctx->nb_cap * 4 + 64))) return rc;
+        }
+        const int wsm = ctx->overlap && ctx->occ_force >= 2 ? (ctx->walk_ctas_per_sm >= ctx->occ_force ? ctx->occ_force - 1 : ctx->walk_ctas_per_sm) : 0;
+        if ((rc = p3t_launch_walk_reset(ctx, ctx->stream))) return rc;       // cursors and counters; nb_total / nb_max are restored below
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[2], ctx->stream));
+        if ((rc = p3t_launch_walk_lists(ctx, q.r_list, q.theta, ctx->stream, ctx->epoch, 1, wsm))) return rc;
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[3], ctx->stream));
+        p3t_devinfo h2;
+        P3T_CUDA(ctx, cudaMemcpyAsync(&h2, ctx->info.p, sizeof(h2), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        h2.nb_total = h.nb_total; h2.nb_max = h.nb_max;
+        P3T_CUDA(ctx, cudaMemcpyAsync((char*)ctx->info.p + offsetof(p3t_devinfo, nb_total), &h.nb_total, sizeof(h.nb_total), cudaMemcpyHostToDevice, ctx->stream));
+        P3T_CUDA(ctx, cudaMemcpyAsync((char*)ctx->info.p + offsetof(p3t_devinfo, nb_max), &h.nb_max, sizeof(h.nb_max), cudaMemcpyHostToDevice, ctx->stream));
+        if (h2.pool_overflow || h2.stack_overflow) { h2.nb_overflow = h.nb_overflow; h = h2; continue; }     // still too small: measured again
+        force_args A;
+        force_fill(ctx, A, 1, evalall);
+        if ((rc = reserve_split(ctx, A))) return rc;
+        A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
+        P3T_CUDA(ctx, cudaEventRecord(ctx->evw[0], ctx->stream));
+        force_launch(A, ctx->order < 2, ctx->occ_force * ctx->num_sms, ctx->stream);
+        ctx->launches += 1;
+        P3T_CUDA(ctx, cudaGetLastError());
+        if ((rc = force_tail(ctx, A, 1, evalall))) return rc;
+        P3T_CUDA(ctx, cudaMemcpyAsync(&h, ctx->info.p, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        P3T_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
     return P3T_OK;
 }

@@ -9,7 +9,8 @@
 #define P3T_RADIX_BITS 8
 #define P3T_RADIX      256
 #define P3T_SORT_THREADS 256
-#define P3T_SORT_ITEMS_MIN 4                                 // keys per thread in one sort tile: 4 (n <= 2^18) or 8
+#define P3T_SORT_ITEMS_MIN 4                                 // keys per thread in one sort tile: 4 (n <= 2^18) or P3T_SORT_ITEMS_BIG
+#define P3T_SORT_ITEMS_BIG 16
 #define P3T_SORT_TILE_MIN  (P3T_SORT_THREADS * P3T_SORT_ITEMS_MIN) // the smallest tile sizes the histogram buffer
 
 // device-side counters written by the build and force kernels (one 256-byte record)
@@ -35,6 +36,22 @@ struct p3t_devinfo {
     uint32_t need_pc, need_pp; // largest per-warp list space used, in entries
     uint32_t minmax[6];      // order-preserving uint encodings of min xyz / max xyz
     int32_t  shard_g0, shard_g1; // target groups of this context's shard (all groups unless p3t_set_shard)
+    int32_t  nb_overflow;    // the neighbour total exceeds the capacity of the index buffers: nothing was emitted (repaired by the host)
+    int32_t  spin_abort;     // a force warp waited too long for a group's lists (no co-resident walker): those groups are repaired
+};
+
+// State of a target group's interaction lists in p3t_ctx::gready, relative to the call's epoch `base` (values of older
+// calls are smaller, so the array is never cleared): base + 1 = lists published by a walker warp, base + 2 = no lists
+// (pool or stack overflow, or a force warp gave up waiting), base + 3 = lists rebuilt by the host's repair pass.
+#define G_READY  1
+#define G_FAILED 2
+#define G_REDONE 3
+
+// arguments of the force call in flight (p3t_force_begin .. p3t_force_finish)
+struct p3t_pending {
+    float r_out, r_in, theta, r_list, half_dt;
+    int pot_mode, active, overlapped, repaired;
+    float4 *acc_pot, *vel;
 };
 
 struct p3t_buf { void* p; size_t bytes; };
@@ -99,6 +116,17 @@ struct p3t_ctx {
     p3t_buf shard_cuts;              // int32[2][nranks+1]: group-aligned cuts as group index / sorted position
     int shard_has_nominal;
     int64_t launches;                // kernels launched so far
+    // walk / force overlap (p3t_force.cu): per-group list state, the epoch of the current call, the walker stream
+    p3t_buf gready;                  // int32 per group (see G_READY)
+    int32_t epoch;
+    cudaStream_t walk_stream;        // created on first use (non-blocking)
+    cudaEvent_t ev_tree, ev_scan, ev_wdone;
+    int overlap;                     // 1 (default): walkers and force kernel run concurrently; 0: one after the other (P3T_OVERLAP=0)
+    int walk_ctas_per_sm;            // CTAs per SM given to the list walk while the force kernel runs (P3T_WALK_CTAS, default 1)
+    int64_t nb_cap;                  // capacity of nbidx / the raw row buffer in entries (grow-only, from the previous call's total)
+    int nb_max_hint;                 // longest row of the previous call (chooses the row-sort variant; any value is correct)
+    p3t_pending pend;
+    int test_fault;                  // P3T_TEST_FAULT (tests only): 1 = the force kernel gives up waiting at once, 2 = no walk-stack spill
 };
 
 #define P3T_CUDA(ctx, call)                                                              \
@@ -114,6 +142,7 @@ template <typename T> static inline T* P(p3t_buf& b) { return (T*)b.p; }
 static inline p3t_devinfo* INFO(p3t_ctx* c) { return (p3t_devinfo*)c->info.p; }
 
 // p3t_sort.cu : a1-a3
+size_t p3t_sort_scratch_bytes(int64_t n);                            // ctx->hist: digit totals, tickets, look-back words
 int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pos_mass);
 int p3t_launch_sort(p3t_ctx* ctx);
 int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
@@ -122,17 +151,35 @@ int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
 // p3t_octupole.cu : SURVEY 8f NEXT-4, octupole variant
 int p3t_launch_octupoles(p3t_ctx* ctx);
-int p3t_launch_octupole_add(p3t_ctx* ctx, float4* acc_pot, float half_dt, float4* vel);
+int p3t_launch_octupole_add(p3t_ctx* ctx, float4* acc_pot, float half_dt, float4* vel, int base, int mode, int evalall);
 // p3t_shard.cu : SURVEY 8e, target groups split among the ranks of a node
 int p3t_launch_shard_range(p3t_ctx* ctx);
 // p3t_walk.cu : a7 (interaction lists), a10 (neighbour counts)
 int p3t_walk_init(p3t_ctx* ctx);
-int p3t_launch_walk_count(p3t_ctx* ctx, float r_list, float theta);   // r_list: neighbour search radius (>= r_out)
-int p3t_launch_walk_lists(p3t_ctx* ctx, float r_list, float theta);
+int p3t_launch_walk_reset(p3t_ctx* ctx, cudaStream_t st);
+int p3t_walk_reserve(p3t_ctx* ctx, int ctas_per_sm);                 // spill + list pools for a walk with this share of the device
+int p3t_launch_walk_count(p3t_ctx* ctx, float r_list, float theta, cudaStream_t st);   // r_list: neighbour search radius (>= r_out)
+// base: epoch of the call (gready); repair: host repair pass (every group again, failed ones become G_REDONE);
+// ctas_per_sm: 0 = the whole device, else the share left to the walk while the force kernel runs
+int p3t_launch_walk_lists(p3t_ctx* ctx, float r_list, float theta, cudaStream_t st, int base, int repair, int ctas_per_sm);
 // p3t_core.cu : SURVEY 8f NEXT-3
 int p3t_launch_core(p3t_ctx* ctx, int64_t ns, const int32_t* sample, int K, int32_t* nbr, float* d2k, double* rho, double* core_dev);
 // p3t_irregular.cu : SURVEY 8f NEXT-1
 int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* jerk);
 // p3t_force.cu : a8-a11
-int p3t_launch_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
-                     float r_list, float half_dt, float4* vel);
+// p3t_force_begin enqueues the whole call (count walk, offsets, list walk and force kernel, row sort) without a host
+// synchronisation; p3t_force_finish synchronises once, reports errors and repairs what an undersized buffer left out.
+int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
+                    float r_list, float half_dt, float4* vel);
+int p3t_force_finish(p3t_ctx* ctx);
+
+// group-state helpers shared by the walk, force and octupole kernels
+__device__ __forceinline__ int ld_acquire_gpu(const int32_t* p)
+{
+    int v; asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ int cas_release_gpu(int32_t* p, int cmp, int val)
+{
+    int old; asm volatile("atom.release.gpu.global.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "l"(p), "r"(cmp), "r"(val) : "memory"); return old;
+}
+__device__ __forceinline__ bool g_decided(int v, int base) { return v >= base + G_READY && v <= base + G_REDONE; }

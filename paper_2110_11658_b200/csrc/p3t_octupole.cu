@@ -125,18 +125,24 @@ struct octadd_args {
     const int32_t* gbegin; const uint4* glist; const int32_t* pcpool;
     float4 *out, *vel; float half_dt;
     p3t_devinfo* info;
+    const int32_t* gready; int base, mode, evalall;      // the group filter of the force kernel (p3t_force.cu)
 };
 
 __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
 {
     __shared__ float4 s_node[OCT_THREADS / 32][4][32];
     const int lane = threadIdx.x & 31;
+    if (A.info->bad_input | A.info->node_overflow | A.info->stack_overflow) return;
     const int g0 = A.info->shard_g0, ng = A.info->shard_g1 - g0;
     const int nwarps = gridDim.x * (OCT_THREADS / 32);
     for (int c = blockIdx.x * (OCT_THREADS / 32) + (threadIdx.x >> 5); c < 2 * ng; c += nwarps) {
         const int g = g0 + (c >> 1);
         const int gb = A.gbegin[g], cnt = A.gbegin[g + 1] - gb, tb = 32 * (c & 1);
         if (tb >= cnt) continue;
+        // the same groups as the force kernel of this pass (the term is ADDED: never twice to the same group)
+        const int st = A.gready[g] - A.base;
+        if (A.mode == 0 ? st != G_READY : !(st == G_REDONE || (A.evalall && st == G_READY))) continue;
+        const bool kick = A.mode == 0 || st == G_REDONE;
         const int i = gb + tb + lane;
         const bool live = tb + lane < cnt;
         const float4 xi = A.spm[live ? i : gb];
@@ -183,7 +189,7 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
             const float dax = (float)ax, day = (float)ay, daz = (float)az;
             r.x += dax; r.y += day; r.z += daz; r.w += (float)ph;
             A.out[o] = r;
-            if (A.vel) {
+            if (A.vel && kick) {
                 float4 v = A.vel[o];
                 v.x = fmaf(A.half_dt, dax, v.x); v.y = fmaf(A.half_dt, day, v.y); v.z = fmaf(A.half_dt, daz, v.z);
                 A.vel[o] = v;
@@ -192,13 +198,14 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupole_add(octadd_args A)
     }
 }
 
-int p3t_launch_octupole_add(p3t_ctx* ctx, float4* acc_pot, float half_dt, float4* vel)
+int p3t_launch_octupole_add(p3t_ctx* ctx, float4* acc_pot, float half_dt, float4* vel, int base, int mode, int evalall)
 {
     octadd_args A;
     A.spm = P<float4>(ctx->spm); A.order = P<uint32_t>(ctx->idx[0]);
     A.ncom = P<float4>(ctx->ncom); A.noct = P<float4>(ctx->noct);
     A.gbegin = P<int32_t>(ctx->gbegin); A.glist = P<uint4>(ctx->glist); A.pcpool = P<int32_t>(ctx->pcpool);
     A.out = acc_pot; A.vel = vel; A.half_dt = half_dt; A.info = INFO(ctx);
+    A.gready = P<int32_t>(ctx->gready); A.base = base; A.mode = mode; A.evalall = evalall;
     P3T_CUDA(ctx, cudaEventRecord(ctx->evo[0], ctx->stream));
     k_octupole_add<<<ctx->num_sms * 8, OCT_THREADS, 0, ctx->stream>>>(A);
     P3T_CUDA(ctx, cudaGetLastError());

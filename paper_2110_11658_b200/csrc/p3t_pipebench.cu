@@ -3,8 +3,10 @@
 // (the driver's MEASURED_PEAKS.json holds HBM and bf16 tensor peaks, no FP32 figure).
 // Eight independent chains per thread, 2 CTAs of 256 threads per SM, CUDA events; a result is the
 // number of SM-clock cycles one warp instruction (or instruction group) occupies an SM sub-partition.
-// Exposed as p3t_pipe_bench (include/p3t.h); `python -m paper_2110_11658_b200.pipebench` prints the table.
-#include "p3t_internal.cuh"
+// Built into its own library, libp3t_diag.so (include/p3t_diag.h): diagnostics, not part of libp3t.so.
+// `python -m paper_2110_11658_b200.pipebench` prints the table.
+#include <cuda_runtime.h>
+#include "p3t_diag.h"
 #include "p3t_f32x2.cuh"
 
 __device__ __forceinline__ f2 vfma2(f2 a, f2 b, f2 c) { f2 r; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
@@ -54,18 +56,18 @@ template <int MODE> static float time_mode(float* d, int blocks, int iters, cuda
     return ms;
 }
 
-extern "C" int p3t_pipe_bench(int device, double* cycles_out, int n_out, double* sm_clock_mhz, int* num_sms)
+extern "C" int p3t_diag_pipe_bench(int device, double* cycles_out, int n_out, double* sm_clock_mhz, int* num_sms)
 {
-    if (!cycles_out || n_out < 8) return P3T_EINVAL;
+    if (!cycles_out || n_out < 8) return -1;
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { (void)cudaGetLastError(); return P3T_EINVAL; }
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { (void)cudaGetLastError(); return -1; }
     cudaSetDevice(device);
     int sms = 0, khz = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device);
     const int bps = 2, iters = 20000, blocks = sms * bps;
     float* d = nullptr;
-    if (cudaMalloc(&d, (size_t)blocks * 256 * sizeof(float)) != cudaSuccess) { (void)cudaGetLastError(); return P3T_ENOMEM; }
+    if (cudaMalloc(&d, (size_t)blocks * 256 * sizeof(float)) != cudaSuccess) { (void)cudaGetLastError(); return -3; }
     cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
     for (int w = 0; w < 40; ++w) (void)time_mode<3>(d, blocks, iters, e0, e1);     // ~50 ms of load: let the SM clock settle
     float ms[8];
@@ -80,5 +82,5 @@ extern "C" int p3t_pipe_bench(int device, double* cycles_out, int n_out, double*
     if (sm_clock_mhz) *sm_clock_mhz = khz * 1e-3;
     if (num_sms) *num_sms = sms;
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
-    return cudaGetLastError() == cudaSuccess ? P3T_OK : P3T_ECUDA;
+    return cudaGetLastError() == cudaSuccess ? 0 : -4;
 }

@@ -75,9 +75,14 @@ __device__ __forceinline__ uint64_t spread3(uint32_t v)   // bit k of v -> bit 3
     return x;
 }
 
-__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pm, int n, int B,
-                                              p3t_devinfo* info, uint64_t* __restrict__ keys)
+// k_keys also counts, for every radix pass, how many keys carry each digit (one read of the particles serves the
+// keys and all the histograms of the sort below)
+#define SORT_MAX_PASSES 8
+__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pm, int n, int B, int passes,
+                                              p3t_devinfo* info, uint64_t* __restrict__ keys, uint32_t* __restrict__ ghist)
 {
+    __shared__ uint32_t s_hist[SORT_MAX_PASSES][P3T_RADIX];
+    for (int k = 0; k < passes; ++k) s_hist[k][threadIdx.x] = 0;
     float lo[3], ext = 0.0f;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
@@ -92,116 +97,186 @@ __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pm, int
         info->lo[0] = lo[0]; info->lo[1] = lo[1]; info->lo[2] = lo[2];
         info->side = side; info->scale = scale;
     }
+    __syncthreads();
     const uint32_t gmax = (1u << B) - 1u;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         float4 p = __ldg(pm + i);
         uint32_t gx = min(gmax, __float2uint_rz(__fmul_rn(__fsub_rn(p.x, lo[0]), scale)));
         uint32_t gy = min(gmax, __float2uint_rz(__fmul_rn(__fsub_rn(p.y, lo[1]), scale)));
         uint32_t gz = min(gmax, __float2uint_rz(__fmul_rn(__fsub_rn(p.z, lo[2]), scale)));
-        keys[i] = (spread3(gx) << 2) | (spread3(gy) << 1) | spread3(gz);
+        const uint64_t key = (spread3(gx) << 2) | (spread3(gy) << 1) | spread3(gz);
+        keys[i] = key;
+        for (int k = 0; k < passes; ++k) atomicAdd(&s_hist[k][(uint32_t)(key >> (k * P3T_RADIX_BITS)) & 255u], 1u);
+    }
+    __syncthreads();
+    for (int k = 0; k < passes; ++k) {
+        const uint32_t c = s_hist[k][threadIdx.x];
+        if (c) atomicAdd(&ghist[k * P3T_RADIX + threadIdx.x], c);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3  stable LSD radix sort (R-S3), 8-bit digits, three kernels per pass:
-//     k_hist   per-tile digit counts            -> hist[digit][tile]
-//     k_scan   exclusive scan of every digit row, row totals
-//     k_scatter stable ranking inside the tile (warp match + per-warp counters) and scatter
+// a3  stable LSD radix sort (R-S3), 8-bit digits, ONE kernel per pass ("onesweep"): the digit totals of every pass are
+//     known from k_keys, so a tile only needs the number of equal digits in the tiles before it.  Tiles take their
+//     number from a ticket counter (a tile with a smaller number is always already running), rank their keys
+//     (warp match + per-warp counters: stable), publish their 256 digit counts in one 64-bit word each
+//     (flag | count) and look back over the earlier tiles' words until they meet an inclusive prefix
+//     (decoupled look-back), publish their own inclusive prefix, and scatter.
+//     status word: high half = 2 pass + 1 (count of this tile) or 2 pass + 2 (inclusive prefix), low half = value;
+//     words of earlier passes have smaller flags, so the array is cleared once per sort, not per pass.
 // ---------------------------------------------------------------------------------------------
-template <int ITEMS>
-__global__ void __launch_bounds__(P3T_SORT_THREADS) k_hist(const uint64_t* __restrict__ keys, int n, int shift,
-                                                           uint32_t* __restrict__ hist, int ntiles)
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* p)
 {
-    __shared__ uint32_t h[P3T_RADIX];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    const int base = blockIdx.x * (P3T_SORT_THREADS * ITEMS);
-#pragma unroll 4
-    for (int k = 0; k < ITEMS; ++k) {
-        int i = base + k * P3T_SORT_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&h[(uint32_t)(keys[i] >> shift) & 255u], 1u);
-    }
-    __syncthreads();
-    hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = h[threadIdx.x];
+    unsigned long long v; asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v;
 }
-
-// one warp per digit row: in-place exclusive scan over the tiles, total -> totals[digit]
-__global__ void __launch_bounds__(256) k_scan_rows(uint32_t* __restrict__ hist, int ntiles, uint32_t* __restrict__ totals)
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long* p, unsigned long long v)
 {
-    const int d = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    uint32_t* row = hist + (size_t)d * ntiles;
-    uint32_t run = 0;
-    for (int b0 = 0; b0 < ntiles; b0 += 32) {
-        int b = b0 + lane;
-        uint32_t v = b < ntiles ? row[b] : 0u, x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-        if (b < ntiles) row[b] = run + x - v;
-        run += __shfl_sync(0xffffffffu, x, 31);
-    }
-    if (lane == 0) totals[d] = run;
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
 
 template <bool FIRST, int ITEMS>
-__global__ void __launch_bounds__(P3T_SORT_THREADS) k_scatter(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
-                                                              uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
-                                                              int n, int shift, const uint32_t* __restrict__ hist, int ntiles,
-                                                              const uint32_t* __restrict__ totals)
+__global__ void __launch_bounds__(P3T_SORT_THREADS) k_sort_pass(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                                                                uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
+                                                                int n, int pass, const uint32_t* __restrict__ ghist,
+                                                                unsigned long long* status, uint32_t* ticket)
 {
+    constexpr int TILE_KEYS = P3T_SORT_THREADS * ITEMS;
     __shared__ uint32_t cnt[8][P3T_RADIX];
-    __shared__ uint32_t s_scan[P3T_RADIX];
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ uint32_t s_gbase[P3T_RADIX];          // where the tile's keys of digit d begin in the output
+    __shared__ uint32_t s_lbase[P3T_RADIX];          // ... and in the tile's own sorted order
+    __shared__ uint32_t s_wsum[8];
+    __shared__ int s_tile;
+    __shared__ uint64_t s_buf[TILE_KEYS];            // the tile in sorted order: keys, then (same space) values
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31, shift = pass * P3T_RADIX_BITS;
+    if (threadIdx.x == 0) s_tile = (int)atomicAdd(&ticket[pass], 1u);
     for (int k = 0; k < 8; ++k) cnt[k][threadIdx.x] = 0;
-    // digit bases: exclusive scan of the 256 row totals
-    {
-        uint32_t v = totals[threadIdx.x], x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-        s_scan[threadIdx.x] = x;                       // inclusive inside the warp
-        __syncthreads();
-        uint32_t add = 0;
-        for (int k = 0; k < w; ++k) add += s_scan[k * 32 + 31];
-        __syncthreads();
-        s_scan[threadIdx.x] = add + x - v + hist[(size_t)threadIdx.x * ntiles + blockIdx.x];
-    }
+    const uint32_t v_tot = ghist[pass * P3T_RADIX + threadIdx.x];
     __syncthreads();
-    const int base = blockIdx.x * (P3T_SORT_THREADS * ITEMS) + w * (32 * ITEMS);
+    // all the tile's keys are requested before anything waits (the barrier below keeps the loads from sinking into
+    // the ranking rounds, where each round would wait for its own load)
+    const int tile = s_tile;
+    const int base = tile * TILE_KEYS + w * (32 * ITEMS);
     uint64_t key[ITEMS];
-    uint32_t rank[ITEMS];
+    uint16_t rank[ITEMS];
 #pragma unroll
     for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
-        key[r] = i < n ? kin[i] : ~0ull;
+        key[r] = i < n ? __ldcs(kin + i) : ~0ull;
+    }
+    // digit bases: exclusive scan of the 256 digit totals of this pass
+    uint32_t dbase;
+    {
+        uint32_t v = v_tot, x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) s_wsum[w] = x;
+        __syncthreads();
+        uint32_t add = 0;
+        for (int k = 0; k < w; ++k) add += s_wsum[k];
+        dbase = add + x - v;
     }
     const uint32_t lt = (1u << lane) - 1u;
 #pragma unroll
     for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
         uint32_t d = i < n ? ((uint32_t)(key[r] >> shift) & 255u) : 256u;
-        uint32_t peers = __match_any_sync(0xffffffffu, d);
+        // lanes with the same digit: nine ballots, one per bit (match.any costs a round per distinct value in the warp)
+        uint32_t peers = 0xffffffffu;
+#pragma unroll
+        for (int b = 0; b < 9; ++b) {
+            const uint32_t m = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+            peers &= ((d >> b) & 1u) ? m : ~m;
+        }
         int leader = __ffs(peers) - 1;
         uint32_t old = 0;
         if (lane == leader && d < 256u) { old = cnt[w][d]; cnt[w][d] = old + __popc(peers); }
         old = __shfl_sync(0xffffffffu, old, leader);
-        rank[r] = old + __popc(peers & lt);
+        rank[r] = (uint16_t)(old + __popc(peers & lt));
         __syncwarp();
     }
     __syncthreads();
-    {   // per digit: exclusive scan over the 8 warps, plus the tile's global offset
-        uint32_t run = s_scan[threadIdx.x];
+    {   // thread = digit: exclusive scan over the 8 warps, the tile's count, look-back over the earlier tiles
+        uint32_t run = 0;
 #pragma unroll
         for (int k = 0; k < 8; ++k) { uint32_t t = cnt[k][threadIdx.x]; cnt[k][threadIdx.x] = run; run += t; }
+        const unsigned long long f_count = (unsigned long long)(2 * pass + 1) << 32, f_prefix = (unsigned long long)(2 * pass + 2) << 32;
+        unsigned long long* mine = status + (size_t)tile * P3T_RADIX + threadIdx.x;
+        if (tile > 0) st_relaxed_u64(mine, f_count | run);
+        // the tile's own digit starts (exclusive scan of its 256 counts) while the earlier tiles publish
+        uint32_t x = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        __syncthreads();                                  // s_wsum is free again (everybody has its dbase)
+        if (lane == 31) s_wsum[w] = x;
+        __syncthreads();
+        uint32_t ladd = 0;
+        for (int k = 0; k < w; ++k) ladd += s_wsum[k];
+        s_lbase[threadIdx.x] = ladd + x - run;
+        uint32_t excl = 0;
+        if (tile > 0) {
+            // look back over the earlier tiles, eight words in flight at a time (one L2 round trip per batch); a word
+            // that is not there yet ends the batch and is polled again
+            const unsigned long long fmin = (unsigned long long)(2 * pass + 1), fpre = (unsigned long long)(2 * pass + 2);
+            int t = tile - 1;
+            bool done = false;
+            while (!done) {
+                unsigned long long sv[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    sv[j] = t - j >= 0 ? ld_relaxed_u64(status + (size_t)(t - j) * P3T_RADIX + threadIdx.x) : (fpre << 32);
+                int used = 0;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (done || used < j) continue;                         // stopped at an earlier word of this batch
+                    if ((sv[j] >> 32) < fmin) continue;                     // not published yet: poll again from here
+                    excl += (uint32_t)sv[j];
+                    used = j + 1;
+                    if ((sv[j] >> 32) == fpre) done = true;
+                }
+                t -= used;
+            }
+        }
+        st_relaxed_u64(mine, f_prefix | (unsigned long long)(excl + run));
+        s_gbase[threadIdx.x] = dbase + excl;
     }
     __syncthreads();
+    // The tile goes through shared memory in sorted order, so that a digit's run leaves as consecutive addresses
+    // (8 or 16 keys per run on average: full sectors instead of one partial sector per key).
+    const int tile_n = min(TILE_KEYS, n - tile * TILE_KEYS);
 #pragma unroll
     for (int r = 0; r < ITEMS; ++r) {
         int i = base + r * 32 + lane;
         if (i < n) {
             uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
-            uint32_t pos = cnt[w][d] + rank[r];
-            kout[pos] = key[r];
-            vout[pos] = FIRST ? (uint32_t)i : vin[i];
+            rank[r] = (uint16_t)(s_lbase[d] + cnt[w][d] + rank[r]);        // position in the tile's sorted order
+            s_buf[rank[r]] = key[r];
         }
+    }
+    __syncthreads();
+    uint32_t gpos[ITEMS];
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+        const int e = r * P3T_SORT_THREADS + threadIdx.x;
+        gpos[r] = 0;
+        if (e < tile_n) {
+            const uint64_t k = s_buf[e];
+            const uint32_t d = (uint32_t)(k >> shift) & 255u;
+            gpos[r] = s_gbase[d] + ((uint32_t)e - s_lbase[d]);
+            kout[gpos[r]] = k;
+        }
+    }
+    __syncthreads();
+    uint32_t* s_val = reinterpret_cast<uint32_t*>(s_buf);
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+        int i = base + r * 32 + lane;
+        if (i < n) s_val[rank[r]] = FIRST ? (uint32_t)i : vin[i];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < ITEMS; ++r) {
+        const int e = r * P3T_SORT_THREADS + threadIdx.x;
+        if (e < tile_n) vout[gpos[r]] = s_val[e];
     }
 }
 
@@ -213,21 +288,34 @@ __global__ void __launch_bounds__(256) k_permute(const float4* __restrict__ pm, 
 }
 
 // ---------------------------------------------------------------------------------------------
+// layout of ctx->hist: digit totals [SORT_MAX_PASSES][256] u32 | tickets [SORT_MAX_PASSES] u32 (+ pad) | status [ntiles][256] u64
+static inline size_t sort_status_offset() { return (size_t)SORT_MAX_PASSES * P3T_RADIX * 4 + 64; }
+static inline int sort_tile(p3t_ctx* ctx) { return P3T_SORT_THREADS * (ctx->n <= (1 << 18) ? P3T_SORT_ITEMS_MIN : P3T_SORT_ITEMS_BIG); }
+size_t p3t_sort_scratch_bytes(int64_t n)
+{
+    const size_t ntiles = ((size_t)n + P3T_SORT_TILE_MIN - 1) / P3T_SORT_TILE_MIN;
+    return sort_status_offset() + ntiles * P3T_RADIX * 8;
+}
+
 int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pm)
 {
     const int n = (int)ctx->n;
     int blocks = (n + 255) / 256;
     int cap = ctx->num_sms * 8;
     if (blocks > cap) blocks = cap;
+    const int passes = (3 * ctx->bits + P3T_RADIX_BITS - 1) / P3T_RADIX_BITS;     // 8 (63-bit) or 4 (30-bit)
+    const int tile = sort_tile(ctx), ntiles = (n + tile - 1) / tile;
+    // digit totals, tickets and the look-back words of this sort: one clear
+    P3T_CUDA(ctx, cudaMemsetAsync(ctx->hist.p, 0, sort_status_offset() + (size_t)ntiles * P3T_RADIX * 8, ctx->stream));
     k_cube<<<blocks, 256, 0, ctx->stream>>>(pm, n, INFO(ctx));
-    k_keys<<<blocks, 256, 0, ctx->stream>>>(pm, n, ctx->bits, INFO(ctx), P<uint64_t>(ctx->keys[0]));
+    k_keys<<<blocks, 256, 0, ctx->stream>>>(pm, n, ctx->bits, passes, INFO(ctx), P<uint64_t>(ctx->keys[0]), P<uint32_t>(ctx->hist));
     P3T_CUDA(ctx, cudaGetLastError());
     ctx->launches += 2;
     return P3T_OK;
 }
 
 // Tiles of 2048 keys (8 per thread); 1024 below 2^18 particles, where the shorter serial chain of a block and
-// the larger grid matter more than the size of the histogram (measured: sort 0.19 -> 0.12 ms at N = 2^14).
+// the larger grid matter more (measured in round 1: sort 0.19 -> 0.12 ms at N = 2^14).
 template <int ITEMS>
 static int sort_passes(p3t_ctx* ctx)
 {
@@ -235,19 +323,17 @@ static int sort_passes(p3t_ctx* ctx)
     const int tile = P3T_SORT_THREADS * ITEMS;
     const int ntiles = (n + tile - 1) / tile;
     const int passes = (3 * ctx->bits + P3T_RADIX_BITS - 1) / P3T_RADIX_BITS;     // 8 (63-bit) or 4 (30-bit)
-    uint32_t* hist = P<uint32_t>(ctx->hist);
-    uint32_t* totals = hist + (size_t)P3T_RADIX * ntiles;
+    uint32_t* ghist = P<uint32_t>(ctx->hist);
+    uint32_t* ticket = ghist + SORT_MAX_PASSES * P3T_RADIX;
+    unsigned long long* status = (unsigned long long*)((char*)ctx->hist.p + sort_status_offset());
     int cur = 0;
     for (int p = 0; p < passes; ++p) {
-        const int shift = p * P3T_RADIX_BITS;
         uint64_t* kin = P<uint64_t>(ctx->keys[cur]);  uint64_t* kout = P<uint64_t>(ctx->keys[cur ^ 1]);
         uint32_t* vin = P<uint32_t>(ctx->idx[cur]);   uint32_t* vout = P<uint32_t>(ctx->idx[cur ^ 1]);
-        k_hist<ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, n, shift, hist, ntiles);
-        k_scan_rows<<<P3T_RADIX / 8, 256, 0, ctx->stream>>>(hist, ntiles, totals);
-        if (p == 0) k_scatter<true, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
-        else        k_scatter<false, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles, totals);
+        if (p == 0) k_sort_pass<true, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, p, ghist, status, ticket);
+        else        k_sort_pass<false, ITEMS><<<ntiles, P3T_SORT_THREADS, 0, ctx->stream>>>(kin, vin, kout, vout, n, p, ghist, status, ticket);
         cur ^= 1;
-        ctx->launches += 3;
+        ctx->launches += 1;
     }
     P3T_CUDA(ctx, cudaGetLastError());
     // an even number of passes leaves the result in buffer 0
@@ -260,7 +346,7 @@ static int sort_passes(p3t_ctx* ctx)
 
 int p3t_launch_sort(p3t_ctx* ctx)
 {
-    return ctx->n <= (1 << 18) ? sort_passes<P3T_SORT_ITEMS_MIN>(ctx) : sort_passes<8>(ctx);
+    return ctx->n <= (1 << 18) ? sort_passes<P3T_SORT_ITEMS_MIN>(ctx) : sort_passes<P3T_SORT_ITEMS_BIG>(ctx);
 }
 
 int p3t_launch_permute(p3t_ctx* ctx, const float4* pm)

@@ -40,6 +40,9 @@ struct walk_args {
     int32_t* spill;
     p3t_devinfo* info;
     float rout2, theta;
+    int32_t* gready;            // WALK_LISTS: per-group list state (p3t_internal.cuh: G_READY ...)
+    int base, repair;           // epoch of the call; repair = host repair pass (no force kernel is waiting)
+    int spill_cap;              // <= SPILL_CAP (smaller only under P3T_TEST_FAULT, to exercise the overflow report)
 };
 
 struct __align__(16) warp_smem {
@@ -144,7 +147,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
             const int total = __shfl_sync(0xffffffffu, x, 31);
-            if (top + total > STACK_CAP + SPILL_CAP) { overflow = 1; break; }
+            if (top + total > STACK_CAP + A.spill_cap) { overflow = 1; break; }
             const int w = top + x - c;
             if (top + total <= STACK_CAP) {                    // warp-uniform: everything stays in shared memory
 #pragma unroll
@@ -235,6 +238,26 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
             atomicAdd(&A.info->n_pp_list, (unsigned long long)npp); atomicAdd(&A.info->n_pc_list, (unsigned long long)npc);
             if (ovf) atomicOr(&A.info->pool_overflow, 1);
         }
+        // Publish the group: the force kernel (running at the same time) waits for this word.  Every lane's list stores
+        // precede the warp barrier, lane 0's release makes them visible with the state.  A group whose lists are
+        // incomplete is marked failed and skipped by the force kernel; the host's repair pass (this kernel again,
+        // larger pools, A.repair) redoes it.
+        __syncwarp();
+        if (lane == 0) {
+            const bool failed = ovf || overflow;
+            if (A.repair) {
+                const int v = A.gready[g];
+                if (v == A.base + G_FAILED && !failed) A.gready[g] = A.base + G_REDONE;
+            } else {
+                const int want = A.base + (failed ? G_FAILED : G_READY);
+                int v = *(volatile int32_t*)&A.gready[g];
+                while (!g_decided(v, A.base)) {                     // decided already: a force warp gave up on this group
+                    const int old = cas_release_gpu(&A.gready[g], v, want);
+                    if (old == v) break;
+                    v = old;
+                }
+            }
+        }
     } else {
 #pragma unroll
         for (int s = 0; s < 2; ++s)
@@ -250,6 +273,7 @@ __global__ void __launch_bounds__(WALK_THREADS) k_walk(walk_args A)
     __shared__ count_smem csm[MODE == WALK_COUNT ? WALK_WARPS : 1];
     __shared__ float s_lt[24];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (A.info->bad_input | A.info->node_overflow) return;       // nothing is written for an invalid build (the host reports it)
     if (threadIdx.x < 24) s_lt[threadIdx.x] = __fdiv_rn(ldexpf(A.info->side, -(int)threadIdx.x), A.theta);
     __syncthreads();
     warp_smem& S = smem[w];
@@ -273,14 +297,15 @@ __global__ void __launch_bounds__(WALK_THREADS) k_walk(walk_args A)
     }
 }
 
-__global__ void k_walk_reset(p3t_devinfo* info, int mode)
+// all cursors and counters of one force call (one launch, before the count walk, the list walk and the force kernel
+// go to their streams)
+__global__ void k_walk_reset(p3t_devinfo* info)
 {
-    if (mode == WALK_COUNT) { info->group_cursor2 = 0; info->nb_total = 0ull; info->nb_max = 0; }
-    else {
-        info->group_cursor = 0; info->group_cursor3 = 0;
-        info->n_pp = info->n_pc = info->n_pp_list = info->n_pc_list = 0ull;
-        info->pool_overflow = 0; info->need_pc = 0; info->need_pp = 0;
-    }
+    info->group_cursor2 = 0; info->nb_total = 0ull; info->nb_max = 0;
+    info->group_cursor = 0; info->group_cursor3 = 0;
+    info->n_pp = info->n_pc = info->n_pp_list = info->n_pc_list = 0ull;
+    info->pool_overflow = 0; info->need_pc = 0; info->need_pp = 0;
+    info->nb_overflow = 0; info->spin_abort = 0;
 }
 
 static int walk_blocks(p3t_ctx* ctx, int mode, int* out, bool limit_by_n = true)
@@ -310,45 +335,67 @@ static void fill_args(p3t_ctx* ctx, walk_args& A, float r_out, float theta)
     A.spill = P<int32_t>(ctx->spill); A.info = INFO(ctx);
     volatile float ro2 = r_out * r_out;           // one fp32 product, as R10 states it
     A.rout2 = ro2; A.theta = theta;
+    A.gready = P<int32_t>(ctx->gready); A.base = 0; A.repair = 0;
+    A.spill_cap = (ctx->test_fault & 2) ? 0 : SPILL_CAP;
 }
 
-// a10, first half: neighbour counts per ORIGINAL id into ctx->nbcount
-int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta)
+int p3t_launch_walk_reset(p3t_ctx* ctx, cudaStream_t st)
 {
-    int blocks, rc;
-    if ((rc = walk_blocks(ctx, WALK_COUNT, &blocks))) return rc;
-    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)ctx->walk_warps_max * SPILL_CAP * sizeof(int32_t)))) return rc;
-    walk_args A; fill_args(ctx, A, r_out, theta);
-    k_walk_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx), WALK_COUNT);
-    k_walk<WALK_COUNT><<<blocks, WALK_THREADS, 0, ctx->stream>>>(A);
+    k_walk_reset<<<1, 1, 0, st>>>(INFO(ctx));
     P3T_CUDA(ctx, cudaGetLastError());
-    ctx->launches += 2;
+    ctx->launches += 1;
     return P3T_OK;
 }
 
-// a7: interaction lists.  Sizes the pools on first use (and after an overflow, from the measured need).
-int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta)
+// a10, first half: neighbour counts per ORIGINAL id into ctx->nbcount
+int p3t_launch_walk_count(p3t_ctx* ctx, float r_out, float theta, cudaStream_t st)
+{
+    int blocks, rc;
+    if ((rc = walk_blocks(ctx, WALK_COUNT, &blocks))) return rc;
+    walk_args A; fill_args(ctx, A, r_out, theta);
+    A.spill = P<int32_t>(ctx->spill) + (size_t)ctx->walk_warps_max * SPILL_CAP;      // second half: the list walk may run at the same time
+    k_walk<WALK_COUNT><<<blocks, WALK_THREADS, 0, st>>>(A);
+    P3T_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return P3T_OK;
+}
+
+// buffers of both walks: reserved before anything of the call is enqueued (a reallocation synchronises)
+int p3t_walk_reserve(p3t_ctx* ctx, int ctas_per_sm)
 {
     int blocks, rc;
     if ((rc = walk_blocks(ctx, WALK_LISTS, &blocks))) return rc;
+    if (ctas_per_sm > 0 && blocks > ctas_per_sm * ctx->num_sms) blocks = ctas_per_sm * ctx->num_sms;
     const long long warps = (long long)blocks * WALK_WARPS;
-    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)ctx->walk_warps_max * SPILL_CAP * sizeof(int32_t)))) return rc;
-    if (ctx->pool_cap_pc == 0) {
-        // first call: a guess from the group count (lists of the paper's workloads hold 4-8 thousand
-        // cells and 1-3 thousand particles at theta = 0.4); corrected below if it was too small
+    if ((rc = p3t_reserve(ctx, &ctx->spill, (size_t)ctx->walk_warps_max * 2 * SPILL_CAP * sizeof(int32_t)))) return rc;
+    if (ctx->pool_cap_pc == 0 || warps != ctx->walk_list_warps) {
+        // first call (or another share of the device): a guess from the group count (lists of the paper's workloads
+        // hold 4-8 thousand cells and 1-3 thousand particles at theta = 0.4); corrected by the repair pass if too small.
+        // A context that has measured its need keeps the total and spreads it over the new number of walker warps.
         const long long ng = (ctx->n + 31) / 32;
-        ctx->pool_cap_pc = ((ng * 6000 / warps + 16384) + 31) & ~31ll;
-        ctx->pool_cap_pp = ((ng * 3000 / warps + 16384) + 31) & ~31ll;
+        long long tot_pc = ng * 6000, tot_pp = ng * 3000;
+        if (ctx->pool_cap_pc != 0) { tot_pc = ctx->pool_cap_pc * ctx->walk_list_warps; tot_pp = ctx->pool_cap_pp * ctx->walk_list_warps; }
+        ctx->pool_cap_pc = ((tot_pc / warps + 16384) + 31) & ~31ll;
+        ctx->pool_cap_pp = ((tot_pp / warps + 16384) + 31) & ~31ll;
+        ctx->walk_list_warps = warps;
     }
     if ((rc = p3t_reserve(ctx, &ctx->pcpool, (size_t)(warps * ctx->pool_cap_pc) * 4))) return rc;
     if ((rc = p3t_reserve(ctx, &ctx->pppool, (size_t)(warps * ctx->pool_cap_pp) * 4))) return rc;
     if ((rc = p3t_reserve(ctx, &ctx->glist, ((size_t)ctx->n + 1) * sizeof(uint4)))) return rc;
+    return P3T_OK;
+}
+
+// a7: interaction lists (p3t_walk_reserve has sized the pools for this share of the device)
+int p3t_launch_walk_lists(p3t_ctx* ctx, float r_out, float theta, cudaStream_t st, int base, int repair, int ctas_per_sm)
+{
+    int blocks, rc;
+    if ((rc = p3t_walk_reserve(ctx, ctas_per_sm))) return rc;
+    blocks = (int)(ctx->walk_list_warps / WALK_WARPS);
     walk_args A; fill_args(ctx, A, r_out, theta);
-    k_walk_reset<<<1, 1, 0, ctx->stream>>>(INFO(ctx), WALK_LISTS);
-    k_walk<WALK_LISTS><<<blocks, WALK_THREADS, 0, ctx->stream>>>(A);
+    A.base = base; A.repair = repair;
+    k_walk<WALK_LISTS><<<blocks, WALK_THREADS, 0, st>>>(A);
     P3T_CUDA(ctx, cudaGetLastError());
-    ctx->launches += 2;
-    ctx->walk_list_warps = warps;
+    ctx->launches += 1;
     return P3T_OK;
 }
 

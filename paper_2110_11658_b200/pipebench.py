@@ -1,7 +1,41 @@
-"""python -m paper_2110_11658_b200.pipebench -- print the FP32-pipe micro-benchmarks of cuda:0."""
-import json
+"""Diagnostics (include/p3t_diag.h, libp3t_diag.so -- not part of libp3t.so): FP32-pipe micro-benchmarks of a device.
+`python -m paper_2110_11658_b200.pipebench` prints the table for cuda:0."""
+from __future__ import annotations
 
-from . import pipe_bench
+import ctypes as C
+from pathlib import Path
+
+DIAG_PATH = Path(__file__).resolve().parent / "libp3t_diag.so"
+DIAG_SYMBOLS = ["p3t_diag_pipe_bench"]
+LABELS = ["FFMA (reuse cache)", "FFMA2, 2 distinct register pairs", "FFMA2, 3 distinct register pairs", "FMUL2",
+          "FMUL2 + FFMA (pair)", "8 FMUL2 + 2 MUFU.RSQ (group)", "MUFU.RSQ", "FFMA, 3 distinct registers"]
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        if not DIAG_PATH.exists():
+            raise ImportError(f"{DIAG_PATH} is missing: build it with `python -m paper_2110_11658_b200.build`")
+        _lib = C.CDLL(str(DIAG_PATH))
+        _lib.p3t_diag_pipe_bench.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+        _lib.p3t_diag_pipe_bench.restype = C.c_int
+    return _lib
+
+
+def pipe_bench(device: int = 0) -> dict:
+    """Cycles per SM sub-partition for each instruction pattern, and the FP32 lane-instruction peak they imply
+    (32 lanes / cycles[FFMA] per sub-partition)."""
+    out = (C.c_double * 8)(); mhz = C.c_double(); sms = C.c_int()
+    rc = lib().p3t_diag_pipe_bench(device, out, 8, C.byref(mhz), C.byref(sms))
+    if rc != 0:
+        raise RuntimeError(f"p3t_diag_pipe_bench failed ({rc})")
+    cyc = [float(x) for x in out]
+    peak = sms.value * 4 * 32 / cyc[0] * mhz.value * 1e6
+    return dict(cycles=dict(zip(LABELS, cyc)), sm_clock_mhz=mhz.value, num_sms=sms.value,
+                fp32_lane_instr_per_s=peak, nominal_lane_instr_per_s=sms.value * 128 * mhz.value * 1e6)
+
 
 if __name__ == "__main__":
+    import json
     print(json.dumps(pipe_bench(0), indent=1))

@@ -98,3 +98,44 @@ def gather_group_costs(ctx, group=None):
         dist.all_reduce(cost, group=group)
         cost = cost.cpu()
     return g["begin"].astype(np.int64), cost.numpy()
+
+
+def merge_neighbour_rows(counts_all, chunks, n: int):
+    """Host-side logic of the neighbour exchange ("one all-gather of acc_pot and of the CSR rows"):
+    counts_all[r] = per-particle row lengths of rank r (int64 [n], zero for the particles it does not own: every
+    particle is owned by exactly one rank), chunks[r] = rank r's indices, rows back to back in original particle order.
+    Returns the CSR of all particles (offsets int64 [n + 1], indices int32), identical to that of an unsharded context.
+    Pure index arithmetic on whatever device the tensors live on (moves entries, computes nothing of the method)."""
+    import torch
+    dev = chunks[0].device
+    total = torch.zeros(n, dtype=torch.int64, device=dev)
+    for c in counts_all:
+        total += c
+    off = torch.zeros(n + 1, dtype=torch.int64, device=dev)
+    torch.cumsum(total, 0, out=off[1:])
+    out = torch.empty(int(off[-1].item()), dtype=torch.int32, device=dev)
+    for c, idx in zip(counts_all, chunks):
+        m = int(idx.shape[0])
+        if m == 0:
+            continue
+        own_off = torch.cumsum(c, 0) - c                                   # this rank's own offsets
+        rows = torch.repeat_interleave(torch.arange(n, device=dev), c)     # particle of every entry of the chunk
+        pos = torch.arange(m, device=dev) - own_off[rows]
+        out[off[rows] + pos] = idx
+    return off, out
+
+
+def exchange_neighbours(ctx, group=None):
+    """Completes the neighbour CSR on every rank: all-gathers the ranks' row lengths and index chunks (padded to the
+    largest) and merges them (merge_neighbour_rows).  Returns (offsets, indices) as tensors on the context's device."""
+    import torch
+    import torch.distributed as dist
+    off, idx = ctx.neighbours()
+    n = off.shape[0] - 1
+    counts = (off[1:] - off[:-1]).contiguous()
+    nr = dist.get_world_size(group)
+    counts_all = [torch.empty_like(counts) for _ in range(nr)]
+    dist.all_gather(counts_all, counts, group=group)
+    sizes = [int(c.sum().item()) for c in counts_all]
+    chunks = all_gather_chunks(idx.reshape(-1, 1), sizes, group)
+    return merge_neighbour_rows(counts_all, [c.reshape(-1) for c in chunks], n)

@@ -93,12 +93,11 @@ def test_product_never_imports_the_oracle():
             assert '#include "p3t.h"' not in t and "p3t_internal" not in t and "libp3t.so" not in t, f
 
 
-def test_regularisation_params_eq18_19(p3t):
-    """eq. 18-19: R_min = 4 r_h / (N rho_core^(1/3)); dT_min = 0.01 sqrt(eta/0.02) sqrt(R_min^3).
-    Hand case: N = 1000, r_h = 0.5, rho_core = 8 -> R_min = 4 * 0.5 / (1000 * 2) = 1e-3; dT_min = 0.01 * 1e-4.5."""
-    r_min, dt_min = p3t.regularisation_params(1000, 0.5, 8.0)
-    assert abs(r_min - 1e-3) < 1e-18 and abs(dt_min - 0.01 * 1e-3 ** 1.5) < 1e-20
-    r2, dt2 = p3t.regularisation_params(1000, 0.5, 8.0, eta=0.08)
-    assert r2 == r_min and abs(dt2 / dt_min - 2.0) < 1e-14
-    assert p3t.lib().p3t_regularisation_params(0, 0.5, 8.0, 0.02, None, None) == p3t.EINVAL
-    assert p3t.lib().p3t_regularisation_params(10, 0.5, -1.0, 0.02, None, None) == p3t.EINVAL
+def test_diagnostics_library_is_separate(p3t):
+    """include/p3t_diag.h (FP32-pipe micro-benchmarks) is exported by libp3t_diag.so, not by the product library."""
+    from paper_2110_11658_b200 import pipebench
+    text = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "p3t_diag.h").read_text(), flags=re.S)
+    decl = sorted(set(re.findall(r"\b(p3t_[a-z0-9_]+)\s*\(", text)))
+    assert decl == sorted(pipebench.DIAG_SYMBOLS)
+    for s in decl:
+        assert hasattr(pipebench.lib(), s) and not hasattr(p3t.lib(), s)

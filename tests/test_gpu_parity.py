@@ -54,15 +54,23 @@ def check_build(ctx, T, pm, bits):
     assert np.array_equal(om["clo"], gm["clo"]) and np.array_equal(om["chi"], gm["chi"])     # exact min/max
     l = side / 2.0 ** on["level"].astype(np.float64)
     mass = om["com_m"][:, 3].astype(np.float64)
-    # moments: fp64 sums in another order, rounded once to fp32: equal up to rare 1-ulp flips
-    assert np.abs(gm["com_m"][:, :3].astype(np.float64) - om["com_m"][:, :3]).max() <= 1e-6 * side
-    assert np.abs(gm["com_m"][:, 3] / om["com_m"][:, 3] - 1).max() <= 2e-7
-    scale_q = np.maximum(np.abs(om["quad"]).max(axis=1), 1e-300)
-    qerr = np.abs(gm["quad"].astype(np.float64) - om["quad"]).max(axis=1)
-    assert np.all(qerr <= 1e-5 * np.maximum(scale_q, 1e-7 * mass * l * l))
-    assert np.abs(gm["delta"].astype(np.float64) - om["delta"]).max() <= 1e-6 * side
+    # Moments: both sides accumulate in fp64 (in different orders) and round ONCE to fp32, so the stored
+    # values are bit-equal except where the two fp64 sums straddle a rounding boundary: at most 1 ulp (1.2e-7
+    # relative) then, with probability ~ (fp64 error) / (fp32 ulp) ~ 1e-8 per value for M, COM, delta.  The traceless
+    # Q_ab = sum m (3 d_a d_b - delta_ab d^2) cancels: its fp64 error is ~1e-16 M l^2 whatever its size, so a small
+    # component flips more often and may differ by that absolute amount: bound 1 ulp + 1e-12 M l^2, flips counted apart.
+    ulp = 1.2e-7
+    assert np.all(np.abs(gm["com_m"][:, :3].astype(np.float64) - om["com_m"][:, :3]) <= ulp * np.abs(om["com_m"][:, :3].astype(np.float64)) + 1e-12 * side)
+    assert np.all(np.abs(gm["com_m"][:, 3].astype(np.float64) - om["com_m"][:, 3]) <= ulp * np.abs(om["com_m"][:, 3].astype(np.float64)))
+    qerr = np.abs(gm["quad"].astype(np.float64) - om["quad"])
+    assert np.all(qerr <= ulp * np.abs(om["quad"].astype(np.float64)) + 1e-12 * (mass * l * l)[:, None])
+    assert np.all(np.abs(gm["delta"].astype(np.float64) - om["delta"]) <= ulp * np.abs(om["delta"].astype(np.float64)) + 1e-12 * side)
     n_flip = sum(int(np.count_nonzero(gm[k] != om[k])) for k in ("com_m", "delta"))
-    assert n_flip <= 2 + T.n_nodes // 100000, f"{n_flip} COM/delta values differ in the last bit"
+    q_flip = int(np.count_nonzero(gm["quad"] != om["quad"]))
+    assert n_flip <= 2 + T.n_nodes // 100000, f"{n_flip} COM/M/delta values differ in the last bit"
+    # measured: 153 of 5.7e6 values at config 5 (equal masses: 2.7e-5 per value), fewer with the Kroupa masses of config 3
+    assert q_flip <= 10 + T.n_nodes // 2000, f"{q_flip} quadrupole values differ in the last bit"
+    return n_flip, q_flip
 
 
 def check_force(ctx, T, w, pot_mode=0, group_ids=None, theta=None, per_particle=True):
@@ -86,7 +94,7 @@ def check_force(ctx, T, w, pot_mode=0, group_ids=None, theta=None, per_particle=
     assert np.all(da <= 1e-6 * cond + 1e-30), (da / np.maximum(cond, 1e-300)).max()
     # potential: same terms, one more rounding each
     pa = np.abs(a[m, 3] - ref[m, 3])
-    assert np.all(pa <= 2e-6 * np.abs(ref[m, 3]) + 1e-30)
+    assert np.all(pa <= 1e-6 * np.abs(ref[m, 3]) + 1e-30)
     return a, f
 
 
@@ -446,7 +454,7 @@ def test_monopole_only_variant(p3t, cfg1):
         ref = f1["acc_pot"]
         assert np.linalg.norm(a1[:, :3] - ref[:, :3]) <= 1e-6 * np.linalg.norm(ref[:, :3])
         assert np.all(np.linalg.norm(a1[:, :3] - ref[:, :3], axis=1) <= 1e-6 * f1["abs_sum"] + 1e-30)
-        assert np.all(np.abs(a1[:, 3] - ref[:, 3]) <= 2e-6 * np.abs(ref[:, 3]))
+        assert np.all(np.abs(a1[:, 3] - ref[:, 3]) <= 1e-6 * np.abs(ref[:, 3]))
         d = oracle.direct(w.pos_mass, w.r_out, w.r_in)
         e1 = _rel(a1[:, :3], d["acc_reg"]); e2 = _rel(a2[:, :3], d["acc_reg"])
         assert np.median(e1) < 2e-3 and np.percentile(e1, 99) < 2e-2 and np.median(e1) > 3 * np.median(e2)
@@ -499,7 +507,7 @@ def test_randomised_shapes_and_tree_parameters(p3t):
             npp, npc = ctx.list_lengths()
             assert np.array_equal(npp, f["npp"]) and np.array_equal(npc, f["npc"]), tag
             assert np.all(np.isfinite(a)), tag
-            assert np.all(np.linalg.norm(a[:, :3] - f["acc_pot"][:, :3], axis=1) <= 2e-6 * f["abs_sum"] + 1e-30), tag
+            assert np.all(np.linalg.norm(a[:, :3] - f["acc_pot"][:, :3], axis=1) <= 1e-6 * f["abs_sum"] + 1e-30), tag
             off, idx = ctx.neighbours()
             ooff, oidx = oracle.neighbours(pm, r_out)
             assert np.array_equal(ooff, off.cpu().numpy()) and np.array_equal(oidx, idx.cpu().numpy()), tag

@@ -89,3 +89,21 @@ def test_all_gather_chunks_gloo(sizes):
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res == [(r, True) for r in range(world)]
+
+
+def test_merge_neighbour_rows_is_the_unsharded_csr():
+    """The CSR exchange of the sharded mode, host logic: random rows split among 3 owners."""
+    rng = np.random.default_rng(3)
+    n = 500
+    lens = rng.integers(0, 9, n); lens[rng.random(n) < 0.4] = 0
+    off = np.concatenate(([0], np.cumsum(lens)))
+    idx = rng.integers(0, n, off[-1]).astype(np.int32)
+    owner = np.sort(rng.integers(0, 3, n))                        # contiguous ownership is not required: shuffle it
+    rng.shuffle(owner)
+    counts_all, chunks = [], []
+    for r in range(3):
+        c = np.where(owner == r, lens, 0)
+        counts_all.append(torch.from_numpy(c.astype(np.int64)))
+        chunks.append(torch.from_numpy(np.concatenate([idx[off[i]:off[i + 1]] for i in range(n) if owner[i] == r] + [np.zeros(0, np.int32)]).astype(np.int32)))
+    goff, gidx = shard.merge_neighbour_rows(counts_all, chunks, n)
+    assert np.array_equal(goff.numpy(), off) and np.array_equal(gidx.numpy(), idx)
