@@ -61,6 +61,7 @@ struct p3t_ctx {
     cudaStream_t stream;
     cudaStream_t copy_stream;        // p3t_step_host: device-to-host copies that overlap the force kernel (created on first use)
     int num_sms;
+    int occ_moments;                 // resident CTAs per SM of k_moments (cooperative launch)
     int occ_walk[2], occ_force;      // resident CTAs per SM of k_walk<COUNT / LISTS> and k_force on this device (0 = not asked yet)
     int nleaf, ncrit;
     int order;               // multipole order of the p-c terms: 2 (default) or 1

@@ -18,6 +18,7 @@
 // Moments then climb the tree with one arrival counter per cell (the last child to arrive
 // computes its parent, combining the children in their fixed order), again without barriers.
 #include "p3t_internal.cuh"
+#include <cooperative_groups.h>
 
 #define TOPO_THREADS 256
 #define TOPO_WARPS   (TOPO_THREADS / 32)
@@ -101,14 +102,19 @@ __global__ void __launch_bounds__(32 * MAXLEV) k_topo_scan(tree_args A)
     if (l >= 1 && l <= A.B) {
         int32_t* row = A.blksum + (size_t)l * A.nblk;
         int run = 0;
-        for (int b0 = 0; b0 < A.nblk; b0 += 32) {
-            const int b = b0 + lane;
-            const int v = b < A.nblk ? row[b] : 0;
-            int x = v;
+        for (int b0 = 0; b0 < A.nblk; b0 += 256) {           // eight loads in flight per lane: the row is read in a few round trips
+            int v[8];
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-            if (b < A.nblk) row[b] = run + x - v;
-            run += __shfl_sync(0xffffffffu, x, 31);
+            for (int j = 0; j < 8; ++j) { const int b = b0 + 32 * j + lane; v[j] = b < A.nblk ? row[b] : 0; }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int b = b0 + 32 * j + lane;
+                int x = v[j];
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+                if (b < A.nblk) row[b] = run + x - v[j];
+                run += __shfl_sync(0xffffffffu, x, 31);
+            }
         }
         if (lane == 0) s_tot[l] = run;
     }
@@ -181,10 +187,12 @@ __global__ void __launch_bounds__(TOPO_THREADS) k_topo_nodes(tree_args A)
 __global__ void __launch_bounds__(NODE_THREADS) k_topo_link(tree_args A)
 {
     const int nn = A.info->n_nodes;
-    const int k = blockIdx.x * NODE_THREADS + threadIdx.x;
     const int* __restrict__ lb = A.info->level_begin;
-    int leaf = 0;
-    if (k < nn && !A.info->node_overflow) {
+    if (A.info->node_overflow) return;
+    int leaves = 0;
+    // the cell count is only known on the device: a fixed grid strides over the cells (a grid sized by the host's bound
+    // on the count would be ten times too large, and empty blocks are not free)
+    for (int k = blockIdx.x * NODE_THREADS + threadIdx.x; k < nn; k += gridDim.x * NODE_THREADS) {
         const int lev = A.nlevel[k];
         int end = A.n;
         for (int w = k, l = lev; l > 0; --l) {
@@ -199,10 +207,21 @@ __global__ void __launch_bounds__(NODE_THREADS) k_topo_link(tree_args A)
         const int nc = lev < A.B ? fc_next - fc : 0;
         A.nnchild[k] = nc; A.nfirst[k] = nc > 0 ? fc : -1;
         A.ncount[k] = 0;
-        leaf = nc == 0;
+        leaves += nc == 0;
     }
-    const int tot = __syncthreads_count(leaf);
-    if (threadIdx.x == 0 && tot) atomicAdd(&A.info->n_leaves, tot);
+    // block sum of the leaf counts
+    const int tot = leaves;
+    __shared__ int s_leaf[NODE_THREADS / 32];
+    int x = tot;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if ((threadIdx.x & 31) == 0) s_leaf[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int k = 0; k < NODE_THREADS / 32; ++k) t += s_leaf[k];
+        if (t) atomicAdd(&A.info->n_leaves, t);
+    }
 }
 
 __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-way bit spread
@@ -245,71 +264,133 @@ __device__ void store_node(const tree_args& A, int k, int level, int b, int e, i
 }
 
 // ---------------- a5 moments (R-S6), fp64 ----------------
-// One thread per cell.  A leaf sums its particles, then climbs: every cell counts the children that
-// have finished; the thread that brings the count to n_child combines the children (in child order,
-// whatever the order of arrival: the result is bit-reproducible) and goes on to the parent.
-__global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
+// One cooperative launch.  Phase 0: every leaf from its particles (one thread per leaf).  Then the internal cells level
+// by level from the deepest up (cells are numbered breadth-first, so a level is a contiguous range), a grid barrier
+// between two levels.  An internal cell is combined by eight lanes, one per child: each lane loads its child's fp64
+// record (one round trip for the whole cell), the sums go through a fixed xor tree over the eight lanes (idle lanes add
+// exact zeros), so the result does not depend on timing: bit-reproducible, and no atomics or fences are needed.
+// (Rounds 1's version climbed from the leaves with one arrival counter per cell: a chain of L2 round trips per level
+// in ever fewer, diverged threads -- 0.12 ms at N = 2^20.)
+__device__ __forceinline__ double shfl_xor_f64(double v, int o)
 {
-    const int nn = A.info->n_nodes;
-    int k = blockIdx.x * NODE_THREADS + threadIdx.x;
-    if (k >= nn || A.info->node_overflow || A.nnchild[k] != 0) return;
-    {
-        const int b = A.nbegin[k], e = A.nend[k];
-        double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
-        float4 p0 = A.spm[b];
-        float clo[3] = { p0.x, p0.y, p0.z }, chi[3] = { p0.x, p0.y, p0.z };
-        for (int i = b; i < e; ++i) {
-            float4 p = A.spm[i];
-            double m = p.w;
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_xor_sync(0xffffffffu, lo, o); hi = __shfl_xor_sync(0xffffffffu, hi, o);
+    return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double seg8_sum(double v)
+{
+    v += shfl_xor_f64(v, 1); v += shfl_xor_f64(v, 2); v += shfl_xor_f64(v, 4);
+    return v;
+}
+__device__ __forceinline__ float seg8_min(float v)
+{
+    v = fminf(v, __shfl_xor_sync(0xffffffffu, v, 1)); v = fminf(v, __shfl_xor_sync(0xffffffffu, v, 2)); v = fminf(v, __shfl_xor_sync(0xffffffffu, v, 4));
+    return v;
+}
+__device__ __forceinline__ float seg8_max(float v)
+{
+    v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1)); v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2)); v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 4));
+    return v;
+}
+
+__device__ void leaf_moments(const tree_args& A, int k)
+{
+    const int b = A.nbegin[k], e = A.nend[k];
+    double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
+    const float4 p0 = A.spm[b];
+    float clo[3] = { p0.x, p0.y, p0.z }, chi[3] = { p0.x, p0.y, p0.z };
+    for (int i0 = b; i0 < e; i0 += 4) {                     // four loads in flight; summed in particle order
+        float4 q[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) q[j] = A.spm[min(i0 + j, e - 1)];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (i0 + j >= e) break;
+            const float4 p = q[j];
+            const double m = p.w;
             M += m; s[0] += m * (double)p.x; s[1] += m * (double)p.y; s[2] += m * (double)p.z;
             clo[0] = fminf(clo[0], p.x); clo[1] = fminf(clo[1], p.y); clo[2] = fminf(clo[2], p.z);
             chi[0] = fmaxf(chi[0], p.x); chi[1] = fmaxf(chi[1], p.y); chi[2] = fmaxf(chi[2], p.z);
         }
-        // R-S6a: a cell of massless particles takes the position of its first particle (sorted order) as its centre
-        const bool massless = M == 0.0;
-        const double c[3] = { massless ? (double)p0.x : s[0] / M, massless ? (double)p0.y : s[1] / M, massless ? (double)p0.z : s[2] / M };
-        double Q[6] = { 0, 0, 0, 0, 0, 0 };
-        for (int i = b; i < e; ++i) {
-            float4 p = A.spm[i];
-            double m = p.w, dx = p.x - c[0], dy = p.y - c[1], dz = p.z - c[2];
-            double d2 = dx * dx + dy * dy + dz * dz;
+    }
+    // R-S6a: a cell of massless particles takes the position of its first particle (sorted order) as its centre
+    const bool massless = M == 0.0;
+    const double c[3] = { massless ? (double)p0.x : s[0] / M, massless ? (double)p0.y : s[1] / M, massless ? (double)p0.z : s[2] / M };
+    double Q[6] = { 0, 0, 0, 0, 0, 0 };
+    for (int i0 = b; i0 < e; i0 += 4) {
+        float4 q[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) q[j] = A.spm[min(i0 + j, e - 1)];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (i0 + j >= e) break;
+            const float4 p = q[j];
+            const double m = p.w, dx = p.x - c[0], dy = p.y - c[1], dz = p.z - c[2];
+            const double d2 = dx * dx + dy * dy + dz * dz;
             Q[0] += m * (3 * dx * dx - d2); Q[1] += m * (3 * dy * dy - d2); Q[2] += m * (3 * dz * dz - d2);
             Q[3] += m * 3 * dx * dy; Q[4] += m * 3 * dx * dz; Q[5] += m * 3 * dy * dz;
         }
-        store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, c, Q, clo, chi);
     }
-    for (;;) {
-        const int p = A.nparent[k];
-        if (p < 0) break;
-        __threadfence();                                           // this cell's data before the count
-        if (atomicAdd(&A.ncount[p], 1) + 1 < A.nnchild[p]) break;  // a later sibling will do the parent
-        __threadfence();
-        // internal cell: parallel-axis combination of the children (read past L1: other SMs wrote them)
-        k = p;
-        const int nc = A.nnchild[k], fc = A.nfirst[k];
-        double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
-        float clo[3] = { INFINITY, INFINITY, INFINITY }, chi[3] = { -INFINITY, -INFINITY, -INFINITY };
-        for (int c = fc; c < fc + nc; ++c) {
-            const double* m = A.m64 + (size_t)c * 13;
-            M += __ldcg(m); s[0] += __ldcg(m + 1); s[1] += __ldcg(m + 2); s[2] += __ldcg(m + 3);
-            float4 lo = __ldcg(&A.nlo[c]), hi = __ldcg(&A.nhi[c]);
-            clo[0] = fminf(clo[0], lo.x); clo[1] = fminf(clo[1], lo.y); clo[2] = fminf(clo[2], lo.z);
-            chi[0] = fmaxf(chi[0], hi.x); chi[1] = fmaxf(chi[1], hi.y); chi[2] = fmaxf(chi[2], hi.z);
+    store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, c, Q, clo, chi);
+}
+
+#define MOM_THREADS 256
+__global__ void __launch_bounds__(MOM_THREADS) k_moments(tree_args A)
+{
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const int nn = A.info->n_nodes;
+    if (A.info->node_overflow) return;                       // uniform over the grid: nobody reaches a barrier
+    const int gtid = blockIdx.x * MOM_THREADS + threadIdx.x, gsize = gridDim.x * MOM_THREADS;
+    for (int k = gtid; k < nn; k += gsize)
+        if (A.nnchild[k] == 0) leaf_moments(A, k);
+    const int* __restrict__ lb = A.info->level_begin;
+    const int lane = threadIdx.x & 31, seg = lane >> 3, j = lane & 7;
+    const int gwarp = gtid >> 5, nwarps = gsize >> 5;
+    for (int l = A.info->max_level - 1; l >= 0; --l) {
+        grid.sync();
+        const int k_end = lb[l + 1];
+        for (int k4 = lb[l] + 4 * gwarp; k4 < k_end; k4 += 4 * nwarps) {          // warp-uniform trip count: four cells per warp
+            const int k = k4 + seg;
+            int nc = 0, fc = 0;
+            if (k < k_end) { nc = A.nnchild[k]; fc = A.nfirst[k]; }
+            const bool have = j < nc;
+            // this lane's child (read past L1: another SM wrote it in this launch)
+            double cM = 0.0, cs[3] = { 0, 0, 0 }, cQ[6] = { 0, 0, 0, 0, 0, 0 }, cc[3] = { 0, 0, 0 };
+            float lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+            if (have) {
+                const double* m = A.m64 + (size_t)(fc + j) * 13;
+                cM = __ldcg(m); cs[0] = __ldcg(m + 1); cs[1] = __ldcg(m + 2); cs[2] = __ldcg(m + 3);
+#pragma unroll
+                for (int q = 0; q < 6; ++q) cQ[q] = __ldcg(m + 4 + q);
+                cc[0] = __ldcg(m + 10); cc[1] = __ldcg(m + 11); cc[2] = __ldcg(m + 12);
+                const float4 l4 = __ldcg(&A.nlo[fc + j]), h4 = __ldcg(&A.nhi[fc + j]);
+                lo[0] = l4.x; lo[1] = l4.y; lo[2] = l4.z; hi[0] = h4.x; hi[1] = h4.y; hi[2] = h4.z;
+            }
+            const double M = seg8_sum(cM);
+            double s[3] = { seg8_sum(cs[0]), seg8_sum(cs[1]), seg8_sum(cs[2]) };
+            float clo[3], chi[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { clo[a] = seg8_min(lo[a]); chi[a] = seg8_max(hi[a]); }
+            // R-S6a: massless cell: the centre of its first child, i.e. its first particle in sorted order
+            const bool massless = M == 0.0;
+            double cm[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const int first = lane & ~7;                                       // lane of the first child
+                int l0 = __shfl_sync(0xffffffffu, __double2loint(cc[a]), first), h0 = __shfl_sync(0xffffffffu, __double2hiint(cc[a]), first);
+                cm[a] = massless ? __hiloint2double(h0, l0) : s[a] / M;
+            }
+            double Q[6];
+            {
+                const double dx = cc[0] - cm[0], dy = cc[1] - cm[1], dz = cc[2] - cm[2];
+                const double d2 = dx * dx + dy * dy + dz * dz;
+                const double t[6] = { cQ[0] + cM * (3 * dx * dx - d2), cQ[1] + cM * (3 * dy * dy - d2), cQ[2] + cM * (3 * dz * dz - d2),
+                                      cQ[3] + cM * 3 * dx * dy, cQ[4] + cM * 3 * dx * dz, cQ[5] + cM * 3 * dy * dz };
+#pragma unroll
+                for (int q = 0; q < 6; ++q) Q[q] = seg8_sum(have ? t[q] : 0.0);
+            }
+            if (j == 0 && nc > 0) store_node(A, k, l, A.nbegin[k], A.nend[k], fc, nc, M, s, cm, Q, clo, chi);
         }
-        // R-S6a: massless cell: the centre of its first child, i.e. its first particle in sorted order
-        const bool massless = M == 0.0;
-        const double* m0 = A.m64 + (size_t)fc * 13;
-        const double cm[3] = { massless ? __ldcg(m0 + 10) : s[0] / M, massless ? __ldcg(m0 + 11) : s[1] / M, massless ? __ldcg(m0 + 12) : s[2] / M };
-        double Q[6] = { 0, 0, 0, 0, 0, 0 };
-        for (int c = fc; c < fc + nc; ++c) {
-            const double* m = A.m64 + (size_t)c * 13;
-            const double Mc = __ldcg(m);
-            const double dx = __ldcg(m + 10) - cm[0], dy = __ldcg(m + 11) - cm[1], dz = __ldcg(m + 12) - cm[2];
-            const double d2 = dx * dx + dy * dy + dz * dz;
-            Q[0] += __ldcg(m + 4) + Mc * (3 * dx * dx - d2); Q[1] += __ldcg(m + 5) + Mc * (3 * dy * dy - d2); Q[2] += __ldcg(m + 6) + Mc * (3 * dz * dz - d2);
-            Q[3] += __ldcg(m + 7) + Mc * 3 * dx * dy; Q[4] += __ldcg(m + 8) + Mc * 3 * dx * dz; Q[5] += __ldcg(m + 9) + Mc * 3 * dy * dz;
-        }
-        store_node(A, k, A.nlevel[k], A.nbegin[k], A.nend[k], fc, nc, M, s, cm, Q, clo, chi);
     }
 }
 
@@ -317,23 +398,24 @@ __global__ void __launch_bounds__(NODE_THREADS) k_moments(tree_args A)
 __global__ void __launch_bounds__(NODE_THREADS) k_group_flags(tree_args A)
 {
     const int nn = A.info->n_nodes;
-    const int k = blockIdx.x * NODE_THREADS + threadIdx.x;
-    if (k == 0 && A.n <= A.ncrit) A.gflag[0] = 1;
-    if (k >= nn || A.info->node_overflow) return;
-    const int b = A.nbegin[k], e = A.nend[k];
-    if (e - b <= A.ncrit) return;
-    const int nc = A.nnchild[k];
-    if (nc == 0) {                                 // over-full leaf at the deepest level
-        for (int s = b; s < e; s += A.ncrit) A.gflag[s] = 1;
-        return;
-    }
-    const int fc = A.nfirst[k];
-    int run = -1;                                  // size of the open run, -1 = none
-    for (int c = fc; c < fc + nc; ++c) {
-        const int cb2 = A.nbegin[c], cnt = A.nend[c] - cb2;
-        if (cnt > A.ncrit) run = -1;               // that child makes its own groups
-        else if (run >= 0 && run + cnt <= A.ncrit) run += cnt;
-        else { A.gflag[cb2] = 1; run = cnt; }
+    if (blockIdx.x == 0 && threadIdx.x == 0 && A.n <= A.ncrit) A.gflag[0] = 1;
+    if (A.info->node_overflow) return;
+    for (int k = blockIdx.x * NODE_THREADS + threadIdx.x; k < nn; k += gridDim.x * NODE_THREADS) {
+        const int b = A.nbegin[k], e = A.nend[k];
+        if (e - b <= A.ncrit) continue;
+        const int nc = A.nnchild[k];
+        if (nc == 0) {                                 // over-full leaf at the deepest level
+            for (int s = b; s < e; s += A.ncrit) A.gflag[s] = 1;
+            continue;
+        }
+        const int fc = A.nfirst[k];
+        int run = -1;                                  // size of the open run, -1 = none
+        for (int c = fc; c < fc + nc; ++c) {
+            const int cb2 = A.nbegin[c], cnt = A.nend[c] - cb2;
+            if (cnt > A.ncrit) run = -1;               // that child makes its own groups
+            else if (run >= 0 && run + cnt <= A.ncrit) run += cnt;
+            else { A.gflag[cb2] = 1; run = cnt; }
+        }
     }
 }
 
@@ -434,11 +516,23 @@ int p3t_launch_tree(p3t_ctx* ctx)
     k_topo_count<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
     k_topo_scan<<<1, 32 * MAXLEV, 0, st>>>(A);
     k_topo_nodes<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
-    // one thread per cell: the cell count is only known on the device; the bound of p3t_build_tree
-    // (node_cap) sizes the grids, threads beyond n_nodes return at once
-    const int nodes_grid = (int)(((long long)ctx->node_cap + NODE_THREADS - 1) / NODE_THREADS);
+    // one thread per cell, striding: the cell count is only known on the device (about n / 4 for the paper's
+    // workloads; the hard bound node_cap is ten times that), so the grid is sized for n / 2 cells, and for the device
+    long long want = ((long long)n / 2 + NODE_THREADS - 1) / NODE_THREADS;
+    const long long full = (long long)ctx->num_sms * 16;
+    const int nodes_grid = (int)(want < 1 ? 1 : want < full ? want : full);
     k_topo_link<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
-    k_moments<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
+    {   // cooperative: every block resident (grid barriers between the levels)
+        if (!ctx->occ_moments) {
+            P3T_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->occ_moments, k_moments, MOM_THREADS, 0));
+            if (ctx->occ_moments < 1) ctx->occ_moments = 1;
+        }
+        long long mb = ((long long)n / 2 + MOM_THREADS - 1) / MOM_THREADS;
+        const long long mfull = (long long)ctx->occ_moments * ctx->num_sms;
+        const int mom_grid = (int)(mb < 1 ? 1 : mb < mfull ? mb : mfull);
+        void* args[] = { (void*)&A };
+        P3T_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_moments, dim3(mom_grid), dim3(MOM_THREADS), args, 0, st));
+    }
     k_group_flags<<<nodes_grid, NODE_THREADS, 0, st>>>(A);
     const int n16 = (n + 15) / 16, gcb = (n16 + GC_THREADS - 1) / GC_THREADS;
     k_group_count<<<gcb, GC_THREADS, 0, st>>>(A);
