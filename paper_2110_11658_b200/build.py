@@ -34,18 +34,28 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
+def build(force: bool = False, verbose: bool = False, checks: bool = False) -> Path:
+    """checks: compile with -DP3T_CHECKS (index assertions inside the kernels; profiles/r02_sanitizer.md).  A checks build is
+    always rebuilt, and so is the build that follows it."""
     srcs = [CSRC / s for s in SOURCES + DIAG_SOURCES]
     deps = srcs + HEADERS + [Path(__file__)]
+    marker = PKG / "build" / "checks.on"
+    if checks or marker.exists():
+        force = True
     if not force and LIB.exists() and DIAG_LIB.exists() and all(min(LIB.stat().st_mtime, DIAG_LIB.stat().st_mtime) >= d.stat().st_mtime for d in deps):
         return LIB
     objdir = PKG / "build"
     objdir.mkdir(exist_ok=True)
     nvcc = _nvcc()
+    flags = NVCC_FLAGS + (["-DP3T_CHECKS"] if checks else [])
+    if checks:
+        marker.write_text("built with -DP3T_CHECKS\n")
+    elif marker.exists():
+        marker.unlink()
     procs = []
     for s in srcs:
         obj = objdir / (s.stem + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-I", str(ROOT / "include"), "-I", str(CSRC), "-c", str(s), "-o", str(obj)]
+        cmd = [nvcc, *flags, "-I", str(ROOT / "include"), "-I", str(CSRC), "-c", str(s), "-o", str(obj)]
         procs.append((s, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     objs = []
     log = []
@@ -70,4 +80,4 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checks="--checks" in sys.argv))

@@ -46,6 +46,7 @@ struct force_args {
     int mode;                   // 0: the walkers run at the same time, wait for every group; 1: host repair pass
     int evalall;                // repair pass: every group again (the lists were not emitted), else only the redone ones
     long long nb_cap;           // capacity of nbraw in entries
+    long long pc_size, pp_size; // entries of the list pools (P3T_CHECKS)
     walk_consts K;
 };
 
@@ -203,7 +204,11 @@ __device__ __forceinline__ void pp_near_pass(target& T, const float (*pp)[TILE],
             if (d2 < K.rlist2) {
                 const int j = ppj[e];
                 if (T.id >= 0 && j != T.id) {                        // self excluded by index; idle lanes
-                    if (emit) A.nbraw[rowbase + atomicAdd(rowcnt, 1)] = (int32_t)A.order[j];
+                    if (emit) {
+                        const int at = atomicAdd(rowcnt, 1);
+                        P3T_CHECK(rowbase + at >= 0 && rowbase + at < A.nb_cap && rowbase + at < A.nboff[A.order[T.id] + 1]);
+                        A.nbraw[rowbase + at] = (int32_t)A.order[j];
+                    }
                     const float m = pp[3][e];
                     if (d2 >= K.rout2) {                               // buffer shell r_out <= r < r_list: on the list, wholly regular
                         const float ri = rsqrt_approx(d2), mr = m * ri, f = mr * ri * ri;
@@ -257,6 +262,7 @@ __device__ __forceinline__ int load_id(const int32_t* ids, int e, int n) { retur
 __device__ __forceinline__ pc_regs gather_pc(const force_args& A, int id)
 {
     pc_regs r;
+    P3T_CHECK(id < A.info->n_nodes);
     if (id >= 0) { r.c = A.ncom[id]; r.q0 = A.nq0[id]; r.q1 = A.nq1[id]; }
     else {                                     // padding: a zero-mass cell far away contributes exactly 0
         r.c = make_float4(FAR_AWAY, FAR_AWAY, FAR_AWAY, 0.0f); r.q0 = make_float4(0, 0, 0, 0); r.q1 = make_float2(0, 0);
@@ -272,6 +278,7 @@ __device__ __forceinline__ void store_pc(float (*pc)[TILE], int lane, const pc_r
 __device__ __forceinline__ pp_regs gather_pp(const force_args& A, int id)
 {
     pp_regs r; r.j = id;
+    P3T_CHECK(id < A.n);
     if (id >= 0) r.p = A.spm[id]; else r.p = make_float4(FAR_AWAY, FAR_AWAY, FAR_AWAY, 0.0f);
     return r;
 }
@@ -318,6 +325,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     {
         const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
         const int n = (int)rec.y, nt = (n + TILE - 1) / TILE;
+        P3T_CHECK(((long long)rec.x << 5) + (long long)nt * TILE <= A.pc_size);
         if (seg < nt) {
             pc_regs r = gather_pc(A, load_id(ids, seg * TILE + lane, n));
             int idn = load_id(ids, (seg + nseg) * TILE + lane, n);
@@ -339,6 +347,7 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     {
         const int32_t* ids = A.pppool + ((long long)rec.z << 5);
         const int n = (int)rec.w, nt = (n + TILE - 1) / TILE;
+        P3T_CHECK(((long long)rec.z << 5) + (long long)nt * TILE <= A.pp_size);
         if (seg < nt) {
             pp_regs r = gather_pp(A, load_id(ids, seg * TILE + lane, n));
             int idn = load_id(ids, (seg + nseg) * TILE + lane, n);
@@ -563,7 +572,7 @@ __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long lon
     if ((long long)info->nb_total > cap || (info->bad_input | info->node_overflow | info->stack_overflow)) return;   // nothing was emitted
     int32_t* s = s_row[LONG ? threadIdx.x >> 5 : 0];
     long long b = 0; int len = 0;
-    if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); }
+    if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); P3T_CHECK(b >= 0 && len >= 0 && b + len <= cap); }
     if (len <= 16) {
         for (int a = 0; a < len; ++a) {
             const int v = raw[b + a]; int r = 0;
@@ -644,6 +653,7 @@ static void force_fill(p3t_ctx* ctx, force_args& A, int mode, int evalall)
     make_consts(A.K, q.r_out, q.r_in, q.theta, q.pot_mode, q.r_list);
     A.vel = q.vel; A.half_dt = q.half_dt; A.mp_order = ctx->order;
     A.gready = P<int32_t>(ctx->gready); A.base = ctx->epoch; A.mode = mode; A.evalall = evalall; A.nb_cap = ctx->nb_cap;
+    A.pc_size = (long long)(ctx->pcpool.bytes / 4); A.pp_size = (long long)(ctx->pppool.bytes / 4);
     A.n = (int)ctx->n; A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
     // A problem with fewer work items (about 1.4 per 32 particles) than three per resident warp shares every item
     // among nseg warps (SPLIT), so that small N still fills the GPU.

@@ -6,6 +6,16 @@
 #include <stddef.h>
 #include "p3t.h"
 
+// -DP3T_CHECKS (python -m paper_2110_11658_b200.build --checks): index assertions inside the kernels; a failed check
+// prints the condition and traps (the call then returns P3T_ECUDA).  Stands in for compute-sanitizer's memcheck on
+// boxes where that tool is not available (profiles/r02_sanitizer.md).  Compiled out of the product build.
+#ifdef P3T_CHECKS
+#include <stdio.h>
+#define P3T_CHECK(c) do { if (!(c)) { printf("P3T_CHECK failed: %s (%s:%d)\n", #c, __FILE__, __LINE__); __trap(); } } while (0)
+#else
+#define P3T_CHECK(c) ((void)0)
+#endif
+
 #define P3T_RADIX_BITS 8
 #define P3T_RADIX      256
 #define P3T_SORT_THREADS 256

@@ -248,6 +248,7 @@ __global__ void __launch_bounds__(P3T_SORT_THREADS) k_sort_pass(const uint64_t* 
         int i = base + r * 32 + lane;
         if (i < n) {
             uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+            P3T_CHECK(s_lbase[d] + cnt[w][d] + rank[r] < (uint32_t)tile_n);
             rank[r] = (uint16_t)(s_lbase[d] + cnt[w][d] + rank[r]);        // position in the tile's sorted order
             s_buf[rank[r]] = key[r];
         }
@@ -262,6 +263,7 @@ __global__ void __launch_bounds__(P3T_SORT_THREADS) k_sort_pass(const uint64_t* 
             const uint64_t k = s_buf[e];
             const uint32_t d = (uint32_t)(k >> shift) & 255u;
             gpos[r] = s_gbase[d] + ((uint32_t)e - s_lbase[d]);
+            P3T_CHECK(gpos[r] < (uint32_t)n);
             kout[gpos[r]] = k;
         }
     }

@@ -239,6 +239,7 @@ __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-w
 __device__ void store_node(const tree_args& A, int k, int level, int b, int e, int first, int nchild,
                            double M, const double s[3], const double c[3], const double Q[6], const float clo[3], const float chi[3])
 {
+    P3T_CHECK(k >= 0 && k < A.node_cap && b >= 0 && e <= A.n && b < e);
     double* m = A.m64 + (size_t)k * 13;
     m[0] = M; m[1] = s[0]; m[2] = s[1]; m[3] = s[2];
 #pragma unroll

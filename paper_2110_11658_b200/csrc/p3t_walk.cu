@@ -40,6 +40,7 @@ struct walk_args {
     int32_t* spill;
     p3t_devinfo* info;
     float rout2, theta;
+    int n;                      // particles (P3T_CHECKS)
     int32_t* gready;            // WALK_LISTS: per-group list state (p3t_internal.cuh: G_READY ...)
     int base, repair;           // epoch of the call; repair = host repair pass (no force kernel is waiting)
     int spill_cap;              // <= SPILL_CAP (smaller only under P3T_TEST_FAULT, to exercise the overflow report)
@@ -60,6 +61,7 @@ __device__ __forceinline__ int stack_get(const warp_smem& S, const int32_t* spil
 }
 __device__ __forceinline__ void stack_put(warp_smem& S, int32_t* spill, int i, int v)
 {
+    P3T_CHECK(i >= 0 && i < STACK_CAP + SPILL_CAP);
     if (i < STACK_CAP) S.stack[i] = v; else spill[i - STACK_CAP] = v;
 }
 
@@ -117,6 +119,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
         const bool valid = lane < take;
         int node = 0;
         if (valid) node = stack_get(S, spill, top + lane);
+        P3T_CHECK(node >= 0 && node < A.info->n_nodes);
         bool open = false;
         int2 link = make_int2(0, 0);
         if (valid) {
@@ -160,6 +163,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
         // accepted cells: their ids go on the particle-cell list
         if (MODE == WALK_LISTS) {
             const uint32_t m = __ballot_sync(0xffffffffu, acc);
+            P3T_CHECK(fill_pc + __popc(m) <= 64);
             if (acc) S.pcid[fill_pc + __popc(m & lt_mask)] = node;
             fill_pc += __popc(m);
             npc += __popc(m);
@@ -188,6 +192,7 @@ __device__ void walk_group(const walk_args& A, warp_smem& S, count_smem* C, int3
             pos = min(pos, 31);
             const int j = __shfl_sync(0xffffffffu, link.x, pos) + (k - __shfl_sync(0xffffffffu, lc_excl, pos));
             if (MODE == WALK_LISTS) {
+                P3T_CHECK(fill_pp + m <= 64 && (lane >= m || (j >= 0 && j < A.n)));
                 if (lane < m) S.ppid[fill_pp + lane] = j;
                 fill_pp += m;
                 __syncwarp();
@@ -334,7 +339,7 @@ static void fill_args(p3t_ctx* ctx, walk_args& A, float r_out, float theta)
     A.cap_pc = ctx->pool_cap_pc; A.cap_pp = ctx->pool_cap_pp;
     A.spill = P<int32_t>(ctx->spill); A.info = INFO(ctx);
     volatile float ro2 = r_out * r_out;           // one fp32 product, as R10 states it
-    A.rout2 = ro2; A.theta = theta;
+    A.rout2 = ro2; A.theta = theta; A.n = (int)ctx->n;
     A.gready = P<int32_t>(ctx->gready); A.base = 0; A.repair = 0;
     A.spill_cap = (ctx->test_fault & 2) ? 0 : SPILL_CAP;
 }
