@@ -60,7 +60,7 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     const char* ev = getenv("P3T_OVERLAP");
     c->overlap = ev ? atoi(ev) != 0 : 1;
     ev = getenv("P3T_WALK_CTAS");
-    c->walk_ctas_per_sm = ev && atoi(ev) > 0 ? atoi(ev) : 1;
+    c->walk_ctas_per_sm = ev && atoi(ev) > 0 ? atoi(ev) : 2;
     ev = getenv("P3T_TEST_FAULT");                         // fault injection for the tests of the error / repair paths
     c->test_fault = ev ? atoi(ev) : 0;
     cudaError_t e = cudaSetDevice(device);
