@@ -142,3 +142,44 @@ def test_two_contexts_on_two_streams(p3t):
         torch.cuda.synchronize()
         for o in outs[1:]:
             assert torch.equal(o, outs[0])
+
+
+def test_two_host_threads_at_the_same_time(p3t):
+    """One context per host thread (include/p3t.h), both threads stepping at the same time on their own streams: only
+    one overlapped call is in flight per device and process (the other thread's call takes the serial order), nothing
+    deadlocks and every step gives the same bits as a single-threaded run."""
+    import threading
+    import torch
+    w = workloads.make_config(2, n_override=70000)
+    pm = _cuda(w.pos_mass)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(pm, 63)
+        ref = ctx.regular_force(w.r_out, w.r_in, w.theta, 0).clone()
+        roff, ridx = ctx.neighbours()
+        roff = roff.clone(); ridx = ridx.clone()
+    torch.cuda.synchronize()
+    errors = []
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                out = torch.empty((w.n, 4), dtype=torch.float32, device="cuda")
+            with p3t.Context(0, stream=st) as c:
+                for _ in range(12):
+                    c.build_tree(pm, 63)
+                    c.regular_force(w.r_out, w.r_in, w.theta, 0, out=out)
+                    off, idx = c.neighbours()
+                    if not (torch.equal(out, ref) and torch.equal(off, roff) and torch.equal(idx, ridx)):
+                        errors.append(f"thread {k}: result differs")
+        except Exception as e:                              # noqa: BLE001 - reported by the main thread
+            errors.append(f"thread {k}: {e!r}")
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+        assert not t.is_alive(), "a thread hangs"
+    assert not errors, errors
