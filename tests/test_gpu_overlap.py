@@ -183,3 +183,24 @@ def test_two_host_threads_at_the_same_time(p3t):
         t.join(timeout=300)
         assert not t.is_alive(), "a thread hangs"
     assert not errors, errors
+
+
+def test_step_host_as_first_call_with_repair(p3t):
+    """p3t_step_host as the very first call of a context, on a dense King core whose neighbour total outgrows the first guess
+    of the index capacity: the repair pass runs inside the call and the host buffers hold the final results."""
+    w = workloads.make_config(4, n_override=50000)
+    w.r_out = 0.06; w.r_in = 0.006
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        a = ctx.regular_force(w.r_out, w.r_in, w.theta).cpu().numpy()
+        a = ctx.regular_force(w.r_out, w.r_in, w.theta).cpu().numpy()
+        off, idx = ctx.neighbours()
+        off = off.cpu().numpy(); idx = idx.cpu().numpy()
+    assert idx.shape[0] > (1 << 20) + (1 << 18)
+    nb_off = np.empty(w.n + 1, dtype=np.int64); nb_idx = np.empty(idx.shape[0] + 10, dtype=np.int32)
+    with p3t.Context(0) as ctx:
+        acc, _, _, total = ctx.step_host(w.pos_mass, w.r_out, w.r_in, w.theta, nb_offsets=nb_off, nb_indices=nb_idx)
+        assert total == idx.shape[0]
+        assert np.array_equal(acc, a) and np.array_equal(nb_off, off) and np.array_equal(nb_idx[:total], idx)
+        acc2, _, _, total2 = ctx.step_host(w.pos_mass, w.r_out, w.r_in, w.theta, nb_offsets=nb_off, nb_indices=nb_idx)
+        assert total2 == total and np.array_equal(acc2, a) and np.array_equal(nb_idx[:total], idx)
