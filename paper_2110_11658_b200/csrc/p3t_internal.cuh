@@ -23,7 +23,7 @@
 #define P3T_SORT_ITEMS_BIG 16
 #define P3T_SORT_TILE_MIN  (P3T_SORT_THREADS * P3T_SORT_ITEMS_MIN) // the smallest tile sizes the histogram buffer
 
-// device-side counters written by the build and force kernels (one 256-byte record)
+// device-side counters written by the build and force kernels (one small record)
 struct p3t_devinfo {
     float    lo[3];          // bounding cube, R-S1
     float    side;
@@ -48,6 +48,8 @@ struct p3t_devinfo {
     int32_t  shard_g0, shard_g1; // target groups of this context's shard (all groups unless p3t_set_shard)
     int32_t  nb_overflow;    // the neighbour total exceeds the capacity of the index buffers: nothing was emitted (repaired by the host)
     int32_t  spin_abort;     // a force warp waited too long for a group's lists (no co-resident walker): those groups are repaired
+    int32_t  topo_done;      // k_topo_scan: blocks (levels) that have finished their row
+    int32_t  level_tot[24];  // k_topo_scan: cells per level
 };
 
 // State of a target group's interaction lists in p3t_ctx::gready, relative to the call's epoch `base` (values of older

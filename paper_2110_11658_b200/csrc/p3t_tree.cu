@@ -81,7 +81,12 @@ __global__ void __launch_bounds__(TOPO_THREADS) k_topo_count(tree_args A)
         lam = min(P + 1, A.B);
         A.pcl[i] = (int8_t)cl; A.plam[i] = (int8_t)lam;
     }
-    for (int l = 1; l <= A.B; ++l) {
+    // only the levels at which some particle of the warp starts a cell (a handful around the leaf level of the
+    // neighbourhood, not all 21): the others keep their zero
+    if (lane < MAXLEV) s_cnt[w][lane] = 0;
+    const int l_lo = max(1, __reduce_min_sync(0xffffffffu, cl + 1)), l_hi = min(A.B, __reduce_max_sync(0xffffffffu, lam));
+    __syncwarp();
+    for (int l = l_lo; l <= l_hi; ++l) {
         const uint32_t m = __ballot_sync(0xffffffffu, cl < l && l <= lam);
         if (lane == 0) s_cnt[w][l] = __popc(m);
     }
@@ -94,37 +99,48 @@ __global__ void __launch_bounds__(TOPO_THREADS) k_topo_count(tree_args A)
     }
 }
 
-// ---------------- a4, pass 2: exclusive prefix over the blocks, one warp per level ----------------
-__global__ void __launch_bounds__(32 * MAXLEV) k_topo_scan(tree_args A)
+// ---------------- a4, pass 2: exclusive prefix over the blocks, one block per level ----------------
+#define TSCAN_THREADS 1024
+__global__ void __launch_bounds__(TSCAN_THREADS) k_topo_scan(tree_args A)
 {
-    __shared__ int s_tot[MAXLEV];
-    const int lane = threadIdx.x & 31, l = threadIdx.x >> 5;
-    if (l >= 1 && l <= A.B) {
-        int32_t* row = A.blksum + (size_t)l * A.nblk;
-        int run = 0;
-        for (int b0 = 0; b0 < A.nblk; b0 += 256) {           // eight loads in flight per lane: the row is read in a few round trips
-            int v[8];
+    __shared__ int s_w[TSCAN_THREADS / 32];
+    __shared__ int s_run;
+    __shared__ int s_last;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, l = blockIdx.x + 1;       // levels 1 .. B
+    int32_t* row = A.blksum + (size_t)l * A.nblk;
+    if (threadIdx.x == 0) s_run = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < A.nblk; b0 += TSCAN_THREADS) {
+        const int b = b0 + threadIdx.x;
+        const int v = b < A.nblk ? row[b] : 0;
+        int x = v;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) { const int b = b0 + 32 * j + lane; v[j] = b < A.nblk ? row[b] : 0; }
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        if (lane == 31) s_w[w] = x;
+        __syncthreads();
+        int add = s_run, tot = 0;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int b = b0 + 32 * j + lane;
-                int x = v[j];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-                if (b < A.nblk) row[b] = run + x - v[j];
-                run += __shfl_sync(0xffffffffu, x, 31);
-            }
-        }
-        if (lane == 0) s_tot[l] = run;
+        for (int k = 0; k < TSCAN_THREADS / 32; ++k) { const int t = s_w[k]; if (k < w) add += t; tot += t; }
+        if (b < A.nblk) row[b] = add + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) s_run += tot;
+        __syncthreads();
+    }
+    // the last level to finish turns the totals into the level offsets
+    if (threadIdx.x == 0) {
+        A.info->level_tot[l] = s_run;
+        __threadfence();
+        s_last = atomicAdd(&A.info->topo_done, 1) == (int)gridDim.x - 1;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
         int off = 1, maxl = 0;                    // the root is cell 0
         A.info->level_begin[0] = 0; A.info->level_begin[1] = 1;
         for (int k = 1; k <= A.B; ++k) {
-            if (s_tot[k] > 0) maxl = k;
-            off += s_tot[k];
+            const int t = *(volatile int32_t*)&A.info->level_tot[k];
+            if (t > 0) maxl = k;
+            off += t;
             A.info->level_begin[k + 1 < 24 ? k + 1 : 23] = off;
         }
         for (int k = A.B + 2; k < 24; ++k) A.info->level_begin[k] = off;
@@ -144,11 +160,13 @@ __global__ void __launch_bounds__(TOPO_THREADS) k_topo_nodes(tree_args A)
     if (i < A.n) { cl = A.pcl[i]; lam = A.plam[i]; }
     const int* __restrict__ lb = A.info->level_begin;
     if (A.info->node_overflow) return;
-    for (int l = 1; l <= A.B; ++l) {
+    if (lane <= MAXLEV) s_cnt[w][lane] = 0;
+    const int l_lo = max(1, __reduce_min_sync(0xffffffffu, cl + 1)), l_hi = min(A.B, __reduce_max_sync(0xffffffffu, lam));
+    __syncwarp();
+    for (int l = l_lo; l <= l_hi; ++l) {                 // the levels at which the warp starts cells (see k_topo_count)
         const uint32_t m = __ballot_sync(0xffffffffu, cl < l && l <= lam);
         if (lane == 0) s_cnt[w][l] = __popc(m);
     }
-    if (lane == 0) s_cnt[w][0] = 0;
     __syncthreads();
     if (tid <= A.B) {
         int run = tid == 0 ? 0 : A.blksum[(size_t)tid * A.nblk + blockIdx.x];
@@ -158,13 +176,14 @@ __global__ void __launch_bounds__(TOPO_THREADS) k_topo_nodes(tree_args A)
     __syncthreads();
     // rank of particle i among the starters of level l = s_cnt[w][l] + popc(ballot_l & lanes below);
     // level 0 has the single starter (0, 0)
-    uint32_t m_prev = 0, m_cur = __ballot_sync(0xffffffffu, cl < 1 && 1 <= lam);
-    int r_prev = i > 0 ? 1 : 0;                  // starters of level 0 before i
     if (i == 0) {                                // the root
         A.nlevel[0] = 0; A.nbegin[0] = 0; A.nparent[0] = -1;
         A.nfc[0] = 1;                            // rank 0 among the level-1 starters
     }
-    for (int l = 1; l <= A.B; ++l) {
+    uint32_t m_prev = 0, m_cur = __ballot_sync(0xffffffffu, cl < l_lo && l_lo <= lam);
+    // starters of level l_lo - 1 before i: none of them is in this warp (level 0: the root, before everybody but i = 0)
+    int r_prev = l_lo == 1 ? (i > 0 ? 1 : 0) : s_cnt[w][l_lo - 1];
+    for (int l = l_lo; l <= l_hi; ++l) {
         const uint32_t m_next = l < A.B ? __ballot_sync(0xffffffffu, cl < l + 1 && l + 1 <= lam) : 0u;
         const int r_cur = s_cnt[w][l] + __popc(m_cur & lt_mask);
         if (cl < l && l <= lam) {
@@ -515,7 +534,7 @@ int p3t_launch_tree(p3t_ctx* ctx)
     cudaStream_t st = ctx->stream;
     P3T_CUDA(ctx, cudaMemsetAsync(ctx->gflag.p, 0, (size_t)n + 32, st));
     k_topo_count<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
-    k_topo_scan<<<1, 32 * MAXLEV, 0, st>>>(A);
+    k_topo_scan<<<A.B, TSCAN_THREADS, 0, st>>>(A);
     k_topo_nodes<<<A.nblk, TOPO_THREADS, 0, st>>>(A);
     // one thread per cell, striding: the cell count is only known on the device (about n / 4 for the paper's
     // workloads; the hard bound node_cap is ten times that), so the grid is sized for n / 2 cells, and for the device
