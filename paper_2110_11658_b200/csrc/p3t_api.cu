@@ -155,7 +155,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     RES(keys[0], N * 8); RES(keys[1], N * 8); RES(idx[0], N * 4); RES(idx[1], N * 4); RES(spm, N * 16); RES(rank, N * 4);
     RES(hist, p3t_sort_scratch_bytes(n));
     RES(nlevel, C * 4); RES(nbegin, C * 4); RES(nend, C * 4); RES(nfirst, C * 4); RES(nnchild, C * 4);
-    RES(m64, C * 104);
+    RES(m64, C * 8 * M64_STRIDE);
     RES(ncom, C * 16); RES(nlo, C * 16); RES(nhi, C * 16); RES(nq0, C * 16); RES(nq1, C * 8); RES(nlink, C * 8);
     RES(scan_tmp, (size_t)22 * ((N + 255) / 256) * 4 + 64); RES(pcl, N + 64); RES(plam, N + 64);
     RES(nparent, C * 4); RES(nfc, C * 4); RES(ncount, C * 4); RES(gsum, ((N + 4095) / 4096 + 1) * 4);

@@ -573,11 +573,18 @@ __global__ void __launch_bounds__(SORTROWS_THREADS) k_nb_sortrows(const long lon
     int32_t* s = s_row[LONG ? threadIdx.x >> 5 : 0];
     long long b = 0; int len = 0;
     if (i < n) { b = off[i]; len = (int)(off[i + 1] - b); P3T_CHECK(b >= 0 && len >= 0 && b + len <= cap); }
-    if (len <= 16) {
-        for (int a = 0; a < len; ++a) {
-            const int v = raw[b + a]; int r = 0;
-            for (int c = 0; c < len; ++c) r += raw[b + c] < v;
-            idx[b + r] = v;
+    if (len <= 16) {                              // the row in registers: one load per entry, then the quadratic rank
+        int v[16];
+#pragma unroll
+        for (int a = 0; a < 16; ++a) v[a] = a < len ? raw[b + a] : 0x7fffffff;
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {
+            if (a < len) {
+                int r = 0;
+#pragma unroll
+                for (int c = 0; c < 16; ++c) r += v[c] < v[a];
+                idx[b + r] = v[a];
+            }
         }
     }
     uint32_t m = __ballot_sync(0xffffffffu, len > 16);

@@ -16,6 +16,7 @@
 #define P3T_CHECK(c) ((void)0)
 #endif
 
+#define M64_STRIDE 14                                         // doubles per cell in m64: M, sum m x (3), Q (6), COM (3), first key (bits)
 #define P3T_RADIX_BITS 8
 #define P3T_RADIX      256
 #define P3T_SORT_THREADS 256
@@ -50,6 +51,7 @@ struct p3t_devinfo {
     int32_t  spin_abort;     // a force warp waited too long for a group's lists (no co-resident walker): those groups are repaired
     int32_t  topo_done;      // k_topo_scan: blocks (levels) that have finished their row
     int32_t  level_tot[24];  // k_topo_scan: cells per level
+    uint32_t grid_bar;       // k_moments: arrivals at its grid barrier (monotone; the record is cleared per build)
 };
 
 // State of a target group's interaction lists in p3t_ctx::gready, relative to the call's epoch `base` (values of older
@@ -89,7 +91,7 @@ struct p3t_ctx {
     p3t_buf rank;                    // int32: original id -> sorted position
     p3t_buf hist;                    // sort: per-block digit counts
     p3t_buf nlevel, nbegin, nend, nfirst, nnchild;        // int32 per node
-    p3t_buf m64;                     // double[13] per node: M, sum m x [3], Q[6], COM[3]
+    p3t_buf m64;                     // double[M64_STRIDE] per node: M, sum m x [3], Q[6], COM[3], first key
     p3t_buf ncom, nlo, nhi, nq0, nq1, nlink;              // walk SoA (see p3t_tree.cu)
     p3t_buf scan_tmp;                // tree build: starters per level and block [22][blocks]
     p3t_buf pcl, plam;               // int8 per particle: cl(i), lam(i) (p3t_tree.cu)

@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupoles(oct_args A)
     int k = blockIdx.x * OCT_THREADS + threadIdx.x;
     if (k >= nn || A.info->node_overflow || A.nnchild[k] != 0) return;
     {
-        const double* mk = A.m64 + (size_t)k * 13;
+        const double* mk = A.m64 + (size_t)k * M64_STRIDE;
         const double c[3] = { mk[10], mk[11], mk[12] };
         double tr = 0.0, T[10] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
         for (int i = A.nbegin[k]; i < A.nend[k]; ++i) {
@@ -69,14 +69,14 @@ __global__ void __launch_bounds__(OCT_THREADS) k_octupoles(oct_args A)
         if (atomicAdd(&A.cnt[p], 1) + 1 < A.nnchild[p]) break;
         __threadfence();
         k = p;
-        const double* mk = A.m64 + (size_t)k * 13;
+        const double* mk = A.m64 + (size_t)k * M64_STRIDE;
         const double cm[3] = { mk[10], mk[11], mk[12] };
         double tr = 0.0, T[10] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
         const int fc = A.nfirst[k], nc = A.nnchild[k];
         for (int c = fc; c < fc + nc; ++c) {
             // parallel-axis rule, s = COM_c - COM: T_abc += T^c_abc + s_a S_bc + s_b S_ac + s_c S_ab + M_c s_a s_b s_c,
             // S = raw second moment of the child about its own COM = (Q + tr(S) 1) / 3
-            const double* m = A.m64 + (size_t)c * 13;
+            const double* m = A.m64 + (size_t)c * M64_STRIDE;
             const double* o = A.o64 + (size_t)c * 11;
             const double Mc = m[0], sx = m[10] - cm[0], sy = m[11] - cm[1], sz = m[12] - cm[2];
             const double trc = __ldcg(o);

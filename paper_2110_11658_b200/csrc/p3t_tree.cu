@@ -255,17 +255,19 @@ __device__ __forceinline__ uint32_t compact3(uint64_t x)   // inverse of the 3-w
 }
 
 // R-S6 output of one cell: fp32 rounding of the fp64 moments, delta, and the walk's link word
-__device__ void store_node(const tree_args& A, int k, int level, int b, int e, int first, int nchild,
+// key0 = Morton key of the cell's first particle (a leaf reads it, a parent takes its first child's: no dependent load)
+__device__ void store_node(const tree_args& A, int k, int level, int b, int e, int first, int nchild, uint64_t key0,
                            double M, const double s[3], const double c[3], const double Q[6], const float clo[3], const float chi[3])
 {
     P3T_CHECK(k >= 0 && k < A.node_cap && b >= 0 && e <= A.n && b < e);
-    double* m = A.m64 + (size_t)k * 13;
+    double* m = A.m64 + (size_t)k * M64_STRIDE;
     m[0] = M; m[1] = s[0]; m[2] = s[1]; m[3] = s[2];
 #pragma unroll
     for (int q = 0; q < 6; ++q) m[4 + q] = Q[q];
     m[10] = c[0]; m[11] = c[1]; m[12] = c[2];       // the parent reads the quotient instead of dividing again (same bits)
+    m[13] = __longlong_as_double((long long)key0);
     // geometric centre from the integer cell coordinates (prefix of the first key)
-    const uint64_t prefix = level == 0 ? 0ull : (A.keys[b] >> (3 * (A.B - level)));
+    const uint64_t prefix = level == 0 ? 0ull : (key0 >> (3 * (A.B - level)));
     const uint32_t p3[3] = { compact3(prefix >> 2), compact3(prefix >> 1), compact3(prefix) };
     const double l = (double)A.info->side / (double)(1ull << level);
     double dd = 0.0;
@@ -297,6 +299,18 @@ __device__ __forceinline__ double shfl_xor_f64(double v, int o)
     lo = __shfl_xor_sync(0xffffffffu, lo, o); hi = __shfl_xor_sync(0xffffffffu, hi, o);
     return __hiloint2double(hi, lo);
 }
+__device__ __forceinline__ double shfl_up_f64(double v, int o)
+{
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_up_sync(0xffffffffu, lo, o); hi = __shfl_up_sync(0xffffffffu, hi, o);
+    return __hiloint2double(hi, lo);
+}
+__device__ __forceinline__ double shfl_idx_f64(double v, int src)
+{
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_sync(0xffffffffu, lo, src); hi = __shfl_sync(0xffffffffu, hi, src);
+    return __hiloint2double(hi, lo);
+}
 __device__ __forceinline__ double seg8_sum(double v)
 {
     v += shfl_xor_f64(v, 1); v += shfl_xor_f64(v, 2); v += shfl_xor_f64(v, 4);
@@ -317,6 +331,7 @@ __device__ void leaf_moments(const tree_args& A, int k)
 {
     const int b = A.nbegin[k], e = A.nend[k];
     double M = 0.0, s[3] = { 0.0, 0.0, 0.0 };
+    const uint64_t key0 = A.keys[b];
     const float4 p0 = A.spm[b];
     float clo[3] = { p0.x, p0.y, p0.z }, chi[3] = { p0.x, p0.y, p0.z };
     for (int i0 = b; i0 < e; i0 += 4) {                     // four loads in flight; summed in particle order
@@ -351,54 +366,102 @@ __device__ void leaf_moments(const tree_args& A, int k)
             Q[3] += m * 3 * dx * dy; Q[4] += m * 3 * dx * dz; Q[5] += m * 3 * dy * dz;
         }
     }
-    store_node(A, k, A.nlevel[k], b, e, -1, 0, M, s, c, Q, clo, chi);
+    store_node(A, k, A.nlevel[k], b, e, -1, 0, key0, M, s, c, Q, clo, chi);
+}
+
+// Grid barrier of k_moments (the launch is cooperative, so every block is resident): one monotone arrival counter;
+// cooperative_groups' grid.sync() measured 8.8 us per barrier here (444 blocks), 75 % of the kernel.  Writes of the level
+// below are fenced before the arrival and read past L1 (__ldcg) after it.
+__device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t nblocks)
+{
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t arrived = atomicAdd(bar, 1u) + 1u;
+        const uint32_t target = (arrived + nblocks - 1u) / nblocks * nblocks;      // end of this round
+        while (*(volatile uint32_t*)bar < target) { }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
 #define MOM_THREADS 256
 __global__ void __launch_bounds__(MOM_THREADS) k_moments(tree_args A)
 {
-    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const int nn = A.info->n_nodes;
     if (A.info->node_overflow) return;                       // uniform over the grid: nobody reaches a barrier
     const int gtid = blockIdx.x * MOM_THREADS + threadIdx.x, gsize = gridDim.x * MOM_THREADS;
     for (int k = gtid; k < nn; k += gsize)
         if (A.nnchild[k] == 0) leaf_moments(A, k);
-    const int* __restrict__ lb = A.info->level_begin;
-    const int lane = threadIdx.x & 31, seg = lane >> 3, j = lane & 7;
+    __shared__ int lb[24];                                       // level offsets: read once (a dependent load per level otherwise)
+    if (threadIdx.x < 24) lb[threadIdx.x] = A.info->level_begin[threadIdx.x];
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
     const int gwarp = gtid >> 5, nwarps = gsize >> 5;
-    for (int l = A.info->max_level - 1; l >= 0; --l) {
-        grid.sync();
-        const int k_end = lb[l + 1];
-        for (int k4 = lb[l] + 4 * gwarp; k4 < k_end; k4 += 4 * nwarps) {          // warp-uniform trip count: four cells per warp
-            const int k = k4 + seg;
-            int nc = 0, fc = 0;
-            if (k < k_end) { nc = A.nnchild[k]; fc = A.nfirst[k]; }
-            const bool have = j < nc;
-            // this lane's child (read past L1: another SM wrote it in this launch)
-            double cM = 0.0, cs[3] = { 0, 0, 0 }, cQ[6] = { 0, 0, 0, 0, 0, 0 }, cc[3] = { 0, 0, 0 };
+    const int max_level = A.info->max_level;
+    // Level l from level l + 1: the children of a cell are consecutive cells of the next level, so a warp takes a window
+    // of 32 consecutive CHILDREN (coalesced loads of their fp64 records, no search for the internal cells among the leaves)
+    // and sums every run of siblings by a segmented scan over the lanes (runs are at most 8 long: distances 1, 2, 4).
+    // Windows advance by 25 = 32 - 7, so every run lies wholly inside the window in which its first child is among the
+    // first 25 lanes: that window, and only that one, stores the parent.
+    for (int l = max_level - 1; l >= 0; --l) {
+        grid_barrier(&A.info->grid_bar, gridDim.x);
+        const int c_begin = lb[l + 1], c_end = lb[l + 2 < 24 ? l + 2 : 23];
+        for (int c0 = c_begin + 25 * gwarp; c0 < c_end; c0 += 25 * nwarps) {
+            const int c = c0 + lane;
+            const bool have = c < c_end;
+            int p = -1 - lane, p_before = -1, cb = 0, ce = 0;    // inactive lanes: all different, never equal to a cell
+            double cM = 0.0, cs[3] = { 0, 0, 0 }, cQ[6] = { 0, 0, 0, 0, 0, 0 }, cc[3] = { 0, 0, 0 }, ckey = 0.0;
             float lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
             if (have) {
-                const double* m = A.m64 + (size_t)(fc + j) * 13;
+                p = A.nparent[c];
+                if (lane == 0 && c > c_begin) p_before = A.nparent[c - 1];     // does a run start at lane 0, or continue?
+                cb = A.nbegin[c]; ce = A.nend[c];
+                const double* m = A.m64 + (size_t)c * M64_STRIDE;  // read past L1: another SM wrote it in this launch
+                ckey = __ldcg(m + 13);
                 cM = __ldcg(m); cs[0] = __ldcg(m + 1); cs[1] = __ldcg(m + 2); cs[2] = __ldcg(m + 3);
 #pragma unroll
                 for (int q = 0; q < 6; ++q) cQ[q] = __ldcg(m + 4 + q);
                 cc[0] = __ldcg(m + 10); cc[1] = __ldcg(m + 11); cc[2] = __ldcg(m + 12);
-                const float4 l4 = __ldcg(&A.nlo[fc + j]), h4 = __ldcg(&A.nhi[fc + j]);
+                const float4 l4 = __ldcg(&A.nlo[c]), h4 = __ldcg(&A.nhi[c]);
                 lo[0] = l4.x; lo[1] = l4.y; lo[2] = l4.z; hi[0] = h4.x; hi[1] = h4.y; hi[2] = h4.z;
             }
-            const double M = seg8_sum(cM);
-            double s[3] = { seg8_sum(cs[0]), seg8_sum(cs[1]), seg8_sum(cs[2]) };
+            // run structure: same[o] = the lane o below belongs to the same parent
+            bool same[3];
+#pragma unroll
+            for (int t = 0; t < 3; ++t) { const int q = __shfl_up_sync(0xffffffffu, p, 1 << t); same[t] = lane >= (1 << t) && q == p; }
+            const bool head = !same[0];
+            const int p_next = __shfl_down_sync(0xffffffffu, p, 1);             // every lane takes part (no short-circuit around it)
+            const uint32_t lastmask = __ballot_sync(0xffffffffu, lane == 31 || p_next != p);
+            const int run_end = lane + __ffs(lastmask >> lane) - 1;               // last lane of this lane's run
+            const int run_head = 31 - __clz(__ballot_sync(0xffffffffu, head) & ((2u << lane) - 1u));
+            auto seg_sum = [&](double x) {
+#pragma unroll
+                for (int t = 0; t < 3; ++t) { const double y = shfl_up_f64(x, 1 << t); if (same[t]) x += y; }
+                return shfl_idx_f64(x, run_end);
+            };
+            auto seg_min = [&](float x) {
+#pragma unroll
+                for (int t = 0; t < 3; ++t) { const float y = __shfl_up_sync(0xffffffffu, x, 1 << t); if (same[t]) x = fminf(x, y); }
+                return __shfl_sync(0xffffffffu, x, run_end);
+            };
+            auto seg_max = [&](float x) {
+#pragma unroll
+                for (int t = 0; t < 3; ++t) { const float y = __shfl_up_sync(0xffffffffu, x, 1 << t); if (same[t]) x = fmaxf(x, y); }
+                return __shfl_sync(0xffffffffu, x, run_end);
+            };
+            const double M = seg_sum(cM);
+            double s[3] = { seg_sum(cs[0]), seg_sum(cs[1]), seg_sum(cs[2]) };
             float clo[3], chi[3];
 #pragma unroll
-            for (int a = 0; a < 3; ++a) { clo[a] = seg8_min(lo[a]); chi[a] = seg8_max(hi[a]); }
+            for (int a = 0; a < 3; ++a) { clo[a] = seg_min(lo[a]); chi[a] = seg_max(hi[a]); }
             // R-S6a: massless cell: the centre of its first child, i.e. its first particle in sorted order
             const bool massless = M == 0.0;
             double cm[3];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                const int first = lane & ~7;                                       // lane of the first child
-                int l0 = __shfl_sync(0xffffffffu, __double2loint(cc[a]), first), h0 = __shfl_sync(0xffffffffu, __double2hiint(cc[a]), first);
-                cm[a] = massless ? __hiloint2double(h0, l0) : s[a] / M;
+                const double first = shfl_idx_f64(cc[a], run_head);
+                cm[a] = massless ? first : s[a] / M;
             }
             double Q[6];
             {
@@ -407,9 +470,13 @@ __global__ void __launch_bounds__(MOM_THREADS) k_moments(tree_args A)
                 const double t[6] = { cQ[0] + cM * (3 * dx * dx - d2), cQ[1] + cM * (3 * dy * dy - d2), cQ[2] + cM * (3 * dz * dz - d2),
                                       cQ[3] + cM * 3 * dx * dy, cQ[4] + cM * 3 * dx * dz, cQ[5] + cM * 3 * dy * dz };
 #pragma unroll
-                for (int q = 0; q < 6; ++q) Q[q] = seg8_sum(have ? t[q] : 0.0);
+                for (int q = 0; q < 6; ++q) Q[q] = seg_sum(have ? t[q] : 0.0);
             }
-            if (j == 0 && nc > 0) store_node(A, k, l, A.nbegin[k], A.nend[k], fc, nc, M, s, cm, Q, clo, chi);
+            // the run's first lane stores the parent, if the run starts here (lane 0 may hold the tail of a run of the
+            // previous window) and among the first 25 lanes
+            const int e_run = __shfl_sync(0xffffffffu, ce, run_end);              // the parent's range: first child's begin .. last child's end
+            if (have && head && lane < 25 && p_before != p)
+                store_node(A, p, l, cb, e_run, c, run_end - lane + 1, (uint64_t)__double_as_longlong(ckey), M, s, cm, Q, clo, chi);
         }
     }
 }
