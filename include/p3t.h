@@ -65,9 +65,9 @@ typedef struct p3t_stats {
     float   cube_side;
     float   ms_build;        /* CUDA-event time of the last p3t_build_tree (a1-a6)      */
     float   ms_force;        /* CUDA-event time of the last p3t_regular_force (a7-a11)  */
-    float   ms_walk;         /* ... of its list-building tree walk kernel (a7) alone    */
+    float   ms_walk;         /* ... of its list-building tree walk kernel (a7), which runs beside the force kernel */
     float   ms_sort;         /* ... of the radix sort inside the last build             */
-    float   ms_eval;         /* ... of the force kernel (a8, a9, a11) alone             */
+    float   ms_eval;         /* ... of the force kernel (a8, a9, a11), first launch to the end of the second */
     float   ms_count;        /* ... of the neighbour count walk + offset scan (a10)     */
     float   ms_irregular;    /* ... of the last p3t_irregular_force kernel (0 if none)  */
     float   ms_core;         /* ... of the last p3t_core_quantities kernels (0 if none)  */

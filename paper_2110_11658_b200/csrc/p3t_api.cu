@@ -283,7 +283,7 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         (void)cudaEventElapsedTime(&out->ms_force, c->ev[4], c->ev[5]);
         (void)cudaEventElapsedTime(&out->ms_eval, c->evw[0], c->evw[1]);
         (void)cudaEventElapsedTime(&out->ms_walk, c->evw[2], c->evw[3]);
-        (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->evw[2]);
+        if (c->walk_stream) (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->ev_scan);
         if (c->irr_done) (void)cudaEventElapsedTime(&out->ms_irregular, c->evi[0], c->evi[1]);
         if (c->order == 3) (void)cudaEventElapsedTime(&out->ms_octupole, c->evo[0], c->evo[1]);
     }

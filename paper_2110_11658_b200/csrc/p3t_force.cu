@@ -643,7 +643,7 @@ static int force_streams(p3t_ctx* ctx)
     if (ctx->walk_stream) return P3T_OK;
     P3T_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->walk_stream, cudaStreamNonBlocking));
     P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_tree, cudaEventDisableTiming));
-    P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_scan, cudaEventDisableTiming));
+    P3T_CUDA(ctx, cudaEventCreate(&ctx->ev_scan));                 // also the end of the count phase (p3t_stats::ms_count)
     P3T_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_wdone, cudaEventDisableTiming));
     return P3T_OK;
 }

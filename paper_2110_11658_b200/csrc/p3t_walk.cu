@@ -13,9 +13,10 @@
 // Why the lists go through HBM on B200: the walk is a serial, latency-bound pointer chase that
 // needs few registers and many resident warps; the force evaluation is an FP32-pipe-bound stream
 // that needs many registers.  Fused in one kernel (this library's first version) the two phases of
-// a warp alternate and the FP32 pipe idles for 30-40 % of the time (profiles/r01_*).  Writing
+// a warp alternate and the FP32 pipe idles for 30-40 % of the time (profiles/r01b_force_walk_full_config3.md).  Writing
 // 4 bytes per interaction-list entry costs 0.57 GB of HBM traffic at N = 2^20 (< 0.2 ms at the
-// measured 6.5 TB/s) and lets either kernel run at its own occupancy.
+// measured 6.5 TB/s) and lets either kernel run with its own register budget -- side by side on every SM: k_walk<WALK_LISTS>
+// runs on its own stream while the force kernel evaluates the groups it has already published (p3t_force.cu).
 // The paper gives no detail of this stage ("the BONSAI library").
 #include "p3t_internal.cuh"
 #include "p3t_f32x2.cuh"
