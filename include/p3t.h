@@ -203,6 +203,55 @@ int p3t_step_host(p3t_ctx* ctx, int64_t n, const float* pos_mass_host, int key_b
                   float* acc_pot_host, int64_t* nb_offsets_host, int32_t* nb_indices_host,
                   int64_t nb_cap, int64_t* nb_total);
 
+/* Steps a1-a3 (bounding cube, Morton keys, stable radix sort: the same kernels and rules as p3t_build_tree,
+ * "the BONSAI library" of PAPER.md:117-119) for callers that must not allocate device memory.
+ *
+ * Who that is.  Every other call of this library takes a p3t_ctx, and a context gets its scratch from cudaMalloc
+ * (p3t_create, then grow-only).  Some hosts of an N-body integrator cannot afford that: a code that has handed
+ * the whole device to its own arena or to a framework's caching allocator has nothing left for the runtime to
+ * hand out; a regular-step loop that also runs an irregular-force stream does not want cudaMalloc / cudaFree in
+ * it, because both stall every stream of the device while they run; and a plug-in loaded into a process under a
+ * fixed device-memory quota may simply be forbidden to grow.  Such a caller can still get the Morton order of its
+ * particles (to reorder its own arrays for locality, or to feed its own tree) from this one call: it needs no
+ * context and calls no cudaMalloc, cudaFree or other allocating routine, at the first call or any later one.
+ *
+ * How.  The scratch the sort needs (its digit totals, tile tickets and look-back words, the cube record and the
+ * second buffer of the key / index ping-pong) lives in ONE fixed array inside the library image, 3 678 976 bytes
+ * (P3T_STATIC_SCRATCH_BYTES), sized for P3T_STATIC_MAX_N = 262 144 particles (the paper's own range, N = 32k ...
+ * 256k).  Every GPU on which the process uses this library holds that array from the moment the
+ * library's code is loaded on it until the process exits, whether or not this call is ever made.
+ *
+ *   pos_mass     DEVICE, n x {x, y, z, m} fp32, 16-byte aligned, read-only           (input)
+ *   sorted_keys  DEVICE uint64[n]: the Morton keys in ascending order                (output; also used as the
+ *   order        DEVICE uint32[n]: sorted position -> original id, ties keep           first ping-pong buffer, so
+ *                original order (stable)                                               both are required)
+ *   cube         DEVICE float[4] = {lo_x, lo_y, lo_z, side} of the bounding cube      (output, may be NULL)
+ *   bad_input    DEVICE int32[1]: 1 if a position or mass is NaN / Inf or a mass       (output, may be NULL)
+ *                is negative (keys and order are then unspecified), else 0
+ * Results equal, bit for bit, p3t_get_keys / p3t_stats::cube_* after p3t_build_tree on the same input.
+ *
+ * device / cuda_stream: as in p3t_create (the call makes `device` current, like every call of the library, and
+ * enqueues on that stream; it does NOT synchronise).  All pointers must belong to `device`.
+ *
+ * First call on a device: the call looks up the device address of the array (cudaGetSymbolAddress) and the SM
+ * count, once per device, and keeps them.  That set-up does not allocate, but it is not stream work: make the
+ * first call on each device from ordinary host code, before any stream capture that is to contain later calls.
+ *
+ * Sharing: all calls on a device use the same array, and it keeps what the last call left there.  The call
+ * clears, on the stream, the part that has to start at zero, so calls that follow one another on ONE stream (or
+ * are ordered by events) are independent of each other.  Two calls whose GPU work overlaps -- different streams
+ * without an event between them, or two host threads -- race on the array and return garbage; ordering them is
+ * the caller's job.  The set-up itself is safe to race (it is serialised inside the library).
+ *
+ * Errors: P3T_EINVAL for a null or misaligned pointer, n < 1, key_bits not 30 / 63, or an unknown device;
+ * P3T_ELIMIT for n > P3T_STATIC_MAX_N (nothing is enqueued; use a context, which has no such limit);
+ * P3T_ECUDA if a CUDA call fails (no context, hence no p3t_last_error text: cudaGetLastError has the cause). */
+#define P3T_ELIMIT  -6   /* p3t_morton_order_static: n exceeds the capacity of the library's fixed scratch array */
+#define P3T_STATIC_MAX_N          (1 << 18)
+#define P3T_STATIC_SCRATCH_BYTES  3678976
+int p3t_morton_order_static(int device, void* cuda_stream, int64_t n, const float* pos_mass, int key_bits,
+                            uint64_t* sorted_keys, uint32_t* order, float* cube, int32_t* bad_input);
+
 /* ---- parity / debug accessors: synchronise; outputs are ANY pointers sized from p3t_get_stats ---- */
 int p3t_get_stats(p3t_ctx* ctx, p3t_stats* out);
 /* sorted Morton keys [n] (30-bit keys are widened to uint64) and order[n] (sorted position -> original id) */

@@ -17,7 +17,8 @@ from pathlib import Path
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libp3t.so"
 
-OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ESTATE, ENOMEM, ECUDA, ERANGE, ELIMIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_N = 1 << 18                # p3t.h: P3T_STATIC_MAX_N, the capacity of p3t_morton_order_static
 
 # every symbol include/p3t.h declares
 SYMBOLS = [
@@ -26,6 +27,7 @@ SYMBOLS = [
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
     "p3t_set_shard", "p3t_get_shard_cuts", "p3t_shard_pack", "p3t_shard_unpack", "p3t_get_octupoles",
+    "p3t_morton_order_static",
 ]
 
 
@@ -92,6 +94,7 @@ def lib() -> C.CDLL:
     L.p3t_get_shard_cuts.argtypes = [vp, vp, vp]
     L.p3t_shard_pack.argtypes = [vp, vp, vp]
     L.p3t_shard_unpack.argtypes = [vp, C.c_int, vp, vp]
+    L.p3t_morton_order_static.argtypes = [C.c_int, vp, i64, vp, C.c_int, vp, vp, vp, vp]
     L.p3t_strerror.argtypes = [C.c_int]; L.p3t_strerror.restype = C.c_char_p
     L.p3t_last_error.argtypes = [vp]; L.p3t_last_error.restype = C.c_char_p
     L.p3t_params_from_n.argtypes = [i64, dbl] + [C.POINTER(dbl)] * 5
@@ -113,6 +116,33 @@ def params_from_n(n: int, sigma: float = 2.0 ** -0.5) -> dict:
     if rc:
         raise P3TError(rc, "p3t_params_from_n")
     return dict(zip(["tau", "r_cut", "r_buff", "dt_reg", "dt_max"], [x.value for x in v]))
+
+
+def morton_order_static(pos_mass, sorted_keys, order, key_bits: int = 63, cube=None, bad_input=None, stream=None):
+    """p3t_morton_order_static: Morton keys, stable sort order and bounding cube of pos_mass (CUDA float32 [n, 4])
+    for callers that must not allocate device memory -- a host code whose own arena or caching allocator already
+    holds the whole device, a step loop that cannot take the device-wide stall of cudaMalloc / cudaFree, a process
+    under a memory quota.  The call needs no Context and allocates nothing: its scratch is a fixed 3.5 MB array
+    inside libp3t.so, good for n <= STATIC_MAX_N (262 144); a larger n raises P3TError(ELIMIT).
+
+    The caller passes every buffer, all CUDA tensors of the same device: sorted_keys int64 [n] (the uint64 keys, bit
+    for bit), order int32 [n] (sorted position -> original id), and optionally cube float32 [4] (lo x, y, z, side)
+    and bad_input int32 [1].  Enqueues on `stream` (a torch.cuda.Stream; None = the legacy default stream) and does
+    not synchronise.  All calls on a device share the one array: order them (one stream, or events); calls that
+    overlap on the GPU race.  The first call on a device also looks up the array's device address -- make it
+    outside any stream capture."""
+    import torch
+    n = int(pos_mass.shape[0])
+    assert pos_mass.is_cuda and pos_mass.dtype == torch.float32 and pos_mass.is_contiguous() and pos_mass.shape[-1] == 4
+    dev = pos_mass.device
+    for t, dt, cnt in ((sorted_keys, torch.int64, n), (order, torch.int32, n), (cube, torch.float32, 4), (bad_input, torch.int32, 1)):
+        assert t is None or (t.device == dev and t.dtype == dt and t.is_contiguous() and t.numel() >= cnt)
+    ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else 0)
+    rc = lib().p3t_morton_order_static(dev.index if dev.index is not None else torch.cuda.current_device(), sp, n,
+                                       ptr(pos_mass), key_bits, ptr(sorted_keys), ptr(order), ptr(cube), ptr(bad_input))
+    if rc != OK:
+        raise P3TError(rc, "p3t_morton_order_static")
 
 
 def _np_ptr(a):

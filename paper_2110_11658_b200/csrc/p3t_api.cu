@@ -38,6 +38,7 @@ const char* p3t_strerror(int code)
     case P3T_ENOMEM: return "out of device memory";
     case P3T_ECUDA: return "CUDA failure (see p3t_last_error)";
     case P3T_ERANGE: return "a neighbour row or list exceeds the capacity given";
+    case P3T_ELIMIT: return "n exceeds P3T_STATIC_MAX_N, the capacity of the fixed scratch array of p3t_morton_order_static";
     default: return "unknown error code";
     }
 }

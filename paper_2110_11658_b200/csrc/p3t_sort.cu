@@ -359,3 +359,99 @@ int p3t_launch_permute(p3t_ctx* ctx, const float4* pm)
     ctx->launches += 1;
     return P3T_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// p3t_morton_order_static (include/p3t.h): a1-a3 without a context and without any device allocation, for hosts
+// that have given all device memory away (their own arena, a caching allocator), that cannot take the device-wide
+// stall of cudaMalloc / cudaFree inside their step loop, or that run under a memory quota.  The kernels are the
+// ones above, unchanged; what differs is where their scratch lives: in the fixed array below, which is part of the
+// library image and so exists on every device that loads this code, for as long as the process runs.
+//
+// Layout of the array (all parts 256-byte aligned):
+//   [ST_INFO]  p3t_devinfo: the cube's min/max words, bad_input, then lo / side / scale        (must start at zero)
+//   [ST_SORT]  digit totals [8][256] u32 | tickets | look-back words [ntiles][256] u64        (must start at zero)
+//   [ST_KEYS]  uint64[P3T_STATIC_MAX_N]: second key buffer of the ping-pong                    (fully written before read)
+//   [ST_IDX]   uint32[P3T_STATIC_MAX_N]: second index buffer                                   (fully written before read)
+// The caller's sorted_keys / order arrays are the first buffers: k_keys writes the unsorted keys there, and the
+// number of passes is even (8 or 4), so the last pass lands there again.
+// ---------------------------------------------------------------------------------------------
+#include <mutex>
+#include <stddef.h>
+
+static constexpr size_t st_round(size_t b) { return (b + 255) / 256 * 256; }
+static constexpr size_t ST_TILES = (P3T_STATIC_MAX_N + P3T_SORT_TILE_MIN - 1) / P3T_SORT_TILE_MIN;
+static constexpr size_t ST_INFO = 0;
+static constexpr size_t ST_SORT = st_round(sizeof(p3t_devinfo));
+static constexpr size_t ST_SORT_HEAD = (size_t)SORT_MAX_PASSES * P3T_RADIX * 4 + 64;       // = sort_status_offset()
+static constexpr size_t ST_KEYS = ST_SORT + st_round(ST_SORT_HEAD + ST_TILES * P3T_RADIX * 8);
+static constexpr size_t ST_IDX = ST_KEYS + st_round((size_t)P3T_STATIC_MAX_N * 8);
+static constexpr size_t ST_BYTES = ST_IDX + st_round((size_t)P3T_STATIC_MAX_N * 4);
+static_assert(ST_BYTES == P3T_STATIC_SCRATCH_BYTES, "include/p3t.h states the size of the static scratch array");
+static_assert(P3T_STATIC_MAX_N <= (1 << 18), "the static entry point uses the small sort tile only");
+static_assert(offsetof(p3t_devinfo, lo) == 0 && offsetof(p3t_devinfo, side) == 12, "cube = the record's first 16 bytes");
+
+// In host code this name is only a handle for cudaGetSymbolAddress; it is not an address a kernel can use.
+static __device__ __align__(256) unsigned char g_static_scratch[ST_BYTES];
+
+#define ST_MAX_DEVICES 64
+static std::mutex g_static_mutex;
+static unsigned char* g_static_ptr[ST_MAX_DEVICES];   // device address of g_static_scratch on each device (0 = not asked yet)
+static int g_static_sms[ST_MAX_DEVICES];
+
+// once per device, with that device current; allocates nothing
+static int static_setup(int device, unsigned char** base, int* sms)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[device]) {
+        void* p = nullptr; int s = 0;
+        P3T_CUDA(nullptr, cudaGetSymbolAddress(&p, g_static_scratch));
+        P3T_CUDA(nullptr, cudaDeviceGetAttribute(&s, cudaDevAttrMultiProcessorCount, device));
+        if (!p || s < 1) return P3T_ECUDA;
+        g_static_sms[device] = s;
+        g_static_ptr[device] = (unsigned char*)p;
+    }
+    *base = g_static_ptr[device]; *sms = g_static_sms[device];
+    return P3T_OK;
+}
+
+extern "C" int p3t_morton_order_static(int device, void* cuda_stream, int64_t n, const float* pos_mass, int key_bits,
+                                       uint64_t* sorted_keys, uint32_t* order, float* cube, int32_t* bad_input)
+{
+    if (!pos_mass || !sorted_keys || !order || n < 1 || (key_bits != 30 && key_bits != 63)) return P3T_EINVAL;
+    if (((uintptr_t)pos_mass & 15u) || ((uintptr_t)sorted_keys & 7u) || ((uintptr_t)order & 3u) ||
+        ((uintptr_t)cube & 3u) || ((uintptr_t)bad_input & 3u)) return P3T_EINVAL;
+    if (device < 0 || device >= ST_MAX_DEVICES) return P3T_EINVAL;
+    if (n > P3T_STATIC_MAX_N) return P3T_ELIMIT;                     // the array is sized for P3T_STATIC_MAX_N: refuse, do not overrun
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { (void)cudaGetLastError(); return P3T_EINVAL; }
+    P3T_CUDA(nullptr, cudaSetDevice(device));
+    unsigned char* base; int sms, rc;
+    if ((rc = static_setup(device, &base, &sms)) != P3T_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int ni = (int)n, bits = key_bits / 3;
+    const int passes = (3 * bits + P3T_RADIX_BITS - 1) / P3T_RADIX_BITS;         // 8 or 4: even
+    const int ntiles = (ni + P3T_SORT_TILE_MIN - 1) / P3T_SORT_TILE_MIN;
+    p3t_devinfo* info = (p3t_devinfo*)(base + ST_INFO);
+    uint32_t* ghist = (uint32_t*)(base + ST_SORT);
+    uint32_t* ticket = ghist + SORT_MAX_PASSES * P3T_RADIX;
+    unsigned long long* status = (unsigned long long*)(base + ST_SORT + ST_SORT_HEAD);
+    uint64_t* ktmp = (uint64_t*)(base + ST_KEYS);
+    uint32_t* vtmp = (uint32_t*)(base + ST_IDX);
+    // what the last call left behind goes: the cube record, the digit totals, the tickets and this call's look-back words
+    P3T_CUDA(nullptr, cudaMemsetAsync(base, 0, ST_SORT + ST_SORT_HEAD + (size_t)ntiles * P3T_RADIX * 8, st));
+    int blocks = (ni + 255) / 256;
+    if (blocks > sms * 8) blocks = sms * 8;
+    const float4* pm = (const float4*)pos_mass;
+    k_cube<<<blocks, 256, 0, st>>>(pm, ni, info);
+    k_keys<<<blocks, 256, 0, st>>>(pm, ni, bits, passes, info, sorted_keys, ghist);
+    for (int p = 0; p < passes; ++p) {
+        const uint64_t* kin = (p & 1) ? ktmp : sorted_keys;  uint64_t* kout = (p & 1) ? sorted_keys : ktmp;
+        const uint32_t* vin = (p & 1) ? vtmp : order;        uint32_t* vout = (p & 1) ? order : vtmp;
+        if (p == 0) k_sort_pass<true, P3T_SORT_ITEMS_MIN><<<ntiles, P3T_SORT_THREADS, 0, st>>>(kin, vin, kout, vout, ni, p, ghist, status, ticket);
+        else        k_sort_pass<false, P3T_SORT_ITEMS_MIN><<<ntiles, P3T_SORT_THREADS, 0, st>>>(kin, vin, kout, vout, ni, p, ghist, status, ticket);
+    }
+    P3T_CUDA(nullptr, cudaGetLastError());
+    if (cube) P3T_CUDA(nullptr, cudaMemcpyAsync(cube, &info->lo[0], 16, cudaMemcpyDeviceToDevice, st));
+    if (bad_input) P3T_CUDA(nullptr, cudaMemcpyAsync(bad_input, &info->bad_input, 4, cudaMemcpyDeviceToDevice, st));
+    return P3T_OK;
+}
