@@ -319,8 +319,11 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
     const long long rowbase = v ? A.nboff[orig] : 0;
     int* rowcnt = SPLIT ? A.nbcnt + (v ? T.id : tb) : &S.nbrow[T.slot];
     if (!SPLIT) S.nbrow[lane] = 0;
-    const uint4 rec = __ldcg(&A.glist[g]);
+    // Only lane 0 has read the group's state word with an acquire (group_state); the shuffle that hands the state to the
+    // other lanes orders no memory.  This warp barrier does: every read of what the walker published for the group --
+    // the list record below and the list entries after it -- comes behind it in every lane.
     __syncwarp();
+    const uint4 rec = __ldcg(&A.glist[g]);
     // ---- a8: particle-cell list; a lane sees TILE / k cells per tile: fold every k tiles ----
     {
         const int32_t* ids = A.pcpool + ((long long)rec.x << 5);
@@ -388,11 +391,22 @@ __device__ void force_item(const force_args& A, tile_smem& S, int g, int tb, int
 }
 
 // SPLIT epilogue (a11): the segments of every particle in segment order, then the kick.  In the host's repair pass
-// (A.mode 1) the sums are written again for everybody (same values) but only the particles of redone groups are kicked.
+// (A.mode 1) only the particles of redone groups are kicked, and -- unless every group was evaluated again (A.evalall) --
+// only they are written: the result of a group that was complete after the first pass stays as it is (the octupole
+// variant has already added its term to it, and p3t_launch_octupole_add visits the same set of groups as this kernel).
 __global__ void __launch_bounds__(256) k_force_final(force_args A, int n, const int32_t* __restrict__ rank)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n || (A.info->bad_input | A.info->node_overflow)) return;
+    bool redone = true;
+    if (A.mode == 1) {                                          // the group of particle i: last g with gbegin[g] <= rank[i]
+        const int sp = rank[i];
+        int lo = 0, hi = A.info->n_groups;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (A.gbegin[mid] <= sp) lo = mid; else hi = mid; }
+        const int st = A.gready[lo] - A.base;
+        redone = st == G_REDONE;
+        if (!(redone || (A.evalall && st == G_READY))) return;
+    }
     double s[4] = { 0, 0, 0, 0 };
     for (int g = 0; g < A.nseg; ++g) {
         const double* q = A.part + ((size_t)g * n + i) * 4;
@@ -400,13 +414,7 @@ __global__ void __launch_bounds__(256) k_force_final(force_args A, int n, const 
     }
     const float4 a = make_float4((float)s[0], (float)s[1], (float)s[2], (float)s[3]);
     A.out[i] = a;
-    bool kick = A.vel != nullptr;
-    if (kick && A.mode == 1) {                                  // the group of particle i: last g with gbegin[g] <= rank[i]
-        const int sp = rank[i];
-        int lo = 0, hi = A.info->n_groups;
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (A.gbegin[mid] <= sp) lo = mid; else hi = mid; }
-        kick = A.gready[lo] == A.base + G_REDONE;
-    }
+    const bool kick = A.vel != nullptr && redone;
     if (kick) {
         float4 u = A.vel[i];
         u.x = fmaf(A.half_dt, a.x, u.x); u.y = fmaf(A.half_dt, a.y, u.y); u.z = fmaf(A.half_dt, a.z, u.z);

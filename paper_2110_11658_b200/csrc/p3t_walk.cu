@@ -312,6 +312,7 @@ __global__ void k_walk_reset(p3t_devinfo* info)
     info->n_pp = info->n_pc = info->n_pp_list = info->n_pc_list = 0ull;
     info->pool_overflow = 0; info->need_pc = 0; info->need_pp = 0;
     info->nb_overflow = 0; info->spin_abort = 0;
+    info->stack_overflow = 0;     // a condition of one force call (its theta), not of the tree: the next call may fit
 }
 
 static int walk_blocks(p3t_ctx* ctx, int mode, int* out, bool limit_by_n = true)

@@ -101,6 +101,55 @@ def test_force_warps_that_stop_waiting(p3t, monkeypatch):
     assert np.linalg.norm(ref["a"][:, :3] - f["acc_pot"][:, :3]) <= 1e-6 * np.linalg.norm(f["acc_pot"][:, :3])
 
 
+def test_repair_keeps_the_octupole_term_of_finished_groups(p3t, monkeypatch):
+    """Order 3 at small N (every work item shared by several warps, so the sums go through k_force_final) with
+    P3T_TEST_FAULT=1: some groups are complete after the first pass, the others are redone.  The repair pass must leave
+    the finished groups alone -- their result already carries the octupole term, which the repair adds only to the
+    groups it redoes -- so that acceleration and kicked velocity are those of an undisturbed call, bit for bit."""
+    w = workloads.make_config(1, n_override=20000)
+    vel = workloads.velocities_for(w)
+    half_dt = float(np.float32(1.0 / 512.0))
+    with p3t.Context(0) as ctx:
+        ctx.set_multipole_order(3)
+        _run(ctx, w, vel, half_dt)
+        ref = _run(ctx, w, vel, half_dt)
+    with p3t.Context(0) as ctx:
+        quad = _run(ctx, w, vel, half_dt)
+    assert np.mean(ref["a"][:, :3] != quad["a"][:, :3]) > 0.5          # the octupole term is really there
+    monkeypatch.setenv("P3T_TEST_FAULT", "1")
+    with p3t.Context(0) as ctx:
+        ctx.set_multipole_order(3)
+        for _ in range(2):
+            got = _run(ctx, w, vel, half_dt)
+            _same(got, ref)                                            # acceleration AND velocity: kicked exactly as undisturbed
+    # the order-3 kick is two fmas (quadrupole-order sum, then the octupole's share): a few ulp from the one-fma value
+    a = ref["a"][:, :3].astype(np.float64)
+    want = vel[:, :3].astype(np.float64) + np.float64(half_dt) * a
+    assert np.all(np.abs(ref["v"][:, :3] - want) <= 4e-7 * (np.abs(want) + half_dt * np.abs(a)) + 1e-30)
+
+
+def test_walk_stack_overflow_is_a_condition_of_one_call(p3t, monkeypatch):
+    """theta may change between calls without a rebuild (include/p3t.h): after a call whose wide-open walk overflowed
+    the walk stack (P3T_ECUDA; P3T_TEST_FAULT=2 takes the spill space away so that 384 entries are all there is), a
+    call on the SAME tree with a theta whose walk fits works, and gives what a fresh context gives."""
+    w = workloads.make_config(1, n_override=20000)
+    pm = _cuda(w.pos_mass)
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(pm, 63)
+        ref = ctx.regular_force(w.r_out, w.r_in, 1.0, 0).cpu().numpy()
+        roff, ridx = [x.cpu().numpy() for x in ctx.neighbours()]
+    monkeypatch.setenv("P3T_TEST_FAULT", "2")
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(pm, 63)
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.regular_force(w.r_out, w.r_in, 1e-3, 0)
+        assert e.value.code == p3t.ECUDA and "stack_overflow=1" in str(e.value)
+        got = ctx.regular_force(w.r_out, w.r_in, 1.0, 0).cpu().numpy()
+        assert np.array_equal(got, ref)
+        off, idx = [x.cpu().numpy() for x in ctx.neighbours()]
+        assert np.array_equal(off, roff) and np.array_equal(idx, ridx)
+
+
 def test_capacity_error_comes_from_the_force_call(p3t, monkeypatch):
     """P3T_TEST_FAULT=2 removes the spill space of the walk stack: a wide-open walk (theta -> 0) overflows it, and
     p3t_regular_force itself returns P3T_ECUDA (not a later accessor); NaN input is reported by it too, and the
