@@ -250,6 +250,8 @@ def time_steps(torch, ctx, pm_dev, out_dev, w, flush, steps: int, warmup: int) -
         step()
         ev[k][1].record()
         st = ctx.stats()                                  # synchronises; after the closing event
+        # a timed step that redid part of its work (undersized buffer, force warps that gave up waiting) is not a measurement
+        assert not st["force_flags"] & 6, f"timed step {k} was repaired (force_flags={st['force_flags']}): more warm-up needed"
         for q in ph:
             ph[q].append(st[q])
     torch.cuda.synchronize()

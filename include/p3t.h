@@ -73,8 +73,16 @@ typedef struct p3t_stats {
     float   ms_core;         /* ... of the last p3t_core_quantities kernels (0 if none)  */
     int64_t launches;        /* kernels this context has launched since p3t_create      */
     float   ms_octupole;     /* ... of the octupole add kernel of the last force (order 3; else 0) */
-    float   reserved_;
+    int32_t force_flags;     /* how the last force call ran: P3T_FF_* bits                */
 } p3t_stats;
+
+#define P3T_FF_OVERLAPPED 1  /* the list walk ran beside the force kernel (the normal case; not when another context of the
+                                process had an overlapped call in flight on the device, or after P3T_FF_SPIN_ABORT)          */
+#define P3T_FF_REPAIRED   2  /* a buffer sized from the previous call was too small: part of the call was redone (normally
+                                only the first call of a context; costs up to a second pass)                                */
+#define P3T_FF_SPIN_ABORT 4  /* force warps stopped waiting for the list walk (~70 ms: no walker was resident, e.g. another
+                                process filled the SMs); the call was repaired and the context runs its later calls without
+                                the overlap, instead of paying that wait every step                                         */
 
 /* Create a context on CUDA device `device`, enqueuing on `cuda_stream` (a cudaStream_t passed as
  * void*; NULL = the legacy default stream).  *out is set on success. */
@@ -153,6 +161,20 @@ int p3t_regular_force(p3t_ctx* ctx, float r_out, float r_in, float theta, int po
  * updated in place; NULL = no kick.  Everything else as p3t_regular_force (= r_buff 0, vel NULL). */
 int p3t_regular_force_ex(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float r_buff,
                          float half_dt, float* vel, float* acc_pot);
+
+/* The same call in two halves, for a host that has work of its own to do meanwhile: in the paper's loop (steps
+ * (i)-(vi)) the CPU integrates the irregular forces between two regular steps, and Fig. 7
+ * puts half of the wall time there.  p3t_regular_force_begin checks the arguments, enqueues the whole
+ * call ("calls enqueue on the context's stream and do not synchronise") and returns;
+ * p3t_regular_force_wait synchronises once, reports the errors listed above, redoes what an undersized buffer left
+ * out, and only then are acc_pot, vel and the neighbour lists complete.  Between the two the caller must not touch
+ * acc_pot / vel; a build, a step, a second begin or p3t_set_shard on this context returns P3T_ESTATE, and so do
+ * the list accessors (the lists are not there yet); p3t_destroy is allowed and drains the call.
+ * A begin that fails has drained whatever it had enqueued; no wait is needed (a wait with nothing pending returns
+ * P3T_ESTATE).  p3t_regular_force_ex is exactly begin followed by wait. */
+int p3t_regular_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                            float half_dt, float* vel, float* acc_pot);
+int p3t_regular_force_wait(p3t_ctx* ctx);
 
 /* core quantities by a sampled k-nearest-neighbour search (PAPER.md:134, :245:
  * "a random sample of min(N, sqrt(5000 N)) particles, then ... those particles' 6 nearest neighbours";

@@ -27,8 +27,9 @@ SYMBOLS = [
     "p3t_get_stats", "p3t_get_keys", "p3t_get_nodes", "p3t_get_moments", "p3t_get_groups",
     "p3t_get_list_lengths", "p3t_strerror", "p3t_last_error", "p3t_params_from_n",
     "p3t_set_shard", "p3t_get_shard_cuts", "p3t_shard_pack", "p3t_shard_unpack", "p3t_get_octupoles",
-    "p3t_morton_order_static",
+    "p3t_morton_order_static", "p3t_regular_force_begin", "p3t_regular_force_wait",
 ]
+FF_OVERLAPPED, FF_REPAIRED, FF_SPIN_ABORT = 1, 2, 4           # p3t.h: bits of Stats.force_flags
 
 
 class Stats(C.Structure):
@@ -40,7 +41,7 @@ class Stats(C.Structure):
         ("cube_lo", C.c_float * 3), ("cube_side", C.c_float),
         ("ms_build", C.c_float), ("ms_force", C.c_float), ("ms_walk", C.c_float), ("ms_sort", C.c_float),
         ("ms_eval", C.c_float), ("ms_count", C.c_float), ("ms_irregular", C.c_float), ("ms_core", C.c_float),
-        ("launches", C.c_int64), ("ms_octupole", C.c_float), ("reserved_", C.c_float),
+        ("launches", C.c_int64), ("ms_octupole", C.c_float), ("force_flags", C.c_int32),
     ]
 
     def as_dict(self) -> dict:
@@ -77,6 +78,8 @@ def lib() -> C.CDLL:
     L.p3t_build_tree.argtypes = [vp, i64, vp, C.c_int]
     L.p3t_regular_force.argtypes = [vp, f32, f32, f32, C.c_int, vp]
     L.p3t_regular_force_ex.argtypes = [vp, f32, f32, f32, C.c_int, f32, f32, vp, vp]
+    L.p3t_regular_force_begin.argtypes = [vp, f32, f32, f32, C.c_int, f32, f32, vp, vp]
+    L.p3t_regular_force_wait.argtypes = [vp]
     L.p3t_irregular_force.argtypes = [vp, vp, vp, vp]
     L.p3t_core_quantities.argtypes = [vp, i64, vp, C.c_int, vp, vp, vp, vp]
     L.p3t_neighbours.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
@@ -254,6 +257,25 @@ class Context:
             self._check(lib().p3t_regular_force_ex(self._h, r_out, r_in, theta, pot_mode, r_buff, half_dt, pv, self._dev_f32(out, 4)),
                         "p3t_regular_force_ex")
         return out
+
+    def regular_force_begin(self, r_out: float, r_in: float, theta: float, pot_mode: int = 0, out=None,
+                            r_buff: float = 0.0, half_dt: float = 0.0, vel=None):
+        """First half of regular_force: enqueues the whole call and returns without waiting, so that the host can do its
+        own work (the irregular steps of PAPER.md:89-94) while the GPU runs.  `out` (and vel) are complete only after
+        regular_force_wait(); no other call on this context in between."""
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
+        pv = None if vel is None else self._dev_f32(vel, 4)
+        self._check(lib().p3t_regular_force_begin(self._h, r_out, r_in, theta, pot_mode, r_buff, half_dt, pv, self._dev_f32(out, 4)),
+                    "p3t_regular_force_begin")
+        self._pending_out = (out, vel)                               # keeps the tensors alive while the GPU writes them
+        return out
+
+    def regular_force_wait(self):
+        """Second half: the call's one synchronisation and its error report."""
+        self._check(lib().p3t_regular_force_wait(self._h), "p3t_regular_force_wait")
+        self._pending_out = None
 
     def irregular_force(self, vel, acc_out=None, jerk_out=None):
         """Irregular force over the neighbour lists of the last regular_force.

@@ -84,6 +84,7 @@ int p3t_destroy(p3t_ctx* c)
 {
     if (!c) return P3T_EINVAL;
     cudaSetDevice(c->device);
+    p3t_force_abandon(c);                                    // a force call still in flight: drained, its overlap slot released
     cudaStreamSynchronize(c->stream);
     p3t_buf* bufs[] = { &c->keys[0], &c->keys[1], &c->idx[0], &c->idx[1], &c->spm, &c->rank, &c->hist, &c->nlevel, &c->nbegin, &c->nend,
                         &c->nfirst, &c->nnchild, &c->m64, &c->ncom, &c->nlo, &c->nhi, &c->nq0, &c->nq1, &c->nlink, &c->scan_tmp, &c->pcl, &c->plam, &c->nparent, &c->nfc, &c->ncount, &c->gsum,
@@ -123,6 +124,7 @@ int p3t_set_shard(p3t_ctx* c, int rank, int nranks, const int64_t* nominal_cuts)
 {
     if (!c || nranks < 1 || nranks > P3T_MAX_RANKS || rank < 0 || rank >= nranks) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
+    if (c->pend.active) return P3T_ESTATE;
     c->shard_rank = rank; c->shard_nranks = nranks; c->shard_has_nominal = 0;
     if (nominal_cuts && nranks > 1) {
         P3T_CUDA(c, cudaSetDevice(c->device));
@@ -141,6 +143,7 @@ int p3t_build_tree(p3t_ctx* c, int64_t n, const float* pos_mass, int key_bits)
     if (!c || !pos_mass || n < 1 || n > P3T_MAX_N || (key_bits != 30 && key_bits != 63)) return P3T_EINVAL;
     if (((uintptr_t)pos_mass & 15u) != 0) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
+    if (c->pend.active) return P3T_ESTATE;                   // between p3t_regular_force_begin and _wait
     P3T_CUDA(c, cudaSetDevice(c->device));
     c->state = 0; c->nb_valid = 0; c->irr_done = 0; c->core_done = 0; c->oct_built = 0;
     c->n = n; c->key_bits = key_bits; c->bits = key_bits / 3;
@@ -198,18 +201,37 @@ static int force_check_args(p3t_ctx* c, float r_out, float r_in, float theta, in
     return P3T_OK;
 }
 
-int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
-                         float half_dt, float* vel, float* acc_pot)
+int p3t_regular_force_begin(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                            float half_dt, float* vel, float* acc_pot)
 {
+    if (c && c->pend.active) return P3T_ESTATE;
     int rc = force_check_args(c, r_out, r_in, theta, pot_mode, r_buff, half_dt, vel, acc_pot);
     if (rc != P3T_OK) return rc;
+    c->state = 1;                                            // no lists until the wait has returned
     if ((rc = p3t_force_begin(c, r_out, r_in, theta, pot_mode, (float4*)acc_pot, c->r_list, half_dt, (float4*)vel)) != P3T_OK) {
         (void)p3t_force_finish(c);                           // whatever was enqueued is drained before the error is returned
         return rc;
     }
-    if ((rc = p3t_force_finish(c)) != P3T_OK) return rc;
+    return P3T_OK;
+}
+
+int p3t_regular_force_wait(p3t_ctx* c)
+{
+    if (!c) return P3T_EINVAL;
+    if (!c->pend.active) return P3T_ESTATE;
+    P3T_CUDA(c, cudaSetDevice(c->device));
+    int rc = p3t_force_finish(c);
+    if (rc != P3T_OK) return rc;
     c->state = 2; c->nb_valid = 1;
     return P3T_OK;
+}
+
+int p3t_regular_force_ex(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float r_buff,
+                         float half_dt, float* vel, float* acc_pot)
+{
+    int rc = p3t_regular_force_begin(c, r_out, r_in, theta, pot_mode, r_buff, half_dt, vel, acc_pot);
+    if (rc != P3T_OK) return rc;
+    return p3t_regular_force_wait(c);
 }
 
 int p3t_regular_force(p3t_ctx* c, float r_out, float r_in, float theta, int pot_mode, float* acc_pot)
@@ -287,6 +309,7 @@ int p3t_get_stats(p3t_ctx* c, p3t_stats* out)
         if (c->walk_stream) (void)cudaEventElapsedTime(&out->ms_count, c->ev[4], c->ev_scan);
         if (c->irr_done) (void)cudaEventElapsedTime(&out->ms_irregular, c->evi[0], c->evi[1]);
         if (c->order == 3) (void)cudaEventElapsedTime(&out->ms_octupole, c->evo[0], c->evo[1]);
+        out->force_flags = c->pend.flags;
     }
     if (c->core_done) {
         (void)cudaEventElapsedTime(&out->ms_core, c->evc[0], c->evc[1]);
@@ -362,6 +385,7 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
 {
     if (!c || !pos_mass_host || !acc_pot_host || n < 1 || n > P3T_MAX_N) return P3T_EINVAL;
     if (c->sticky) return P3T_ECUDA;
+    if (c->pend.active) return P3T_ESTATE;
     P3T_CUDA(c, cudaSetDevice(c->device));
     int rc;
     if ((rc = p3t_reserve(c, &c->stage_in, (size_t)n * 32)) != P3T_OK) return rc;     // pos_mass in, acc_pot out
@@ -373,21 +397,25 @@ int p3t_step_host(p3t_ctx* c, int64_t n, const float* pos_mass_host, int key_bit
     if ((rc = p3t_force_begin(c, r_out, r_in, theta, pot_mode, (float4*)d_out, c->r_list, 0.0f, nullptr)) != P3T_OK) { (void)p3t_force_finish(c); return rc; }
     // The CSR offsets and the entry count are final once the offset scan is through (ev_scan), long before the force
     // kernel ends: their copies go to a second stream and overlap it.  The host waits for that stream only.
-    if (!c->copy_stream) P3T_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    // From here to p3t_force_finish a call is in flight: every failure goes through p3t_force_finish (IN_FLIGHT), which
+    // drains the stream and gives the device's overlap slot back -- a plain return would keep it for good.
+#define IN_FLIGHT(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { (void)p3t_force_finish(c); return p3t_fail_cuda(c, e_, #call, __LINE__); } } while (0)
+    if (!c->copy_stream) IN_FLIGHT(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    if (c->test_fault & 4) IN_FLIGHT(cudaErrorInvalidValue);          // tests: a CUDA failure with the call in flight
     p3t_devinfo h;
-    P3T_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_scan, 0));
-    if (nb_offsets_host) P3T_CUDA(c, cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->copy_stream));
-    P3T_CUDA(c, cudaMemcpyAsync(&h, c->info.p, sizeof(h), cudaMemcpyDeviceToHost, c->copy_stream));
-    cudaError_t e = cudaStreamSynchronize(c->copy_stream);
-    if (e != cudaSuccess) { (void)p3t_force_finish(c); return p3t_fail_cuda(c, e, "copy stream", __LINE__); }
+    IN_FLIGHT(cudaStreamWaitEvent(c->copy_stream, c->ev_scan, 0));
+    if (nb_offsets_host) IN_FLIGHT(cudaMemcpyAsync(nb_offsets_host, c->nboff.p, ((size_t)n + 1) * 8, cudaMemcpyDeviceToHost, c->copy_stream));
+    IN_FLIGHT(cudaMemcpyAsync(&h, c->info.p, sizeof(h), cudaMemcpyDeviceToHost, c->copy_stream));
+    IN_FLIGHT(cudaStreamSynchronize(c->copy_stream));
     int64_t total = (int64_t)h.nb_total;
     const bool fits = total <= c->nb_cap && !h.bad_input;                 // else nothing was emitted: the repair pass of finish does it
-    P3T_CUDA(c, cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
+    IN_FLIGHT(cudaMemcpyAsync(acc_pot_host, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
     int over = 0;
     if (nb_indices_host) {
         if (total > nb_cap) over = 1;
-        else if (total > 0 && fits) P3T_CUDA(c, cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
+        else if (total > 0 && fits) IN_FLIGHT(cudaMemcpyAsync(nb_indices_host, c->nbidx.p, (size_t)total * 4, cudaMemcpyDeviceToHost, c->stream));
     }
+#undef IN_FLIGHT
     if ((rc = p3t_force_finish(c)) != P3T_OK) return rc;            // synchronises the stream: the copies above are done
     c->state = 2; c->nb_valid = 1;
     if (c->pend.repaired || !fits) {                                // (first call of a context, normally) results changed after the copies

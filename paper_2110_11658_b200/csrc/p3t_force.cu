@@ -731,7 +731,7 @@ int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_
     if ((rc = force_streams(ctx))) return rc;
     p3t_pending& q = ctx->pend;
     q.r_out = r_out; q.r_in = r_in; q.theta = theta; q.r_list = r_list; q.half_dt = half_dt; q.pot_mode = pot_mode;
-    q.acc_pot = acc_pot; q.vel = vel; q.active = 1; q.repaired = 0;
+    q.acc_pot = acc_pot; q.vel = vel; q.active = 1; q.repaired = 0; q.flags = 0;
     // ---- every buffer before anything is enqueued (a reallocation synchronises the stream) ----
     const int nsb = (n + SCAN_TILE - 1) / SCAN_TILE;
     if ((rc = p3t_reserve(ctx, &ctx->nbcount, (size_t)n * 4))) return rc;
@@ -754,6 +754,7 @@ int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_
         overlapped = g_overlap_owner[ctx->device & 63].compare_exchange_strong(expect, 1) ? 1 : 0;
     }
     q.overlapped = overlapped;
+    if (overlapped) q.flags |= P3T_FF_OVERLAPPED;
     int wsm = overlapped ? ctx->walk_ctas_per_sm : 0;
     if (wsm >= ctx->occ_force) wsm = ctx->occ_force - 1;
     if ((rc = p3t_walk_reserve(ctx, wsm))) return rc;
@@ -813,6 +814,13 @@ int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_
     return force_tail(ctx, A, 0, 0);
 }
 
+void p3t_force_abandon(p3t_ctx* ctx)
+{
+    p3t_pending& q = ctx->pend;
+    if (q.active) { (void)cudaStreamSynchronize(ctx->stream); q.active = 0; }
+    if (q.overlapped) { g_overlap_owner[ctx->device & 63].store(0); q.overlapped = 0; }
+}
+
 int p3t_force_finish(p3t_ctx* ctx)
 {
     p3t_pending& q = ctx->pend;
@@ -835,7 +843,12 @@ int p3t_force_finish(p3t_ctx* ctx)
         if (!h.pool_overflow && !h.nb_overflow && !h.spin_abort) break;
         if (attempt >= 4) { snprintf(ctx->err, sizeof(ctx->err), "list buffers still too small after %d repair passes", attempt); return P3T_ECUDA; }
         // ---- repair pass (stream order, no overlap): larger buffers, every list again, then only what is missing ----
-        q.repaired = 1;
+        q.repaired = 1; q.flags |= P3T_FF_REPAIRED;
+        if (h.spin_abort && !(ctx->test_fault & 1)) {
+            // force warps waited ~70 ms for a walker that never became resident: this context stops overlapping
+            // rather than paying that wait at every step (reported in p3t_stats::force_flags)
+            q.flags |= P3T_FF_SPIN_ABORT; ctx->overlap = 0;
+        }
         const int evalall = h.nb_overflow ? 1 : 0;
         if (h.pool_overflow) {
             ctx->pool_cap_pc = (((long long)h.need_pc + h.need_pc / 4 + 16384) + 31) & ~31ll;

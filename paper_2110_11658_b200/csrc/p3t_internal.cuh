@@ -65,6 +65,7 @@ struct p3t_devinfo {
 struct p3t_pending {
     float r_out, r_in, theta, r_list, half_dt;
     int pot_mode, active, overlapped, repaired;
+    int flags;                       // P3T_FF_* of the call (p3t_stats::force_flags)
     float4 *acc_pot, *vel;
 };
 
@@ -141,7 +142,8 @@ struct p3t_ctx {
     int64_t nb_cap;                  // capacity of nbidx / the raw row buffer in entries (grow-only, from the previous call's total)
     int nb_max_hint;                 // longest row of the previous call (chooses the row-sort variant; any value is correct)
     p3t_pending pend;
-    int test_fault;                  // P3T_TEST_FAULT (tests only): 1 = the force kernel gives up waiting at once, 2 = no walk-stack spill
+    int test_fault;                  // P3T_TEST_FAULT (tests only), bits: 1 = the force kernel gives up waiting at once, 2 = no walk-stack spill,
+                                     // 4 = p3t_step_host meets a CUDA failure while its force call is in flight
 };
 
 #define P3T_CUDA(ctx, call)                                                              \
@@ -187,6 +189,7 @@ int p3t_launch_irregular(p3t_ctx* ctx, const float4* vel, float4* acc, float4* j
 int p3t_force_begin(p3t_ctx* ctx, float r_out, float r_in, float theta, int pot_mode, float4* acc_pot,
                     float r_list, float half_dt, float4* vel);
 int p3t_force_finish(p3t_ctx* ctx);
+void p3t_force_abandon(p3t_ctx* ctx);        // p3t_destroy with a call in flight: the stream is drained, the device's overlap slot released
 
 // group-state helpers shared by the walk, force and octupole kernels
 __device__ __forceinline__ int ld_acquire_gpu(const int32_t* p)

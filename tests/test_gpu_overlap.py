@@ -253,3 +253,69 @@ def test_step_host_as_first_call_with_repair(p3t):
         assert np.array_equal(acc, a) and np.array_equal(nb_off, off) and np.array_equal(nb_idx[:total], idx)
         acc2, _, _, total2 = ctx.step_host(w.pos_mass, w.r_out, w.r_in, w.theta, nb_offsets=nb_off, nb_indices=nb_idx)
         assert total2 == total and np.array_equal(acc2, a) and np.array_equal(nb_idx[:total], idx)
+
+
+def test_begin_wait_is_the_blocking_call_in_two_halves(p3t):
+    """p3t_regular_force_begin returns with the call enqueued (the host is free: PAPER.md:89-94, the CPU integrates the
+    irregular forces meanwhile), p3t_regular_force_wait completes it: same bits as the blocking call; the state rules
+    of include/p3t.h hold in between; a context destroyed with a call in flight leaves the device's overlap slot free."""
+    import torch
+    w = workloads.make_config(1, n_override=120000)
+    vel = workloads.velocities_for(w)
+    half_dt = float(np.float32(1.0 / 512.0))
+    pm = _cuda(w.pos_mass)
+    with p3t.Context(0) as ctx:
+        _run(ctx, w, vel, half_dt)
+        ref = _run(ctx, w, vel, half_dt)
+        assert ref["st"]["force_flags"] == p3t.FF_OVERLAPPED          # overlapped, nothing repaired
+    L = p3t.lib()
+    with p3t.Context(0) as ctx:
+        assert L.p3t_regular_force_wait(ctx._h) == p3t.ESTATE        # nothing pending
+        for k in range(2):                                           # first call of the context (repair inside wait), then a normal one
+            ctx.build_tree(pm, 63)
+            v = _cuda(vel)
+            out = ctx.regular_force_begin(w.r_out, w.r_in, w.theta, 0, half_dt=half_dt, vel=v)
+            host_work = sum(i * i for i in range(20000))             # the host is not blocked
+            assert L.p3t_build_tree(ctx._h, w.n, pm.data_ptr(), 63) == p3t.ESTATE
+            assert L.p3t_regular_force_begin(ctx._h, w.r_out, w.r_in, w.theta, 0, 0.0, 0.0, None, out.data_ptr()) == p3t.ESTATE
+            with pytest.raises(p3t.P3TError):
+                ctx.neighbours()
+            ctx.regular_force_wait()
+            off, idx = ctx.neighbours()
+            npp, npc = ctx.list_lengths()
+            got = dict(a=out.cpu().numpy(), v=v.cpu().numpy(), off=off.cpu().numpy(), idx=idx.cpu().numpy(), npp=npp, npc=npc, st=ctx.stats())
+            _same(got, ref)
+            assert host_work > 0
+        assert got["st"]["force_flags"] == p3t.FF_OVERLAPPED
+    # destroyed between begin and wait
+    ctx = p3t.Context(0)
+    ctx.build_tree(pm, 63)
+    out = ctx.regular_force_begin(w.r_out, w.r_in, w.theta, 0)
+    ctx.close()
+    del out
+    with p3t.Context(0) as ctx:
+        got = _run(ctx, w, vel, half_dt)
+        assert got["st"]["force_flags"] & p3t.FF_OVERLAPPED, "the overlap slot of the device was not given back"
+        _same(got, ref)
+
+
+def test_failed_step_host_gives_the_overlap_slot_back(p3t, monkeypatch):
+    """A CUDA failure inside p3t_step_host after the force call has been enqueued (P3T_TEST_FAULT=4 injects one) is
+    reported, the context is drained, and the per-device overlap slot is free again: the next context still runs the
+    walk beside the force kernel (it used to fall back to the serial order for the rest of the process)."""
+    w = workloads.make_config(1, n_override=50000)
+    pm_host = np.ascontiguousarray(w.pos_mass)
+    monkeypatch.setenv("P3T_TEST_FAULT", "4")
+    with p3t.Context(0) as ctx:
+        with pytest.raises(p3t.P3TError) as e:
+            ctx.step_host(pm_host, w.r_out, w.r_in, w.theta, nb_offsets=np.empty(w.n + 1, np.int64))
+        assert e.value.code == p3t.ECUDA
+        with pytest.raises(p3t.P3TError):                         # a CUDA failure is sticky for its context
+            ctx.build_tree(_cuda(w.pos_mass), 63)
+    monkeypatch.delenv("P3T_TEST_FAULT")
+    with p3t.Context(0) as ctx:
+        ctx.build_tree(_cuda(w.pos_mass), 63)
+        ctx.regular_force(w.r_out, w.r_in, w.theta, 0)
+        assert ctx.stats()["force_flags"] & p3t.FF_OVERLAPPED, "the overlap slot of the device was not given back"
+        a, off, idx, total = ctx.step_host(pm_host, w.r_out, w.r_in, w.theta, nb_offsets=np.empty(w.n + 1, np.int64))
+        assert ctx.stats()["force_flags"] & p3t.FF_OVERLAPPED and total > 0
