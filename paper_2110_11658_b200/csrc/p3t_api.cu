@@ -73,7 +73,6 @@ int p3t_create(p3t_ctx** out, int device, void* cuda_stream)
     for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->evo[k]);
     if (e != cudaSuccess) { delete c; (void)cudaGetLastError(); return P3T_ECUDA; }
     int rc = p3t_reserve(c, &c->info, sizeof(p3t_devinfo));
-    if (rc == P3T_OK) rc = p3t_tree_init(c);
     if (rc == P3T_OK) rc = p3t_walk_init(c);
     if (rc != P3T_OK) { p3t_destroy(c); return rc; }
     *out = c;

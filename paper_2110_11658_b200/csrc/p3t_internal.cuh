@@ -164,7 +164,6 @@ int p3t_launch_cube_keys(p3t_ctx* ctx, const float4* pos_mass);
 int p3t_launch_sort(p3t_ctx* ctx);
 int p3t_launch_permute(p3t_ctx* ctx, const float4* pos_mass);
 // p3t_tree.cu : a4-a6
-int p3t_tree_init(p3t_ctx* ctx);
 int p3t_launch_tree(p3t_ctx* ctx);
 // p3t_octupole.cu : SURVEY 8f NEXT-4, octupole variant
 int p3t_launch_octupoles(p3t_ctx* ctx);

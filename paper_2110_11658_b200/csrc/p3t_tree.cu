@@ -579,7 +579,6 @@ __global__ void __launch_bounds__(GC_THREADS) k_group_compact(tree_args A)
 }
 
 // ---------------------------------------------------------------------------------------------
-int p3t_tree_init(p3t_ctx* ctx) { (void)ctx; return P3T_OK; }
 
 int p3t_launch_tree(p3t_ctx* ctx)
 {
