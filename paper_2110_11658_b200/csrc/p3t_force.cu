@@ -672,7 +672,9 @@ static void force_fill(p3t_ctx* ctx, force_args& A, int mode, int evalall)
     A.n = (int)ctx->n; A.nbcnt = P<int32_t>(ctx->nbcnt); A.part = P<double>(ctx->part);
     // A problem with fewer work items (about 1.4 per 32 particles) than three per resident warp shares every item
     // among nseg warps (SPLIT), so that small N still fills the GPU.
-    const long long warps = (long long)ctx->occ_force * ctx->num_sms * FORCE_WARPS;
+    // (the nominal 4 CTAs per SM, not the occupancy ptxas happened to leave: nseg fixes the order of the partial sums,
+    // so the bits of the result must not move with the register count of a build -- the -DP3T_CHECKS build has 3)
+    const long long warps = 4ll * ctx->num_sms * FORCE_WARPS;
     const long long items = (long long)ctx->n / ctx->shard_nranks * 14 / 320 + 1;
     int nseg = 1;
     while (nseg < 8 && items * nseg < 3 * warps) nseg *= 2;
