@@ -326,12 +326,11 @@ def run_ours(args, w, rank, world, local_rank, dist):
     launches = t["launches"]
     ph = t["phases"]
 
-    # ---- the same step with the list walk and the force kernel one after the other (P3T_OVERLAP=0, read by p3t_create):
+    # ---- the same step with the list walk and the force kernel one after the other (p3t_diag_set_overlap, libp3t_diag.so):
     # the force kernel's duration with the SMs to itself, for the roofline ----
-    os.environ["P3T_OVERLAP"] = "0"
     with p3t.Context(local_rank) as cs:
+        pipebench.set_overlap(cs, False)
         ts = time_steps(torch, cs, pm_dev, out_dev, w, flush, min(args.steps, 5), 3)
-    del os.environ["P3T_OVERLAP"]
 
     # ---- SURVEY 8f NEXT-1 (outside the step): irregular force + jerk over the emitted lists ----
     vel_dev = torch.from_numpy(workloads.velocities_for(w)).to(dev)
@@ -444,7 +443,7 @@ def run_ours(args, w, rank, world, local_rank, dist):
         "kernel_note": "k_force as it runs in the timed step: beside the list walk (k_walk<LISTS> holds 1 CTA per SM for the first ~40 % of it), so its duration includes that competition",
         "kernel_alone": (lambda a, m: {"kernel_ms": m, "frac": a["frac"], "frac_sass_counts": a["frac_sass"],
                                        "ms_per_step": float(np.median(ts["step_ms"])), "ms_walk": float(np.median(ts["phases"]["ms_walk"])),
-                                       "note": "same step with P3T_OVERLAP=0: list walk, then the force kernel with the SMs to itself"})(
+                                       "note": "same step without the overlap (p3t_diag_set_overlap 0): list walk, then the force kernel with the SMs to itself"})(
             alu_fractions(ts["st"], float(np.median(ts["phases"]["ms_eval"])), sms, pk["sm_max_mhz"]), float(np.median(ts["phases"]["ms_eval"]))),
         "frac_at_observed_clock": (fr["achieved"] / (sms * 128 * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None,
     }

@@ -18,7 +18,7 @@ CSRC = PKG / "csrc"
 LIB = PKG / "libp3t.so"
 SOURCES = ["p3t_api.cu", "p3t_sort.cu", "p3t_tree.cu", "p3t_walk.cu", "p3t_force.cu", "p3t_irregular.cu", "p3t_core.cu", "p3t_shard.cu", "p3t_octupole.cu"]
 DIAG_LIB = PKG / "libp3t_diag.so"          # diagnostics (include/p3t_diag.h): its own library, not linked into libp3t.so
-DIAG_SOURCES = ["p3t_pipebench.cu"]
+DIAG_SOURCES = ["p3t_pipebench.cu", "p3t_diagknobs.cu"]
 HEADERS = [CSRC / "p3t_internal.cuh", CSRC / "p3t_cutoff.cuh", CSRC / "p3t_f32x2.cuh", ROOT / "include" / "p3t.h", ROOT / "include" / "p3t_diag.h"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -137,12 +137,12 @@ struct p3t_ctx {
     int32_t epoch;
     cudaStream_t walk_stream;        // created on first use (non-blocking)
     cudaEvent_t ev_tree, ev_scan, ev_wdone;
-    int overlap;                     // 1 (default): walkers and force kernel run concurrently; 0: one after the other (P3T_OVERLAP=0)
-    int walk_ctas_per_sm;            // CTAs per SM given to the list walk while the force kernel runs (P3T_WALK_CTAS, default 2: measured 9.03 vs 9.06 ms at config 3)
+    int overlap;                     // 1 (default): walkers and force kernel run concurrently; 0: one after the other (p3t_diag_set_overlap)
+    int walk_ctas_per_sm;            // CTAs per SM given to the list walk while the force kernel runs (p3t_diag_set_overlap, default 2: measured 9.03 vs 9.06 ms at config 3)
     int64_t nb_cap;                  // capacity of nbidx / the raw row buffer in entries (grow-only, from the previous call's total)
     int nb_max_hint;                 // longest row of the previous call (chooses the row-sort variant; any value is correct)
     p3t_pending pend;
-    int test_fault;                  // P3T_TEST_FAULT (tests only), bits: 1 = the force kernel gives up waiting at once, 2 = no walk-stack spill,
+    int test_fault;                  // p3t_diag_set_fault (tests only), bits: 1 = the force kernel gives up waiting at once, 2 = no walk-stack spill,
                                      // 4 = p3t_step_host meets a CUDA failure while its force call is in flight
 };
 

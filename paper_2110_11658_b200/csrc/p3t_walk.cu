@@ -44,7 +44,7 @@ struct walk_args {
     int n;                      // particles (P3T_CHECKS)
     int32_t* gready;            // WALK_LISTS: per-group list state (p3t_internal.cuh: G_READY ...)
     int base, repair;           // epoch of the call; repair = host repair pass (no force kernel is waiting)
-    int spill_cap;              // <= SPILL_CAP (smaller only under P3T_TEST_FAULT, to exercise the overflow report)
+    int spill_cap;              // <= SPILL_CAP (smaller only under p3t_diag_set_fault bit 2, to exercise the overflow report)
 };
 
 struct __align__(16) warp_smem {

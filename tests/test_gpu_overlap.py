@@ -24,6 +24,11 @@ def p3t():
     return m
 
 
+def _diag():
+    from paper_2110_11658_b200 import pipebench
+    return pipebench
+
+
 def _cuda(a):
     import torch
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
@@ -52,12 +57,12 @@ def _kicked_once(r, vel, half_dt):
 
 
 @pytest.mark.parametrize("overlap", ["1", "0"])
-def test_repair_after_undersized_buffers(p3t, monkeypatch, overlap):
+def test_repair_after_undersized_buffers(p3t, overlap):
     """A context sized by a tiny problem meets (a) a problem 20 x larger (list pools overflow: failed groups are
     redone) and (b) a dense King core with a long search radius (the neighbour total outgrows the index buffer: no row is
     emitted in the first pass, every group is evaluated again without a second kick).  Both with and without
     the walk / force overlap."""
-    monkeypatch.setenv("P3T_OVERLAP", overlap)
+    ov = overlap == "1"                                       # set on every context below (libp3t_diag.so)
     small = workloads.make_config(1, n_override=3000)
     big = workloads.make_config(2, n_override=60000, theta=0.3)
     king = workloads.make_config(4, n_override=50000)
@@ -66,10 +71,12 @@ def test_repair_after_undersized_buffers(p3t, monkeypatch, overlap):
     for w in (big, king):
         vel = workloads.velocities_for(w)
         with p3t.Context(0) as ref_ctx:
+            _diag().set_overlap(ref_ctx, ov)
             _run(ref_ctx, w, vel, half_dt)                   # first call of a fresh context (its own repair, if any)
             ref = _run(ref_ctx, w, vel, half_dt)             # second call: buffers fit, nothing is repaired
         _kicked_once(ref, vel, half_dt)
         with p3t.Context(0) as ctx:
+            _diag().set_overlap(ctx, ov)
             _run(ctx, small, workloads.velocities_for(small), half_dt)
             got = _run(ctx, w, vel, half_dt)                 # outgrows the pools / index buffers of the small problem
             _same(got, ref)
@@ -81,8 +88,8 @@ def test_repair_after_undersized_buffers(p3t, monkeypatch, overlap):
     assert np.array_equal(ooff, ref["off"]) and np.array_equal(oidx, ref["idx"])
 
 
-def test_force_warps_that_stop_waiting(p3t, monkeypatch):
-    """P3T_TEST_FAULT=1: every force warp gives up at once on a group whose lists are not there yet (what the
+def test_force_warps_that_stop_waiting(p3t):
+    """Fault bit 1 (p3t_diag_set_fault): every force warp gives up at once on a group whose lists are not there yet (what the
     time-out does when no walker is resident): those groups are marked failed and redone by the repair pass."""
     w = workloads.make_config(2, n_override=80000)
     vel = workloads.velocities_for(w)
@@ -90,20 +97,21 @@ def test_force_warps_that_stop_waiting(p3t, monkeypatch):
     with p3t.Context(0) as ctx:
         _run(ctx, w, vel, half_dt)
         ref = _run(ctx, w, vel, half_dt)
-    monkeypatch.setenv("P3T_TEST_FAULT", "1")
     with p3t.Context(0) as ctx:
+        _diag().set_fault(ctx, 1)
         for _ in range(2):
             got = _run(ctx, w, vel, half_dt)
             _same(got, ref)
             _kicked_once(got, vel, half_dt)
+            assert got["st"]["force_flags"] & p3t.FF_REPAIRED
     T = oracle.Tree(w.pos_mass, 63, 16, 64)
     f = T.force(w.r_out, w.r_in, w.theta, 0)
     assert np.linalg.norm(ref["a"][:, :3] - f["acc_pot"][:, :3]) <= 1e-6 * np.linalg.norm(f["acc_pot"][:, :3])
 
 
-def test_repair_keeps_the_octupole_term_of_finished_groups(p3t, monkeypatch):
+def test_repair_keeps_the_octupole_term_of_finished_groups(p3t):
     """Order 3 at small N (every work item shared by several warps, so the sums go through k_force_final) with
-    P3T_TEST_FAULT=1: some groups are complete after the first pass, the others are redone.  The repair pass must leave
+    fault bit 1: some groups are complete after the first pass, the others are redone.  The repair pass must leave
     the finished groups alone -- their result already carries the octupole term, which the repair adds only to the
     groups it redoes -- so that acceleration and kicked velocity are those of an undisturbed call, bit for bit."""
     w = workloads.make_config(1, n_override=20000)
@@ -116,8 +124,8 @@ def test_repair_keeps_the_octupole_term_of_finished_groups(p3t, monkeypatch):
     with p3t.Context(0) as ctx:
         quad = _run(ctx, w, vel, half_dt)
     assert np.mean(ref["a"][:, :3] != quad["a"][:, :3]) > 0.5          # the octupole term is really there
-    monkeypatch.setenv("P3T_TEST_FAULT", "1")
     with p3t.Context(0) as ctx:
+        _diag().set_fault(ctx, 1)
         ctx.set_multipole_order(3)
         for _ in range(2):
             got = _run(ctx, w, vel, half_dt)
@@ -128,9 +136,9 @@ def test_repair_keeps_the_octupole_term_of_finished_groups(p3t, monkeypatch):
     assert np.all(np.abs(ref["v"][:, :3] - want) <= 4e-7 * (np.abs(want) + half_dt * np.abs(a)) + 1e-30)
 
 
-def test_walk_stack_overflow_is_a_condition_of_one_call(p3t, monkeypatch):
+def test_walk_stack_overflow_is_a_condition_of_one_call(p3t):
     """theta may change between calls without a rebuild (include/p3t.h): after a call whose wide-open walk overflowed
-    the walk stack (P3T_ECUDA; P3T_TEST_FAULT=2 takes the spill space away so that 384 entries are all there is), a
+    the walk stack (P3T_ECUDA; fault bit 2 takes the spill space away so that 384 entries are all there is), a
     call on the SAME tree with a theta whose walk fits works, and gives what a fresh context gives."""
     w = workloads.make_config(1, n_override=20000)
     pm = _cuda(w.pos_mass)
@@ -138,8 +146,8 @@ def test_walk_stack_overflow_is_a_condition_of_one_call(p3t, monkeypatch):
         ctx.build_tree(pm, 63)
         ref = ctx.regular_force(w.r_out, w.r_in, 1.0, 0).cpu().numpy()
         roff, ridx = [x.cpu().numpy() for x in ctx.neighbours()]
-    monkeypatch.setenv("P3T_TEST_FAULT", "2")
     with p3t.Context(0) as ctx:
+        _diag().set_fault(ctx, 2)
         ctx.build_tree(pm, 63)
         with pytest.raises(p3t.P3TError) as e:
             ctx.regular_force(w.r_out, w.r_in, 1e-3, 0)
@@ -150,19 +158,18 @@ def test_walk_stack_overflow_is_a_condition_of_one_call(p3t, monkeypatch):
         assert np.array_equal(off, roff) and np.array_equal(idx, ridx)
 
 
-def test_capacity_error_comes_from_the_force_call(p3t, monkeypatch):
-    """P3T_TEST_FAULT=2 removes the spill space of the walk stack: a wide-open walk (theta -> 0) overflows it, and
+def test_capacity_error_comes_from_the_force_call(p3t):
+    """Fault bit 2 removes the spill space of the walk stack: a wide-open walk (theta -> 0) overflows it, and
     p3t_regular_force itself returns P3T_ECUDA (not a later accessor); NaN input is reported by it too, and the
     velocities are not kicked in that case."""
     import torch
     w = workloads.make_config(1, n_override=20000)
-    monkeypatch.setenv("P3T_TEST_FAULT", "2")
     with p3t.Context(0) as ctx:
+        _diag().set_fault(ctx, 2)
         ctx.build_tree(_cuda(w.pos_mass), 63)
         with pytest.raises(p3t.P3TError) as e:
             ctx.regular_force(w.r_out, w.r_in, 1e-3, 0)
         assert e.value.code == p3t.ECUDA and "stack_overflow" in str(e.value)
-    monkeypatch.delenv("P3T_TEST_FAULT")
     with p3t.Context(0) as ctx:
         bad = w.pos_mass.copy(); bad[17, 2] = np.nan
         ctx.build_tree(_cuda(bad), 63)
@@ -299,20 +306,19 @@ def test_begin_wait_is_the_blocking_call_in_two_halves(p3t):
         _same(got, ref)
 
 
-def test_failed_step_host_gives_the_overlap_slot_back(p3t, monkeypatch):
-    """A CUDA failure inside p3t_step_host after the force call has been enqueued (P3T_TEST_FAULT=4 injects one) is
+def test_failed_step_host_gives_the_overlap_slot_back(p3t):
+    """A CUDA failure inside p3t_step_host after the force call has been enqueued (fault bit 4 injects one) is
     reported, the context is drained, and the per-device overlap slot is free again: the next context still runs the
     walk beside the force kernel (it used to fall back to the serial order for the rest of the process)."""
     w = workloads.make_config(1, n_override=50000)
     pm_host = np.ascontiguousarray(w.pos_mass)
-    monkeypatch.setenv("P3T_TEST_FAULT", "4")
     with p3t.Context(0) as ctx:
+        _diag().set_fault(ctx, 4)
         with pytest.raises(p3t.P3TError) as e:
             ctx.step_host(pm_host, w.r_out, w.r_in, w.theta, nb_offsets=np.empty(w.n + 1, np.int64))
         assert e.value.code == p3t.ECUDA
         with pytest.raises(p3t.P3TError):                         # a CUDA failure is sticky for its context
             ctx.build_tree(_cuda(w.pos_mass), 63)
-    monkeypatch.delenv("P3T_TEST_FAULT")
     with p3t.Context(0) as ctx:
         ctx.build_tree(_cuda(w.pos_mass), 63)
         ctx.regular_force(w.r_out, w.r_in, w.theta, 0)
