@@ -61,10 +61,13 @@ def peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+TRAFFIC_CSV = "r03_traffic.csv"                            # ncu --set full capture of the round's final build (profiles/r03_traffic.md)
+
+
 def ncu_traffic(workload: str, kernel: str = "k_force"):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r02_traffic.csv:
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r03_traffic.csv:
     workload, kernel, dram_bytes_read, dram_bytes_write), or None when there is no row for this workload."""
-    p = ROOT / "profiles" / "r02_traffic.csv"
+    p = ROOT / "profiles" / TRAFFIC_CSV
     if not p.exists():
         return None
     with p.open() as f:
@@ -284,6 +287,7 @@ def config_summary(cfg: int, w, t: dict, sms: int, pk: dict) -> dict:
         "pp_per_particle": st["n_pp"] / n, "pc_per_particle": st["n_pc"] / n,
         "frac_alu_survey_counts": fr["frac"], "frac_alu_sass_counts": fr["frac_sass"],
         "work_vs_survey": (mine / surv) if surv else None,
+        "frac_vs_survey_work": (fr["frac"] / (mine / surv)) if surv else None,
         "build_gbs": 354.0 * n / (ph["ms_build"] * 1e-3) / 1e9, "build_frac_hbm": 354.0 * n / (ph["ms_build"] * 1e-3) / 1e9 / pk["hbm_gbs"],
         "nodes": st["n_nodes"], "groups": st["n_groups"], "neighbours_total": st["nb_total"], "neighbours_max": st["nb_max"],
         "gpu_launches_per_step": t["launches"] / len(t["step_ms"]),
@@ -423,6 +427,8 @@ def run_ours(args, w, rank, world, local_rank, dist):
     peak_meas = pipes["fp32_lane_instr_per_s"] / 1e12
     surv = SURVEY_INSTR_PER_PARTICLE.get((args.config, round(w.theta, 2))) if args.n is None else None
     mine = (INSTR_PP * st["n_pp"] + INSTR_PC * st["n_pc"]) / n
+    alone_ms = float(np.median(ts["phases"]["ms_eval"]))
+    alone = alu_fractions(ts["st"], alone_ms, sms, pk["sm_max_mhz"])
     roofline = {
         "bound": "alu", "kernel": "k_force (p-c / p-p force + cutoff + neighbour emission over the interaction lists)",
         "achieved": fr["achieved"], "peak": fr["peak"], "unit": "Tinstr/s (FP32 lane-instructions)", "frac": fr["frac"],
@@ -433,13 +439,16 @@ def run_ours(args, w, rank, world, local_rank, dist):
         "work_vs_survey_note": ("FP32 instructions per particle of this run (15 pp + 37 pc, NCRIT 64 sibling-run groups) over SURVEY 8(d)'s table "
                                 "(NCRIT 32 canonical groups): the extra interactions that `achieved` credits as useful"),
         "frac_vs_survey_work": (fr["frac"] / (mine / surv)) if surv else None,
-        "traffic": ncu_traffic(w.name), "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full; profiles/r02_traffic.csv)",
+        "traffic": ncu_traffic(w.name), "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full; profiles/" + TRAFFIC_CSV + ")",
         "peak_source": f"{sms} SMs x 128 FP32 lanes x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
         "achieved_tflops": (FLOP_PP * st["n_pp"] + FLOP_PC * st["n_pc"]) / (wms * 1e-3) / 1e12,
         "peak_measured": peak_meas, "frac_of_measured": fr["achieved"] / peak_meas,
         "peak_measured_source": "p3t_diag_pipe_bench: FFMA chain, 32 lanes / %.3f cycles per SM sub-partition" % pipes["cycles"]["FFMA (reuse cache)"],
         "pipe_cycles": pipes["cycles"],
         "kernel_ms": wms, "kernel_share_of_step": wms * args.steps / total_ms,
+        # the two kernel numbers side by side: beside the list walk (the step as it runs) and with the SMs to itself
+        "kernel_ms_beside_walk": wms, "frac_beside_walk": fr["frac"], "frac_sass_beside_walk": fr["frac_sass"],
+        "kernel_ms_alone": alone_ms, "frac_alone": alone["frac"], "frac_sass_alone": alone["frac_sass"],
         "kernel_note": "k_force as it runs in the timed step: beside the list walk (k_walk<LISTS> holds 1 CTA per SM for the first ~40 % of it), so its duration includes that competition",
         "kernel_alone": (lambda a, m: {"kernel_ms": m, "frac": a["frac"], "frac_sass_counts": a["frac_sass"],
                                        "ms_per_step": float(np.median(ts["step_ms"])), "ms_walk": float(np.median(ts["phases"]["ms_walk"])),

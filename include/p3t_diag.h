@@ -12,7 +12,8 @@ extern "C" {
 
 /* cycles_out: HOST double[n_out >= 8], SM-clock cycles per SM sub-partition of: [0] FFMA (best case: operands in
  * the reuse cache), [1] FFMA2 with two distinct register pairs, [2] FFMA2 with three, [3] FMUL2, [4] one FMUL2 + one
- * FFMA, [5] eight FMUL2 + two MUFU.RSQ, [6] MUFU.RSQ, [7] FFMA with three distinct registers.  sm_clock_mhz /
+ * FFMA, [5] eight FMUL2 + two MUFU.RSQ, [6] MUFU.RSQ, [7] FFMA with three distinct registers, and, if n_out >= 9, [8] FFMA2 with three distinct register pairs one of
+ * which is the same in consecutive instructions.  sm_clock_mhz /
  * num_sms: HOST, may be NULL (the device's nominal maximum clock, which the cycle counts assume).
  * Returns 0, -1 (bad argument), -3 (allocation) or -4 (CUDA failure).  Synchronises the device; ~20 ms. */
 int p3t_diag_pipe_bench(int device, double* cycles_out, int n_out, double* sm_clock_mhz, int* num_sms);

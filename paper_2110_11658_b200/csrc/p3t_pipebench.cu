@@ -18,6 +18,8 @@ __device__ __forceinline__ float vrsq(float x) { float y; asm volatile("rsqrt.ap
 //      2: FFMA2, three distinct register pairs     3: FMUL2
 //      4: FMUL2 + FFMA alternating (per pair)      5: 8 FMUL2 + 2 MUFU.RSQ (per group of 10)
 //      6: MUFU.RSQ alone                            7: FFMA, three distinct registers (bank conflicts as allocated)
+//      8: FFMA2, three distinct register pairs of which one is the SAME in consecutive instructions (what two targets per
+//         lane would give the p-c loop: q . d_A, q . d_B share the cell operand, so the reuse cache can serve it)
 template <int MODE> __global__ void __launch_bounds__(256) k_pipe(float* out, int iters, float s)
 {
     f2 a[8], b[8], c[8]; float t[8], u[8], v[8];
@@ -32,6 +34,7 @@ template <int MODE> __global__ void __launch_bounds__(256) k_pipe(float* out, in
             if (MODE == 7) t[i] = vfma1(u[i], v[i], t[i]);
             if (MODE == 1) c[i] = vfma2(a[i], a[i], c[i]);
             if (MODE == 2) c[i] = vfma2(a[i], b[i], c[i]);
+            if (MODE == 8) c[i] = vfma2(a[i], b[0], c[i]);
             if (MODE == 3) c[i] = vmul2(c[i], b[i]);
             if (MODE == 4) { c[i] = vmul2(c[i], b[i]); t[i] = vfma1(t[i], s, s); }
             if (MODE == 5) { c[i] = vmul2(c[i], b[i]); if ((i & 3) == 0) t[i] = vrsq(t[i]); }
@@ -75,10 +78,12 @@ extern "C" int p3t_diag_pipe_bench(int device, double* cycles_out, int n_out, do
     ms[2] = time_mode<2>(d, blocks, iters, e0, e1); ms[3] = time_mode<3>(d, blocks, iters, e0, e1);
     ms[4] = time_mode<4>(d, blocks, iters, e0, e1); ms[5] = time_mode<5>(d, blocks, iters, e0, e1);
     ms[6] = time_mode<6>(d, blocks, iters, e0, e1); ms[7] = time_mode<7>(d, blocks, iters, e0, e1);
+    const float ms8 = time_mode<8>(d, blocks, iters, e0, e1);
     // per SM sub-partition: bps * 8 warps / 4 sub-partitions = 4 warps, each 8 instruction groups per iteration
     const double groups = (double)iters * 8.0 * (bps * 2);
     for (int k = 0; k < 8; ++k) cycles_out[k] = (double)ms[k] * 1e-3 * (double)khz * 1e3 / groups;
     cycles_out[5] *= 8.0;                                       // mode 5: cycles per group of 8 FMUL2 + 2 MUFU.RSQ
+    if (n_out >= 9) cycles_out[8] = (double)ms8 * 1e-3 * (double)khz * 1e3 / groups;
     if (sm_clock_mhz) *sm_clock_mhz = khz * 1e-3;
     if (num_sms) *num_sms = sms;
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);

@@ -9,7 +9,8 @@ from pathlib import Path
 DIAG_PATH = Path(__file__).resolve().parent / "libp3t_diag.so"
 DIAG_SYMBOLS = ["p3t_diag_pipe_bench", "p3t_diag_set_overlap", "p3t_diag_set_fault"]
 LABELS = ["FFMA (reuse cache)", "FFMA2, 2 distinct register pairs", "FFMA2, 3 distinct register pairs", "FMUL2",
-          "FMUL2 + FFMA (pair)", "8 FMUL2 + 2 MUFU.RSQ (group)", "MUFU.RSQ", "FFMA, 3 distinct registers"]
+          "FMUL2 + FFMA (pair)", "8 FMUL2 + 2 MUFU.RSQ (group)", "MUFU.RSQ", "FFMA, 3 distinct registers",
+          "FFMA2, 3 distinct register pairs, one shared with the previous instruction"]
 _lib = None
 
 
@@ -43,8 +44,8 @@ def set_fault(ctx, bits: int) -> None:
 def pipe_bench(device: int = 0) -> dict:
     """Cycles per SM sub-partition for each instruction pattern, and the FP32 lane-instruction peak they imply
     (32 lanes / cycles[FFMA] per sub-partition)."""
-    out = (C.c_double * 8)(); mhz = C.c_double(); sms = C.c_int()
-    rc = lib().p3t_diag_pipe_bench(device, out, 8, C.byref(mhz), C.byref(sms))
+    out = (C.c_double * 9)(); mhz = C.c_double(); sms = C.c_int()
+    rc = lib().p3t_diag_pipe_bench(device, out, 9, C.byref(mhz), C.byref(sms))
     if rc != 0:
         raise RuntimeError(f"p3t_diag_pipe_bench failed ({rc})")
     cyc = [float(x) for x in out]
